@@ -1,0 +1,304 @@
+"""Float64 CPU oracle for the fused GRPO policy-loss step.
+
+TEST INFRASTRUCTURE ONLY.  Nothing in the product path (``paper_2606_26997_b200``)
+imports this module; only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py`` may call it.  It shares
+no code, tables or helpers with the CUDA path.
+
+What it computes is the *plain definition* of the step:
+the method reaches an exactly defined result, so there is no tiling, no online
+log-sum-exp and no fusion here.  Logits ARE materialised (in token chunks, only to
+bound memory).  All arithmetic is float64; bf16 inputs are widened exactly.
+
+Passages followed:
+  * group advantage ............ Eq. 1, PAPER.md:86-90 (sigma reading: DESIGN.md R1-R4)
+  * one advantage per response, broadcast over its tokens + loss mask ... PAPER.md:40
+  * clipped surrogate with current/old ratios ...... PAPER.md:38 (form: north_star)
+  * k3 KL, masked token mean, backward (softmax - onehot) * coeff ...... north_star
+  * gradients only accumulated across groups of a logical update ..... PAPER.md:111
+
+Pins (tests/test_oracle_pins.py): P1-P14 of SURVEY.md §8(c).  The paper prints no
+worked number for the loss, so every pin is a closed form, invariant, library special
+case, finite difference or brute force.  Unpinned by the paper: everything except
+Eq. 1 — pinned here by P4-P14 only.  ``metrics`` (clip fraction etc.) are checked
+against brute-force loops only: "parity unpinned" beyond that.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+__all__ = [
+    "OracleConfig", "bf16_bits_to_f64", "group_advantage", "token_advantage",
+    "token_logprobs", "loss_terms", "backward", "grpo_step", "grpo_step_loops",
+]
+
+
+@dataclass
+class OracleConfig:
+    eps_std: float = 1e-6        # Eq. 1 stabiliser ("a small stabilizer")
+    std_ddof: int = 0            # 0 population std (default reading), 1 sample std
+    clip_lo: float = 0.2
+    clip_hi: float = 0.28
+    kl_beta: float = 0.0         # 0 disables the k3 term
+    loss_agg: int = 0            # 0 token mean over the logical update, 1 per-sequence mean
+    logit_scale: float = 1.0     # 1 / temperature
+    chunk_tokens: int = 1024     # memory bound only; results do not depend on it
+
+
+def bf16_bits_to_f64(bits: np.ndarray) -> np.ndarray:
+    """uint16 bf16 bit patterns -> float64, exactly (bf16 is the top half of an fp32)."""
+    bits = np.ascontiguousarray(bits, dtype=np.uint16)
+    return (bits.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+# --------------------------------------------------------------------------- step 1
+def group_advantage(rewards, cu_groups=None, G=None, eps_std=1e-6, ddof=0):
+    """Eq. 1:  A_i = (r_i - mu_group) / (sigma_group + eps_std).
+
+    ``cu_groups`` [n_groups+1] gives ragged group boundaries; otherwise groups are
+    uniform of size ``G``.  sigma uses divisor (G - ddof); if that is <= 0, sigma = 0.
+    Returns (adv float64 [S], zero_var bool [n_groups]).
+    """
+    r = np.asarray(rewards, dtype=np.float64)
+    if cu_groups is None:
+        assert G is not None and r.size % G == 0
+        cu = np.arange(0, r.size + 1, G, dtype=np.int64)
+    else:
+        cu = np.asarray(cu_groups, dtype=np.int64)
+    adv = np.zeros_like(r)
+    zero_var = np.zeros(cu.size - 1, dtype=bool)
+    for g in range(cu.size - 1):
+        rg = r[cu[g]:cu[g + 1]]
+        n = rg.size
+        if n == 0:
+            zero_var[g] = True
+            continue
+        mu = rg.sum() / n
+        dev = rg - mu
+        div = n - ddof
+        sigma = np.sqrt((dev * dev).sum() / div) if div > 0 else 0.0
+        adv[cu[g]:cu[g + 1]] = dev / (sigma + eps_std)
+        zero_var[g] = bool(sigma == 0.0)
+    return adv, zero_var
+
+
+# --------------------------------------------------------------------------- step 2
+def token_advantage(adv, cu_seqlens):
+    """A_t = A_seq(t): one advantage per response, broadcast to its tokens."""
+    cu = np.asarray(cu_seqlens, dtype=np.int64)
+    return np.repeat(np.asarray(adv, dtype=np.float64), np.diff(cu))
+
+
+# ----------------------------------------------------------------------- steps 3, 4
+def token_logprobs(H, W, y, logit_scale=1.0, chunk_tokens=1024):
+    """z = s * H W^T ; lse_t = m + log sum_v exp(z_tv - m) ; logp_t = z_t[y_t] - lse_t.
+
+    Tokens with y_t < 0 or y_t >= V are ignored (R13): logp = lse-only
+    bookkeeping, ``zy`` taken as 0 and ``logp`` reported as 0.
+    Returns (lse, logp) float64 [T].
+    """
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    y = np.asarray(y, dtype=np.int64)
+    T, V = H.shape[0], W.shape[0]
+    lse = np.zeros(T)
+    logp = np.zeros(T)
+    valid = (y >= 0) & (y < V)
+    for t0 in range(0, T, chunk_tokens):
+        t1 = min(T, t0 + chunk_tokens)
+        z = logit_scale * (H[t0:t1] @ W.T)                       # [Tc, V] materialised
+        m = z.max(axis=1)
+        l = m + np.log(np.exp(z - m[:, None]).sum(axis=1))
+        lse[t0:t1] = l
+        yy = np.where(valid[t0:t1], y[t0:t1], 0)
+        zy = z[np.arange(t1 - t0), yy]
+        logp[t0:t1] = np.where(valid[t0:t1], zy - l, 0.0)
+    return lse, logp
+
+
+# ---------------------------------------------------------------------- steps 5 - 9a
+def loss_terms(logp, old_logp, ref_logp, mask, adv_tok, cu_seqlens, cfg: OracleConfig,
+               loss_denom=None, valid=None):
+    """Per-token surrogate, k3, weights, loss, and c_t = d loss / d logp_t.
+
+    rho = exp(logp - old);  s = min(rho A, clip(rho, 1-eps_lo, 1+eps_hi) A)
+    delta = ref - logp;     k3 = exp(delta) - delta - 1
+    l_t = -s_t + beta k3_t; loss = sum_t w_t l_t
+    mode 0: w_t = m_t / denom, denom = max(sum m, 1) unless ``loss_denom`` given
+    mode 1: w_t = m_t / (max(sum_{t' in seq(t)} m_t', 1) * S)
+    u_t = 0 iff (A>0 and rho > 1+eps_hi) or (A<0 and rho < 1-eps_lo)   [bounds inclusive]
+    c_t = w_t [ -A rho u + beta (1 - exp(ref - logp)) ]
+    """
+    logp = np.asarray(logp, dtype=np.float64)
+    old = np.asarray(old_logp, dtype=np.float64)
+    A = np.asarray(adv_tok, dtype=np.float64)
+    T = logp.size
+    cu = np.asarray(cu_seqlens, dtype=np.int64)
+    S = cu.size - 1
+    m = np.ones(T) if mask is None else (np.asarray(mask) != 0).astype(np.float64)
+    if valid is not None:
+        m = m * np.asarray(valid, dtype=np.float64)
+    if cfg.loss_agg == 0:
+        denom = max(m.sum(), 1.0) if (loss_denom is None or loss_denom <= 0) else float(loss_denom)
+        w = m / denom
+    else:
+        w = np.zeros(T)
+        for s in range(S):
+            ms = m[cu[s]:cu[s + 1]]
+            w[cu[s]:cu[s + 1]] = ms / (max(ms.sum(), 1.0) * S)
+    rho = np.exp(logp - old)
+    lo, hi = 1.0 - cfg.clip_lo, 1.0 + cfg.clip_hi
+    surr = np.minimum(rho * A, np.clip(rho, lo, hi) * A)
+    use_kl = cfg.kl_beta != 0.0 and ref_logp is not None
+    if use_kl:
+        delta = np.asarray(ref_logp, dtype=np.float64) - logp
+        k3 = np.exp(delta) - delta - 1.0
+        dk3 = 1.0 - np.exp(delta)                      # d k3 / d logp
+    else:
+        k3 = np.zeros(T)
+        dk3 = np.zeros(T)
+    ell = -surr + cfg.kl_beta * k3
+    clipped = ((A > 0) & (rho > hi)) | ((A < 0) & (rho < lo))
+    u = np.where(clipped, 0.0, 1.0)
+    coeff = w * (-A * rho * u + cfg.kl_beta * dk3)
+    # w == 0 tokens (masked / invalid) contribute exact zeros even if ell is inf/nan-free
+    ell_w = np.where(w != 0.0, w * ell, 0.0)
+    coeff = np.where(w != 0.0, coeff, 0.0)
+    loss = ell_w.sum()
+    metrics = np.array([
+        m.sum(),                                   # [0] loss-bearing tokens
+        (m * rho).sum(),                           # [1] sum of rho over them
+        (m * k3).sum(),                            # [2] sum of k3 over them
+        (m * clipped).sum(),                       # [3] tokens whose policy gradient is clipped away
+    ])
+    return dict(rho=rho, surr=surr, k3=k3, ell=ell, w=w, coeff=coeff, loss=loss,
+                abs_loss=np.abs(ell_w).sum(), metrics=metrics, u=u)
+
+
+# --------------------------------------------------------------------------- step 9b
+def backward(H, W, y, lse, coeff, logit_scale=1.0, chunk_tokens=1024, grad_scale=1.0):
+    """p = exp(z - lse);  dz_tv = c_t (1[v = y_t] - p_tv);  dH = s dz W;  dW = s dz^T H.
+
+    ("(softmax - onehot) * coeff" of north_star with coeff = -c_t.)
+    """
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    y = np.asarray(y, dtype=np.int64)
+    c = np.asarray(coeff, dtype=np.float64) * grad_scale
+    T, V = H.shape[0], W.shape[0]
+    dH = np.zeros_like(H)
+    dW = np.zeros_like(W)
+    valid = (y >= 0) & (y < V)
+    for t0 in range(0, T, chunk_tokens):
+        t1 = min(T, t0 + chunk_tokens)
+        z = logit_scale * (H[t0:t1] @ W.T)
+        p = np.exp(z - np.asarray(lse, dtype=np.float64)[t0:t1, None])
+        dz = -p
+        rows = np.arange(t1 - t0)[valid[t0:t1]]
+        dz[rows, y[t0:t1][valid[t0:t1]]] += 1.0
+        dz *= c[t0:t1, None]
+        dH[t0:t1] = logit_scale * (dz @ W)
+        dW += logit_scale * (dz.T @ H[t0:t1])
+    return dH, dW
+
+
+# ------------------------------------------------------------------------ whole step
+def grpo_step(H, W, y, cu_seqlens, rewards, old_logp, ref_logp=None, mask=None,
+              cfg: OracleConfig | None = None, G=None, cu_groups=None, loss_denom=None,
+              adv=None, need_grads=True, grad_scale=1.0):
+    """Steps 1-9 in order.  ``adv`` may be given directly (skips step 1)."""
+    cfg = cfg or OracleConfig()
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    y = np.asarray(y, dtype=np.int64)
+    V = W.shape[0]
+    zero_var = None
+    if adv is None:
+        adv, zero_var = group_advantage(rewards, cu_groups=cu_groups, G=G,
+                                        eps_std=cfg.eps_std, ddof=cfg.std_ddof)
+    A_tok = token_advantage(adv, cu_seqlens)
+    lse, logp = token_logprobs(H, W, y, cfg.logit_scale, cfg.chunk_tokens)
+    valid = (y >= 0) & (y < V)
+    lt = loss_terms(logp, old_logp, ref_logp, mask, A_tok, cu_seqlens, cfg,
+                    loss_denom=loss_denom, valid=valid)
+    out = dict(adv=np.asarray(adv, dtype=np.float64), zero_var=zero_var, lse=lse, logp=logp, **lt)
+    if need_grads:
+        dH, dW = backward(H, W, y, lse, lt["coeff"], cfg.logit_scale, cfg.chunk_tokens, grad_scale)
+        out["dH"], out["dW"] = dH, dW
+    return out
+
+
+def grpo_step_loops(H, W, y, cu_seqlens, rewards, old_logp, ref_logp=None, mask=None,
+                    cfg: OracleConfig | None = None, G=None, loss_denom=None):
+    """The same definition with explicit Python loops (tiny shapes only).
+
+    Independent of the numpy-vectorised path above except for ``math``: used to check
+    ``grpo_step`` against.
+    """
+    import math
+    cfg = cfg or OracleConfig()
+    T, d = len(H), len(H[0])
+    V = len(W)
+    S = len(cu_seqlens) - 1
+    n_groups = S // G
+    adv = [0.0] * S
+    for g in range(n_groups):
+        rs = [float(rewards[g * G + i]) for i in range(G)]
+        mu = sum(rs) / G
+        div = G - cfg.std_ddof
+        sigma = math.sqrt(sum((r - mu) ** 2 for r in rs) / div) if div > 0 else 0.0
+        for i in range(G):
+            adv[g * G + i] = (rs[i] - mu) / (sigma + cfg.eps_std)
+    seq_of = [0] * T
+    for s in range(S):
+        for t in range(cu_seqlens[s], cu_seqlens[s + 1]):
+            seq_of[t] = s
+    mk = [1.0 if (mask is None or mask[t]) else 0.0 for t in range(T)]
+    for t in range(T):
+        if y[t] < 0 or y[t] >= V:
+            mk[t] = 0.0
+    if cfg.loss_agg == 0:
+        denom = max(sum(mk), 1.0) if (loss_denom is None or loss_denom <= 0) else float(loss_denom)
+        w = [mk[t] / denom for t in range(T)]
+    else:
+        cnt = [max(sum(mk[cu_seqlens[s]:cu_seqlens[s + 1]]), 1.0) for s in range(S)]
+        w = [mk[t] / (cnt[seq_of[t]] * S) for t in range(T)]
+    logp = [0.0] * T
+    lse = [0.0] * T
+    z = [[cfg.logit_scale * sum(float(W[v][k]) * float(H[t][k]) for k in range(d))
+          for v in range(V)] for t in range(T)]
+    loss = 0.0
+    coeff = [0.0] * T
+    lo, hi = 1.0 - cfg.clip_lo, 1.0 + cfg.clip_hi
+    for t in range(T):
+        mx = max(z[t])
+        lse[t] = mx + math.log(sum(math.exp(zv - mx) for zv in z[t]))
+        if mk[t] == 0.0 and (y[t] < 0 or y[t] >= V):
+            continue
+        logp[t] = z[t][y[t]] - lse[t]
+        A = adv[seq_of[t]]
+        rho = math.exp(logp[t] - float(old_logp[t]))
+        surr = min(rho * A, min(max(rho, lo), hi) * A)
+        k3 = dk3 = 0.0
+        if cfg.kl_beta != 0.0 and ref_logp is not None:
+            delta = float(ref_logp[t]) - logp[t]
+            k3 = math.exp(delta) - delta - 1.0
+            dk3 = 1.0 - math.exp(delta)
+        clipped = (A > 0 and rho > hi) or (A < 0 and rho < lo)
+        if w[t] != 0.0:
+            loss += w[t] * (-surr + cfg.kl_beta * k3)
+            coeff[t] = w[t] * (-A * rho * (0.0 if clipped else 1.0) + cfg.kl_beta * dk3)
+    dH = [[0.0] * d for _ in range(T)]
+    dW = [[0.0] * d for _ in range(V)]
+    for t in range(T):
+        if coeff[t] == 0.0:
+            continue
+        for v in range(V):
+            dz = coeff[t] * ((1.0 if v == y[t] else 0.0) - math.exp(z[t][v] - lse[t]))
+            for k in range(d):
+                dH[t][k] += cfg.logit_scale * dz * float(W[v][k])
+                dW[v][k] += cfg.logit_scale * dz * float(H[t][k])
+    return dict(adv=np.array(adv), lse=np.array(lse), logp=np.array(logp), loss=loss,
+                coeff=np.array(coeff), dH=np.array(dH), dW=np.array(dW))
