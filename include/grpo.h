@@ -1,0 +1,187 @@
+/*
+ * grpo.h — C ABI of the B200 (sm_100a) fused GRPO policy-loss step.
+ *
+ * The trainer-side hot path that RolloutPipe's complete-group pipelining (CGP) feeds
+ * (arxiv/paper_2606_26997; citations are PAPER.md line numbers):
+ *
+ *   A0  CGP handoff: FIFO of complete groups, feasible prefix under a token budget, dispatch in
+ *       logical updates of U groups                       PAPER.md:92, 111, 187; Alg. 1 l.16-22
+ *   A1  group-relative advantage  A_i = (r_i - mu_g)/(sigma_g + eps_std)      Eq. 1
+ *   A2  LM-head contraction + online log-sum-exp + target gather  -> logp_t    ("Megatron executes
+ *       forward"; definition: BASELINE.json north_star)
+ *   A3  clipped importance-ratio surrogate + optional k3 KL + masked mean (loss mask,
+ *       PAPER.md:40)
+ *   A4-A6 backward: recompute logits chunk, dZ = c_t (1[v=y_t] - p_tv), dH = dZ W, dW += dZ^T H
+ *   A7  gradients / loss only ever ACCUMULATE until the caller's optimizer boundary
+ *
+ * Conventions
+ *   - Every function returns a grpo_status (int32).  No exception crosses the ABI.
+ *     grpo_last_error() gives a thread-local message for the last non-OK status on this thread.
+ *   - Unless a parameter says HOST, tensor pointers are DEVICE pointers owned by the caller and must
+ *     stay valid until the stream reaches the work of the call.  The library owns only its context.
+ *   - No function synchronises the host with the device unless its name ends in _sync or _host.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - Layouts: hidden bf16 [T, d] row-major; W bf16 [V, d] row-major; dW fp32 [V, d] row-major;
+ *     per-token arrays are [T] over the PACKED token stream; cu_seqlens int32 [S+1] gives sequence
+ *     boundaries in that stream.  Row t of `hidden` is the state that predicts targets[t]
+ *     (caller pre-shifts; only loss-bearing positions are packed).
+ *   - Requirements: d % 8 == 0, V >= 1, T >= 1, hidden/W/dW 16-byte aligned.  Otherwise GRPO_ERR_SHAPE.
+ *   - Device arch must be sm_100; otherwise GRPO_ERR_ARCH.  There is no CPU or other-GPU fallback.
+ */
+#ifndef GRPO_B200_H_
+#define GRPO_B200_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GRPO_OK = 0,
+  GRPO_ERR_INVALID_ARG = 1,
+  GRPO_ERR_SHAPE = 2,
+  GRPO_ERR_WORKSPACE = 3,
+  GRPO_ERR_ARCH = 4,
+  GRPO_ERR_CUDA = 5,
+  GRPO_ERR_INCOMPLETE_GROUP = 6,
+  GRPO_ERR_QUEUE_FULL = 7
+} grpo_status;
+
+typedef struct grpo_ctx grpo_ctx;
+
+typedef struct {
+  int32_t d;                 /* hidden width */
+  int32_t V;                 /* vocabulary size */
+  float   eps_std;           /* Eq. 1 stabiliser; 1e-6 */
+  int32_t std_ddof;          /* 0: population sigma (default reading of PAPER.md:90), 1: sample sigma */
+  float   clip_lo, clip_hi;  /* ratio clipped to [1-clip_lo, 1+clip_hi]; 0.2 / 0.28 */
+  float   kl_beta;           /* weight of the k3 term; 0 disables it */
+  int32_t loss_agg;          /* 0: token mean over the logical update; 1: per-sequence mean, then mean over sequences */
+  float   logit_scale;       /* 1 / temperature; 1 */
+  int32_t dhidden_fp32;      /* 0: dHidden written as bf16, 1: fp32 */
+  int32_t group_size;        /* K: responses per complete group; 0 = do not check */
+  int32_t groups_per_update; /* U = B/K; >= 1 */
+  int32_t groups_per_round;  /* R; 0 = unknown (round-complete flag never raised) */
+  int64_t token_budget;      /* feasible-batch token budget per launch; 0 = unlimited */
+  int64_t bwd_chunk_tokens;  /* tokens per backward dZ chunk; 0 = default (9472) */
+  int32_t max_pending_groups;/* FIFO capacity; 0 = default (4096) */
+} grpo_config;
+
+/* Fill *cfg with the defaults above (d, V must still be set). */
+int32_t grpo_default_config(grpo_config* cfg);
+
+/* Create / destroy a context on the CURRENT CUDA device.  HOST pointers. */
+int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out);
+int32_t grpo_destroy(grpo_ctx* ctx);
+
+/* Thread-local, never NULL; valid until the next failing call on this thread. */
+const char* grpo_last_error(void);
+
+/* Bytes of ONE workspace slot able to process launches of up to max_T packed tokens. */
+int32_t grpo_workspace_bytes(const grpo_ctx* ctx, int64_t max_T, int64_t* bytes_out /*HOST*/);
+
+/* Hand the library n_slots workspace slots (caller-allocated device memory, 256-byte aligned,
+ * bytes >= n_slots * grpo_workspace_bytes(max_T)).  Direct fwd/bwd calls use slot 0 and must
+ * not run concurrently with each other; grpo_enqueue_groups uses slot (stream index). */
+int32_t grpo_set_workspace(grpo_ctx* ctx, void* dev_ptr, int64_t bytes, int64_t max_T, int32_t n_slots);
+
+/* A1 — Eq. 1.  rewards fp32 [S]; groups are [cu_groups[g], cu_groups[g+1]) if
+ * cu_groups (int32 [n_groups+1], device) is given, else uniform of size G.  adv_out fp32 [S];
+ * zero_var_out u8 [n_groups] or NULL (1 where all rewards of the group are equal => advantages are
+ * exactly 0).  One warp per group. */
+int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, const int32_t* cu_groups, int32_t n_groups,
+                             int32_t G, float* adv_out, uint8_t* zero_var_out, void* stream);
+
+/* A2 + A3.  targets int32 [T] (<0: token ignored; >=V: ignored and an error bit is raised, see
+ * grpo_check_errors_sync).  adv fp32 [S].  old_logp fp32 [T].  ref_logp fp32 [T] or NULL (no KL).
+ * mask u8 [T] or NULL (all ones).  loss_denom > 0: explicit denominator of the whole logical update
+ * (loss_agg 0); <= 0: max(sum of this call's mask, 1).
+ * Outputs: logp_out, lse_out, coeff_out fp32 [T] (coeff_t = d loss / d logp_t, consumed by bwd);
+ * loss_accum fp32 [1] is ADDED to; metrics_accum fp32 [4] or NULL is ADDED to:
+ * {loss-bearing tokens, sum rho, sum k3, tokens whose policy gradient is clipped}. */
+int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const void* W, const int32_t* targets,
+                                    const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv,
+                                    const float* old_logp, const float* ref_logp, const uint8_t* mask,
+                                    double loss_denom, float* logp_out, float* lse_out, float* coeff_out,
+                                    float* loss_accum, float* metrics_accum, void* stream);
+
+/* A4-A6.  lse, coeff from the forward.  grad_scale multiplies both gradients (upstream dLoss).
+ * dhidden_out [T, d] (bf16, or fp32 if cfg.dhidden_fp32) is OVERWRITTEN; dW_accum fp32 [V, d] is
+ * ADDED to with atomics (caller zeroes it at the optimizer boundary).  Either may be NULL to skip. */
+int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden, const void* W, const int32_t* targets,
+                                    const float* lse, const float* coeff, int64_t T, float grad_scale,
+                                    void* dhidden_out, float* dW_accum, void* stream);
+
+/* One COMPLETE group (all K responses present, rewards verified). */
+typedef struct {
+  int64_t group_order;          /* submission order; informational, FIFO is by arrival */
+  int32_t G;                    /* responses in the group */
+  const int32_t* seqlens_host;  /* HOST int32 [G]: loss-bearing tokens per response (copied by the call) */
+  const void* hidden;           /* bf16 [T_g, d], the group's packed tokens */
+  const int32_t* targets;       /* [T_g] */
+  const float* old_logp;        /* [T_g] */
+  const float* ref_logp;        /* [T_g] or NULL */
+  const uint8_t* mask;          /* [T_g] or NULL */
+  const float* rewards;         /* device fp32 [G] */
+  void* dhidden_out;            /* [T_g, d] or NULL */
+  float* logp_out;              /* [T_g] or NULL */
+} grpo_group_desc;
+
+/* A0 + A7.  Append n complete groups to the FIFO in arrival order, then, if at least U
+ * groups are pending, run ONE logical update over the earliest U: they are split into launches, each
+ * the largest prefix of whole groups within cfg.token_budget (at least one group); launch
+ * k of the context runs on streams[k % n_streams] with workspace slot k % n_streams; each launch is
+ * A1 -> A2/A3 -> A4-A6 on its packed tokens.  dW_accum / loss_accum are only ADDED to.
+ * loss_denom as in the forward but over the whole update (<= 0: derived from the update's masks).
+ * A group with G != cfg.group_size (when set), G <= 0, a NULL pointer where one is required or a
+ * non-positive sequence length is GRPO_ERR_INCOMPLETE_GROUP and nothing is appended.
+ * HOST outputs: groups_consumed_out (total consumed so far), update_boundary_out (1 if an update was
+ * run by this call: the caller may step the optimizer and zero dW once the streams reach this work).
+ * n = 0 is allowed (continue draining the FIFO). */
+int32_t grpo_enqueue_groups(grpo_ctx* ctx, const grpo_group_desc* groups, int32_t n, const void* W,
+                            float* dW_accum, float* loss_accum, float* metrics_accum, double loss_denom,
+                            void* const* streams, int32_t n_streams, int32_t* groups_consumed_out,
+                            int32_t* update_boundary_out);
+
+/* End of round: run whatever is pending (< U groups) as a final, short update. */
+int32_t grpo_flush(grpo_ctx* ctx, const void* W, float* dW_accum, float* loss_accum, float* metrics_accum,
+                   double loss_denom, void* const* streams, int32_t n_streams, int32_t* groups_consumed_out,
+                   int32_t* update_boundary_out);
+
+/* FIFO state (HOST outputs, any may be NULL): groups / tokens pending, groups consumed,
+ * round_complete = 1 once consumed >= cfg.groups_per_round > 0 (Alg. 1 l.22). */
+int32_t grpo_queue_state(const grpo_ctx* ctx, int32_t* pending_groups, int64_t* pending_tokens,
+                         int32_t* consumed_groups, int32_t* round_complete);
+int32_t grpo_reset_round(grpo_ctx* ctx);
+
+/* Pure host helper (no CUDA): how the next logical update is cut into launches.  group_tokens HOST
+ * int64 [n_pending] in FIFO order.  Returns in launch_sizes_out[0..*n_launches_out) the number of
+ * groups per launch; *n_launches_out = 0 if fewer than U groups are pending and flush == 0. */
+int32_t grpo_cgp_plan(const int64_t* group_tokens, int32_t n_pending, int32_t U, int64_t token_budget,
+                      int32_t flush, int32_t* launch_sizes_out, int32_t cap, int32_t* n_launches_out);
+
+/* Reads the device error word (bit 0: a target id >= V was seen) and clears it.  Synchronises. */
+int32_t grpo_check_errors_sync(grpo_ctx* ctx, int32_t* flags_out /*HOST*/);
+
+/* End-to-end convenience over HOST buffers (pinned recommended): copies one packed batch to the
+ * device (slot 0 staging), runs A1 -> A6 with W / dW_accum resident on the device, copies
+ * loss, logp and dHidden back, and synchronises `stream`.  n_groups uniform groups of size G.
+ * hidden_host bf16 [T,d]; dhidden_host [T,d] or NULL; logp_host [T] or NULL; loss_host fp32 [1]. */
+int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const int32_t* targets_host,
+                       const int32_t* cu_seqlens_host, const float* rewards_host, const float* old_logp_host,
+                       const float* ref_logp_host, const uint8_t* mask_host, int32_t n_groups, int32_t G,
+                       int64_t T, const void* W, float* dW_accum, double loss_denom, float* loss_host,
+                       float* logp_host, void* dhidden_host, void* stream);
+
+/* Test hook: C[M,N] (fp32, row-major, pitch N) = A * B with the production tcgen05 kernel.
+ * layout 0: A [M,K] K-major, B [N,K] K-major;  1: A [M,K] K-major, B [K,N] MN-major;
+ * 2: A [K,M] MN-major, B [K,N] MN-major.  accumulate != 0: C += (atomic).  bf16 inputs.
+ * M, N, K multiples of 8. */
+int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A, const void* B, float* C, int32_t M,
+                        int32_t N, int32_t K, int32_t accumulate, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRPO_B200_H_ */

@@ -1,0 +1,330 @@
+// Persistent, warp-specialised tcgen05 GEMM for the four vocab-sized contractions of the GRPO step
+// (SURVEY.md §8(a) rows A2, A4, A5, A6), with the method's epilogues fused behind the TMEM accumulator.
+//
+//   warp 0      : TMA producer   (cp.async.bulk.tensor -> 128B-swizzled smem ring, mbarrier complete_tx)
+//   warp 1      : MMA issuer     (one thread: tcgen05.mma kind::f16, fp32 accumulators in TMEM, 2 stages)
+//   warps 2..5  : epilogue       (tcgen05.ld 32x32b: one accumulator row per thread)
+//
+// C tile = 128 x 256, K block = 64 bf16 (one 128-byte swizzle row), 4-stage smem ring (192 KB),
+// 2 x 256 TMEM columns so the epilogue of tile i overlaps the MMAs of tile i+1.
+//
+// Operand layouts (template): K-major (row = M/N index, 64 contiguous k) or MN-major (row = k index,
+// 64 contiguous m/n per 8 KB box).  Row-major tensors are consumed as they are; nothing is transposed
+// in memory:
+//   A2/A4  z  = H W^T        A = H  [T,d]  K-major   B = W  [V,d]  K-major    K = d
+//   A5     dH = dZ W         A = dZ [Tc,V] K-major   B = W  [V,d]  MN-major   K = V
+//   A6     dW += dZ^T H      A = dZ [Tc,V] MN-major  B = H  [Tc,d] MN-major   K = Tc
+#pragma once
+#include "ptx_sm100.cuh"
+
+namespace grpo {
+
+constexpr int BM = 128, BN = 256, BK = 64;
+constexpr int kStages = 4;
+constexpr int kABytes = BM * BK * 2;        // 16 KB
+constexpr int kBBytes = BN * BK * 2;        // 32 KB
+constexpr int kStageBytes = kABytes + kBBytes;
+constexpr int kGemmThreads = 192;
+constexpr int kTmemCols = 512;
+constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+
+enum Epi : int { EPI_LSE = 0, EPI_DZ = 1, EPI_STORE = 2, EPI_RED_F32 = 3 };
+
+struct GemmParams {
+  int m_total, n_total;              // valid rows / cols of C
+  int m_tiles, n_tiles, k_blocks;
+  int n_fastest;                     // unit order: 1 = n tile fastest (A5/A6), 0 = m tile fastest (A2/A4)
+  int n_split, tiles_per_split;      // EPI_LSE: a unit is (m tile, contiguous range of n tiles)
+  uint32_t lbo_a, sbo_a, kadv_a;     // smem descriptor constants (bytes); see make_smem_desc
+  uint32_t lbo_b, sbo_b, kadv_b;
+  // per-token arrays are indexed by (row_offset + local row)
+  int64_t row_offset;
+  const int32_t* targets;
+  float scale_log2e;                 // logit_scale * log2(e)
+  float logit_scale;
+  // EPI_LSE outputs (log2 domain running max / sum per split) + the target logit
+  float* part_m;
+  float* part_s;
+  int64_t part_stride;
+  float* zy;
+  // EPI_DZ
+  const float* lse;
+  const float* coeff;
+  float coeff_mul;                   // logit_scale * grad_scale
+  __nv_bfloat16* dz;
+  int64_t dz_pitch;
+  // EPI_STORE (bf16 or fp32) / EPI_RED_F32
+  void* c_out;
+  int64_t c_pitch;                   // elements
+  int c_fp32;
+};
+
+struct alignas(8) GemmBarriers {
+  uint64_t full[kStages];
+  uint64_t empty[kStages];
+  uint64_t tmem_full[2];
+  uint64_t tmem_empty[2];
+  uint32_t tmem_base;
+};
+
+__device__ __forceinline__ void unit_to_tiles(const GemmParams& p, int u, int epi, int& m_tile, int& n0, int& n1) {
+  if (epi == EPI_LSE) {
+    m_tile = u % p.m_tiles;
+    int split = u / p.m_tiles;
+    n0 = split * p.tiles_per_split;
+    n1 = min(p.n_tiles, n0 + p.tiles_per_split);
+  } else if (p.n_fastest) {
+    n0 = u % p.n_tiles;
+    m_tile = u / p.n_tiles;
+    n1 = n0 + 1;
+  } else {
+    m_tile = u % p.m_tiles;
+    n0 = u / p.m_tiles;
+    n1 = n0 + 1;
+  }
+}
+
+template <bool A_MN, bool B_MN, int EPI>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                 const GemmParams p, const int n_units) {
+  extern __shared__ uint8_t smem_raw[];
+  // SWIZZLE_128B atoms need 1024-byte alignment of the tile bases
+  const uint32_t raw_addr = smem_u32(smem_raw);
+  const uint32_t pad = (1024u - (raw_addr & 1023u)) & 1023u;
+  uint8_t* smem = smem_raw + pad;
+  const uint32_t tiles_addr = raw_addr + pad;
+  GemmBarriers* bars = reinterpret_cast<GemmBarriers*>(smem + kStages * kStageBytes);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&tmA);
+    prefetch_tmap(&tmB);
+    for (int i = 0; i < kStages; ++i) {
+      mbar_init(&bars->full[i], 1);
+      mbar_init(&bars->empty[i], 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&bars->tmem_full[i], 1);
+      mbar_init(&bars->tmem_empty[i], 4);     // one arrive per epilogue warp
+    }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc<1>(&bars->tmem_base, kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_base;
+
+  if (warp == 0) {
+    // ================================================================ TMA producer
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        int m_tile, n0, n1;
+        unit_to_tiles(p, u, EPI, m_tile, n0, n1);
+        for (int n_tile = n0; n_tile < n1; ++n_tile) {
+          for (int kb = 0; kb < p.k_blocks; ++kb) {
+            mbar_wait(&bars->empty[stage], phase ^ 1);
+            mbar_arrive_expect_tx(&bars->full[stage], kStageBytes);
+            const uint32_t a_dst = tiles_addr + stage * kStageBytes;
+            const uint32_t b_dst = a_dst + kABytes;
+            if constexpr (!A_MN) {
+              tma_load_2d(a_dst, &tmA, &bars->full[stage], kb * BK, m_tile * BM);
+            } else {
+#pragma unroll
+              for (int i = 0; i < BM / 64; ++i)
+                tma_load_2d(a_dst + i * 8192, &tmA, &bars->full[stage], m_tile * BM + i * 64, kb * BK);
+            }
+            if constexpr (!B_MN) {
+              tma_load_2d(b_dst, &tmB, &bars->full[stage], kb * BK, n_tile * BN);
+            } else {
+#pragma unroll
+              for (int i = 0; i < BN / 64; ++i)
+                tma_load_2d(b_dst + i * 8192, &tmB, &bars->full[stage], n_tile * BN + i * 64, kb * BK);
+            }
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================ MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc = make_idesc_bf16(BM, BN, A_MN ? 1 : 0, B_MN ? 1 : 0);
+      int stage = 0;
+      uint32_t phase = 0;
+      int acc = 0;
+      uint32_t acc_phase = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        int m_tile, n0, n1;
+        unit_to_tiles(p, u, EPI, m_tile, n0, n1);
+        for (int n_tile = n0; n_tile < n1; ++n_tile) {
+          mbar_wait(&bars->tmem_empty[acc], acc_phase ^ 1);
+          tc_fence_after();
+          const uint32_t d_tmem = tmem_base + acc * BN;
+          for (int kb = 0; kb < p.k_blocks; ++kb) {
+            mbar_wait(&bars->full[stage], phase);
+            tc_fence_after();
+            const uint32_t a_addr = tiles_addr + stage * kStageBytes;
+            const uint32_t b_addr = a_addr + kABytes;
+#pragma unroll
+            for (int k = 0; k < BK / 16; ++k) {
+              const uint64_t adesc = make_smem_desc(a_addr + k * p.kadv_a, p.lbo_a, p.sbo_a);
+              const uint64_t bdesc = make_smem_desc(b_addr + k * p.kadv_b, p.lbo_b, p.sbo_b);
+              umma_bf16<1>(d_tmem, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
+            }
+            umma_commit(&bars->empty[stage]);          // smem slot reusable once these MMAs retire
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+          }
+          umma_commit(&bars->tmem_full[acc]);          // accumulator complete -> epilogue
+          acc ^= 1;
+          if (acc == 0) acc_phase ^= 1;
+        }
+      }
+    }
+  } else {
+    // ================================================================ epilogue (4 warps, 128 rows)
+    const int quad = warp & 3;                         // TMEM lane quarter this warp may access
+    const int row_in_tile = quad * 32 + lane;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      int m_tile, n0, n1;
+      unit_to_tiles(p, u, EPI, m_tile, n0, n1);
+      const int row_local = m_tile * BM + row_in_tile;          // row within this launch's C
+      const bool row_ok = row_local < p.m_total;
+      const int64_t row_g = p.row_offset + row_local;            // index into per-token arrays
+
+      [[maybe_unused]] int y = -1;
+      [[maybe_unused]] float run_m = -INFINITY, run_s = 0.f;     // EPI_LSE running stats (log2 domain)
+      [[maybe_unused]] float lse2 = 0.f, kcoef = 0.f;            // EPI_DZ per-row constants
+      if constexpr (EPI == EPI_LSE || EPI == EPI_DZ) {
+        if (row_ok) {
+          y = p.targets[row_g];
+          if (y >= p.n_total) y = -1;
+        }
+      }
+      if constexpr (EPI == EPI_DZ) {
+        if (row_ok) {
+          lse2 = p.lse[row_g] * kLog2e;
+          kcoef = p.coeff[row_g] * p.coeff_mul;
+        }
+      }
+
+      for (int n_tile = n0; n_tile < n1; ++n_tile) {
+        mbar_wait(&bars->tmem_full[acc], acc_phase);
+        tc_fence_after();
+        const uint32_t t_addr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
+        const int col_tile = n_tile * BN;
+#pragma unroll 1
+        for (int c = 0; c < BN / 32; ++c) {
+          const int cbase = col_tile + c * 32;
+          if (cbase >= p.n_total) break;                          // warp-uniform
+          float v[32];
+          tmem_ld32(t_addr + c * 32, v);
+          tmem_ld_wait();
+          const int nvalid = p.n_total - cbase;                   // >= 1; columns >= nvalid are padding
+
+          if constexpr (EPI == EPI_LSE) {
+            float cmax = -INFINITY;
+            if (nvalid >= 32) {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) { v[i] *= p.scale_log2e; cmax = fmaxf(cmax, v[i]); }
+            } else {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                v[i] = i < nvalid ? v[i] * p.scale_log2e : -INFINITY;
+                cmax = fmaxf(cmax, v[i]);
+              }
+            }
+            const float new_m = fmaxf(run_m, cmax);
+            float s = 0.f;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) s += ex2_approx(v[i] - new_m);
+            run_s = run_s * ex2_approx(run_m - new_m) + s;
+            run_m = new_m;
+            if (static_cast<uint32_t>(y - cbase) < 32u) {          // rare: target column in this chunk
+              float zy2 = 0.f;
+#pragma unroll
+              for (int i = 0; i < 32; ++i) zy2 = (y - cbase == i) ? v[i] : zy2;
+              p.zy[row_g] = zy2 * kLn2;                            // back to natural units: s * z
+            }
+          } else if constexpr (EPI == EPI_DZ) {
+            // dz = k (1[v = y] - p),  p = 2^(z s log2e - lse log2e)
+            float dzv[32];
+#pragma unroll
+            for (int i = 0; i < 32; ++i) dzv[i] = -kcoef * ex2_approx(fmaf(v[i], p.scale_log2e, -lse2));
+            if (static_cast<uint32_t>(y - cbase) < 32u) {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) dzv[i] = (y - cbase == i) ? dzv[i] + kcoef : dzv[i];
+            }
+            if (row_ok) {
+              __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
+#pragma unroll
+              for (int g = 0; g < 4; ++g)
+                st_global_v4(dst + g * 8, pack_bf16x2(dzv[g * 8 + 0], dzv[g * 8 + 1]),
+                             pack_bf16x2(dzv[g * 8 + 2], dzv[g * 8 + 3]), pack_bf16x2(dzv[g * 8 + 4], dzv[g * 8 + 5]),
+                             pack_bf16x2(dzv[g * 8 + 6], dzv[g * 8 + 7]));
+            }
+          } else if constexpr (EPI == EPI_STORE) {
+            if (row_ok) {
+              if (p.c_fp32) {
+                float* dst = reinterpret_cast<float*>(p.c_out) + static_cast<int64_t>(row_local) * p.c_pitch + cbase;
+#pragma unroll
+                for (int g = 0; g < 8; ++g)
+                  if (g * 4 < nvalid)
+                    *reinterpret_cast<float4*>(dst + g * 4) =
+                        make_float4(v[g * 4], v[g * 4 + 1], v[g * 4 + 2], v[g * 4 + 3]);
+              } else {
+                __nv_bfloat16* dst =
+                    reinterpret_cast<__nv_bfloat16*>(p.c_out) + static_cast<int64_t>(row_local) * p.c_pitch + cbase;
+#pragma unroll
+                for (int g = 0; g < 4; ++g)
+                  if (g * 8 < nvalid)
+                    st_global_v4(dst + g * 8, pack_bf16x2(v[g * 8 + 0], v[g * 8 + 1]),
+                                 pack_bf16x2(v[g * 8 + 2], v[g * 8 + 3]), pack_bf16x2(v[g * 8 + 4], v[g * 8 + 5]),
+                                 pack_bf16x2(v[g * 8 + 6], v[g * 8 + 7]));
+              }
+            }
+          } else {  // EPI_RED_F32: C += acc (fp32, atomic so launches on other streams may accumulate too)
+            if (row_ok) {
+              float* dst = reinterpret_cast<float*>(p.c_out) + static_cast<int64_t>(row_local) * p.c_pitch + cbase;
+#pragma unroll
+              for (int g = 0; g < 8; ++g)
+                if (g * 4 < nvalid) red_add_v4_f32(dst + g * 4, v[g * 4], v[g * 4 + 1], v[g * 4 + 2], v[g * 4 + 3]);
+            }
+          }
+        }
+        // all of this warp's TMEM reads of the accumulator are done: hand it back to the MMA warp
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars->tmem_empty[acc]);
+        acc ^= 1;
+        if (acc == 0) acc_phase ^= 1;
+      }
+
+      if constexpr (EPI == EPI_LSE) {
+        if (row_ok) {
+          const int split = u / p.m_tiles;
+          p.part_m[split * p.part_stride + row_g] = run_m;
+          p.part_s[split * p.part_stride + row_g] = run_s;
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc<1>(tmem_base, kTmemCols);
+  }
+}
+
+}  // namespace grpo

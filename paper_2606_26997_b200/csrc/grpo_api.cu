@@ -1,0 +1,771 @@
+// C ABI (include/grpo.h) of the fused GRPO policy-loss step: context, workspace, launch logic, CGP FIFO.
+// Every step of the path runs in the kernels of this directory; there is no CPU or library fallback.
+#include "../../include/grpo.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <deque>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "cgp_queue.h"
+#include "gemm_sm100.cuh"
+#include "token_kernels.cuh"
+
+using namespace grpo;
+
+// ------------------------------------------------------------------------------------- errors
+static thread_local char g_err[512] = "";
+static int32_t fail(int32_t code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+#define CU_OK(expr)                                                                                   \
+  do {                                                                                                \
+    cudaError_t e__ = (expr);                                                                         \
+    if (e__ != cudaSuccess)                                                                           \
+      return fail(GRPO_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+  } while (0)
+#define GRPO_TRY(expr)                  \
+  do {                                  \
+    int32_t s__ = (expr);               \
+    if (s__ != GRPO_OK) return s__;     \
+  } while (0)
+
+// ------------------------------------------------------------------------------------- context
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+struct SlotLayout {
+  int64_t part_cap = 0;   // floats per partial array
+  int64_t s_max = 0;
+  int64_t chunk_rows = 0;
+  int64_t v_pad = 0;
+  int64_t off_part_m = 0, off_part_s = 0, off_zy = 0, off_total = 0, off_seq_count = 0, off_dz = 0;
+  int64_t off_hidden = 0, off_targets = 0, off_old = 0, off_ref = 0, off_mask = 0, off_rewards = 0, off_adv = 0,
+          off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0;
+  int64_t bytes = 0;
+};
+
+struct PendingGroup {
+  grpo_group_desc desc;
+  std::vector<int32_t> seqlens;
+  int64_t tokens;
+};
+
+struct grpo_ctx {
+  grpo_config cfg;
+  int device = 0;
+  int num_sms = 0;
+  EncodeTiledFn encode = nullptr;
+  int32_t* err_dev = nullptr;
+  float* denom_ring = nullptr;   // device scalars for implicit per-update denominators
+  int denom_next = 0;
+  cudaEvent_t denom_event = nullptr;
+  uint8_t* ws = nullptr;
+  int64_t ws_max_T = 0;
+  int n_slots = 0;
+  SlotLayout lay;
+  std::deque<PendingGroup> fifo;
+  int64_t launches = 0;
+  int32_t consumed = 0;
+};
+static const int kDenomRing = 64;
+
+static int64_t chunk_tokens(const grpo_config& c) { return c.bwd_chunk_tokens > 0 ? c.bwd_chunk_tokens : 9472; }
+
+static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
+  SlotLayout L;
+  int64_t off = 0;
+  auto take = [&](int64_t bytes) {
+    int64_t o = off;
+    off = align_up(off + bytes, 256);
+    return o;
+  };
+  L.part_cap = max_T + 148LL * 128 * 4;
+  L.s_max = std::min<int64_t>(max_T, 1 << 20);
+  L.chunk_rows = std::min<int64_t>(align_up(chunk_tokens(c), 128), align_up(max_T, 128));
+  L.v_pad = align_up(c.V, 64);
+  L.off_part_m = take(L.part_cap * 4);
+  L.off_part_s = take(L.part_cap * 4);
+  L.off_zy = take(max_T * 4);
+  L.off_total = take(256);
+  L.off_seq_count = take(L.s_max * 4);
+  L.off_dz = take(L.chunk_rows * L.v_pad * 2);
+  L.off_hidden = take(max_T * c.d * 2);
+  L.off_targets = take(max_T * 4);
+  L.off_old = take(max_T * 4);
+  L.off_ref = take(max_T * 4);
+  L.off_mask = take(max_T);
+  L.off_rewards = take(L.s_max * 4);
+  L.off_adv = take(L.s_max * 4);
+  L.off_cu_seq = take((L.s_max + 1) * 4);
+  L.off_cu_grp = take((L.s_max + 1) * 4);
+  L.off_logp = take(max_T * 4);
+  L.off_lse = take(max_T * 4);
+  L.off_coeff = take(max_T * 4);
+  L.off_dh = take(max_T * c.d * (c.dhidden_fp32 ? 4 : 2));
+  L.bytes = off;
+  return L;
+}
+
+template <typename T>
+static T* slot_ptr(const grpo_ctx* ctx, int slot, int64_t off) {
+  return reinterpret_cast<T*>(ctx->ws + static_cast<int64_t>(slot) * ctx->lay.bytes + off);
+}
+
+// ------------------------------------------------------------------------------------- TMA maps
+// 2-D bf16 tensor, `inner` contiguous elements per row, `outer` rows, row pitch in bytes; 128B swizzle;
+// out-of-bounds elements of a box read as zero (this is what makes ragged M/N/K tails work).
+static int32_t make_tmap(const grpo_ctx* ctx, CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer,
+                         uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_outer) {
+  if ((reinterpret_cast<uintptr_t>(base) & 15) != 0 || (pitch_bytes & 15) != 0)
+    return fail(GRPO_ERR_SHAPE, "tensor base/pitch not 16-byte aligned (base %p pitch %llu)", base,
+                (unsigned long long)pitch_bytes);
+  cuuint64_t dims[2] = {inner, outer};
+  cuuint64_t strides[1] = {pitch_bytes};
+  cuuint32_t box[2] = {box_inner, box_outer};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(GRPO_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return GRPO_OK;
+}
+
+static void set_desc_defaults(GemmParams& p, bool a_mn, bool b_mn) {
+  // K-major SW128: 8-row groups 1024 B apart, +32 B per 16-element k step inside the 128 B row.
+  // MN-major SW128: 64-element MN groups 8192 B apart (one TMA box), 8-row k groups 1024 B apart,
+  // +2048 B per 16-row k step.
+  p.lbo_a = a_mn ? 8192 : 16; p.sbo_a = 1024; p.kadv_a = a_mn ? 2048 : 32;
+  p.lbo_b = b_mn ? 8192 : 16; p.sbo_b = 1024; p.kadv_b = b_mn ? 2048 : 32;
+}
+
+template <bool A_MN, bool B_MN, int EPI>
+static int32_t launch_gemm(const grpo_ctx* ctx, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
+                           int n_units, cudaStream_t st) {
+  static bool attr_set = false;
+  auto kern = grpo_gemm_kernel<A_MN, B_MN, EPI>;
+  if (!attr_set) {
+    CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    attr_set = true;
+  }
+  if (n_units <= 0) return GRPO_OK;
+  const int grid = std::min(n_units, ctx->num_sms);
+  kern<<<grid, kGemmThreads, kSmemBytes, st>>>(tmA, tmB, p, n_units);
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
+}
+
+static int choose_n_split(int m_tiles, int n_tiles, int sms, int64_t max_split) {
+  int best = 1;
+  int64_t best_cost = INT64_MAX;
+  const int lim = static_cast<int>(std::min<int64_t>(std::min<int64_t>(max_split, n_tiles), 4 * sms));
+  for (int s = 1; s <= std::max(lim, 1); ++s) {
+    const int tps = (n_tiles + s - 1) / s;
+    const int s_eff = (n_tiles + tps - 1) / tps;
+    if (s_eff != s) continue;
+    const int64_t waves = (static_cast<int64_t>(m_tiles) * s + sms - 1) / sms;
+    const int64_t cost = waves * tps;
+    if (cost < best_cost) { best_cost = cost; best = s; }
+  }
+  return best;
+}
+
+// ------------------------------------------------------------------------------------- API: misc
+extern "C" const char* grpo_last_error(void) { return g_err; }
+
+extern "C" int32_t grpo_default_config(grpo_config* cfg) {
+  if (!cfg) return fail(GRPO_ERR_INVALID_ARG, "cfg is NULL");
+  std::memset(cfg, 0, sizeof(*cfg));
+  cfg->eps_std = 1e-6f;
+  cfg->clip_lo = 0.2f;
+  cfg->clip_hi = 0.28f;
+  cfg->logit_scale = 1.0f;
+  cfg->groups_per_update = 1;
+  cfg->bwd_chunk_tokens = 9472;
+  cfg->max_pending_groups = 4096;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
+  if (!cfg || !out) return fail(GRPO_ERR_INVALID_ARG, "cfg/out is NULL");
+  if (cfg->d <= 0 || cfg->V <= 0 || cfg->d % 8 != 0)
+    return fail(GRPO_ERR_SHAPE, "need d > 0, d %% 8 == 0, V > 0 (got d=%d V=%d)", cfg->d, cfg->V);
+  if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
+    return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
+  int dev = 0;
+  CU_OK(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CU_OK(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10)
+    return fail(GRPO_ERR_ARCH, "device %d is sm_%d%d; this library is built for sm_100a only", dev, prop.major,
+                prop.minor);
+  grpo_ctx* ctx = new (std::nothrow) grpo_ctx();
+  if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "out of host memory");
+  ctx->cfg = *cfg;
+  if (ctx->cfg.max_pending_groups <= 0) ctx->cfg.max_pending_groups = 4096;
+  ctx->device = dev;
+  ctx->num_sms = prop.multiProcessorCount;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+    delete ctx;
+    return fail(GRPO_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+  }
+  ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
+  if (cudaMalloc(&ctx->err_dev, 256) != cudaSuccess || cudaMalloc(&ctx->denom_ring, kDenomRing * 4) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->denom_event, cudaEventDisableTiming) != cudaSuccess) {
+    delete ctx;
+    return fail(GRPO_ERR_CUDA, "context allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  CU_OK(cudaMemset(ctx->err_dev, 0, 256));
+  *out = ctx;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_destroy(grpo_ctx* ctx) {
+  if (!ctx) return GRPO_OK;
+  cudaFree(ctx->err_dev);
+  cudaFree(ctx->denom_ring);
+  if (ctx->denom_event) cudaEventDestroy(ctx->denom_event);
+  delete ctx;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_workspace_bytes(const grpo_ctx* ctx, int64_t max_T, int64_t* bytes_out) {
+  if (!ctx || !bytes_out || max_T <= 0) return fail(GRPO_ERR_INVALID_ARG, "bad ctx / max_T / bytes_out");
+  *bytes_out = make_layout(ctx->cfg, max_T).bytes;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_set_workspace(grpo_ctx* ctx, void* dev_ptr, int64_t bytes, int64_t max_T, int32_t n_slots) {
+  if (!ctx || !dev_ptr || max_T <= 0 || n_slots < 1) return fail(GRPO_ERR_INVALID_ARG, "bad workspace arguments");
+  if (reinterpret_cast<uintptr_t>(dev_ptr) & 255) return fail(GRPO_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+  SlotLayout L = make_layout(ctx->cfg, max_T);
+  if (bytes < L.bytes * n_slots)
+    return fail(GRPO_ERR_WORKSPACE, "workspace too small: %lld < %d x %lld", (long long)bytes, n_slots,
+                (long long)L.bytes);
+  ctx->ws = static_cast<uint8_t*>(dev_ptr);
+  ctx->ws_max_T = max_T;
+  ctx->n_slots = n_slots;
+  ctx->lay = L;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_check_errors_sync(grpo_ctx* ctx, int32_t* flags_out) {
+  if (!ctx || !flags_out) return fail(GRPO_ERR_INVALID_ARG, "ctx/flags_out is NULL");
+  CU_OK(cudaDeviceSynchronize());
+  CU_OK(cudaMemcpy(flags_out, ctx->err_dev, 4, cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemset(ctx->err_dev, 0, 4));
+  return GRPO_OK;
+}
+
+// ------------------------------------------------------------------------------------- A1
+extern "C" int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, const int32_t* cu_groups,
+                                        int32_t n_groups, int32_t G, float* adv_out, uint8_t* zero_var_out,
+                                        void* stream) {
+  if (!ctx || !rewards || !adv_out) return fail(GRPO_ERR_INVALID_ARG, "ctx/rewards/adv_out is NULL");
+  if (n_groups < 0 || (!cu_groups && G <= 0)) return fail(GRPO_ERR_INVALID_ARG, "need n_groups >= 0 and G > 0 or cu_groups");
+  if (n_groups == 0) return GRPO_OK;
+  const int threads = 128;
+  const int blocks = (n_groups * 32 + threads - 1) / threads;
+  group_advantage_kernel<<<blocks, threads, 0, static_cast<cudaStream_t>(stream)>>>(
+      rewards, cu_groups, n_groups, G, ctx->cfg.eps_std, ctx->cfg.std_ddof, adv_out, zero_var_out);
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
+}
+
+// ------------------------------------------------------------------------------------- A2 + A3
+static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
+                        const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv, const float* old_logp,
+                        const float* ref_logp, const uint8_t* mask, double loss_denom, const float* denom_dev,
+                        float* logp_out, float* lse_out, float* coeff_out, float* loss_accum, float* metrics_accum,
+                        cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
+  if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
+  if (S > ctx->lay.s_max) return fail(GRPO_ERR_WORKSPACE, "S=%d exceeds workspace capacity", S);
+  if (T > INT32_MAX - 256) return fail(GRPO_ERR_SHAPE, "T too large");
+  const SlotLayout& L = ctx->lay;
+  float* part_m = slot_ptr<float>(ctx, slot, L.off_part_m);
+  float* part_s = slot_ptr<float>(ctx, slot, L.off_part_s);
+  float* zy = slot_ptr<float>(ctx, slot, L.off_zy);
+  float* total = slot_ptr<float>(ctx, slot, L.off_total);
+  float* seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
+
+  const bool implicit_denom = c.loss_agg == 0 && !(loss_denom > 0.0) && denom_dev == nullptr;
+  if (c.loss_agg == 1 || implicit_denom) {
+    CU_OK(cudaMemsetAsync(total, 0, 4, st));
+    const int threads = 128;
+    const int blocks = (S * 32 + threads - 1) / threads;
+    token_count_kernel<<<blocks, threads, 0, st>>>(mask, targets, c.V, cu_seqlens, S, seq_count, total);
+    CU_OK(cudaGetLastError());
+  }
+
+  CUtensorMap tmH, tmW;
+  GRPO_TRY(make_tmap(ctx, &tmH, hidden, c.d, T, static_cast<uint64_t>(c.d) * 2, BK, BM));
+  GRPO_TRY(make_tmap(ctx, &tmW, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN));
+  GemmParams p;
+  std::memset(&p, 0, sizeof(p));
+  set_desc_defaults(p, false, false);
+  p.m_total = static_cast<int>(T);
+  p.n_total = c.V;
+  p.m_tiles = static_cast<int>((T + BM - 1) / BM);
+  p.n_tiles = (c.V + BN - 1) / BN;
+  p.k_blocks = (c.d + BK - 1) / BK;
+  p.n_split = choose_n_split(p.m_tiles, p.n_tiles, ctx->num_sms, std::max<int64_t>(1, L.part_cap / T));
+  p.tiles_per_split = (p.n_tiles + p.n_split - 1) / p.n_split;
+  p.targets = targets;
+  p.scale_log2e = c.logit_scale * kLog2e;
+  p.logit_scale = c.logit_scale;
+  p.part_m = part_m;
+  p.part_s = part_s;
+  p.part_stride = T;
+  p.zy = zy;
+  GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, tmH, tmW, p, p.m_tiles * p.n_split, st)));
+
+  LossParams lp;
+  std::memset(&lp, 0, sizeof(lp));
+  lp.T = T; lp.S = S; lp.V = c.V; lp.n_split = p.n_split; lp.part_stride = T;
+  lp.part_m = part_m; lp.part_s = part_s; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = cu_seqlens;
+  lp.adv = adv; lp.old_logp = old_logp; lp.ref_logp = ref_logp; lp.mask = mask;
+  lp.seq_count = seq_count; lp.total_count = denom_dev ? denom_dev : total;
+  lp.denom_host = loss_denom > 0.0 ? static_cast<float>(loss_denom) : 0.f;
+  lp.loss_agg = c.loss_agg; lp.clip_lo = c.clip_lo; lp.clip_hi = c.clip_hi; lp.kl_beta = c.kl_beta;
+  lp.logp = logp_out; lp.lse = lse_out; lp.coeff = coeff_out; lp.loss_accum = loss_accum;
+  lp.metrics_accum = metrics_accum; lp.err_flag = ctx->err_dev;
+  const int threads = 256;
+  const int blocks = static_cast<int>((T + threads - 1) / threads);
+  loss_epilogue_kernel<<<blocks, threads, 0, st>>>(lp);
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const void* W,
+                                               const int32_t* targets, const int32_t* cu_seqlens, int32_t S,
+                                               int64_t T, const float* adv, const float* old_logp,
+                                               const float* ref_logp, const uint8_t* mask, double loss_denom,
+                                               float* logp_out, float* lse_out, float* coeff_out, float* loss_accum,
+                                               float* metrics_accum, void* stream) {
+  if (!ctx || !hidden || !W || !targets || !cu_seqlens || !adv || !old_logp || !logp_out || !lse_out || !coeff_out ||
+      !loss_accum)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0 and S > 0 (got T=%lld S=%d)", (long long)T, S);
+  return fwd_impl(ctx, 0, hidden, W, targets, cu_seqlens, S, T, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
+                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum, static_cast<cudaStream_t>(stream));
+}
+
+// ------------------------------------------------------------------------------------- A4 - A6
+static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
+                        const float* lse, const float* coeff, int64_t T, float grad_scale, void* dhidden_out,
+                        float* dW_accum, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
+  if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
+  if (!dhidden_out && !dW_accum) return GRPO_OK;
+  const SlotLayout& L = ctx->lay;
+  __nv_bfloat16* dz = slot_ptr<__nv_bfloat16>(ctx, slot, L.off_dz);
+  const int64_t Tc = L.chunk_rows;
+  const int n_chunks = static_cast<int>((T + Tc - 1) / Tc);
+  // equalise chunks (whole 128-row tiles) so the last one is not a sliver
+  const int64_t rows_per_chunk = std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, BM));
+  const uint8_t* Hb = static_cast<const uint8_t*>(hidden);
+  const int dh_elem = c.dhidden_fp32 ? 4 : 2;
+
+  CUtensorMap tmW_k, tmW_mn;
+  GRPO_TRY(make_tmap(ctx, &tmW_k, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN));
+  GRPO_TRY(make_tmap(ctx, &tmW_mn, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, 64, BK));
+
+  for (int64_t t0 = 0; t0 < T; t0 += rows_per_chunk) {
+    const int64_t rows = std::min<int64_t>(rows_per_chunk, T - t0);
+    const void* Hc = Hb + t0 * c.d * 2;
+    const int m_tiles = static_cast<int>((rows + BM - 1) / BM);
+    CUtensorMap tmH_k, tmH_mn, tmDZ_k, tmDZ_mn;
+    GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
+    GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
+
+    {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
+      GemmParams p;
+      std::memset(&p, 0, sizeof(p));
+      set_desc_defaults(p, false, false);
+      p.m_total = static_cast<int>(rows); p.n_total = c.V;
+      p.m_tiles = m_tiles; p.n_tiles = (c.V + BN - 1) / BN; p.k_blocks = (c.d + BK - 1) / BK;
+      p.n_fastest = 0;
+      p.row_offset = t0; p.targets = targets;
+      p.scale_log2e = c.logit_scale * kLog2e; p.logit_scale = c.logit_scale;
+      p.lse = lse; p.coeff = coeff; p.coeff_mul = c.logit_scale * grad_scale;
+      p.dz = dz; p.dz_pitch = L.v_pad;
+      GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
+    }
+    if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d]
+      GemmParams p;
+      std::memset(&p, 0, sizeof(p));
+      set_desc_defaults(p, false, true);
+      p.m_total = static_cast<int>(rows); p.n_total = c.d;
+      p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
+      p.n_fastest = 1;
+      p.c_out = static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem; p.c_pitch = c.d; p.c_fp32 = c.dhidden_fp32;
+      GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
+    }
+    if (dW_accum) {  // A6: dW[V, d] += dZ^T[V, rows] H[rows, d]
+      GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
+      GRPO_TRY(make_tmap(ctx, &tmH_mn, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, 64, BK));
+      GemmParams p;
+      std::memset(&p, 0, sizeof(p));
+      set_desc_defaults(p, true, true);
+      p.m_total = c.V; p.n_total = c.d;
+      p.m_tiles = (c.V + BM - 1) / BM; p.n_tiles = (c.d + BN - 1) / BN;
+      p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
+      p.n_fastest = 1;
+      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1;
+      GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st)));
+    }
+  }
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden, const void* W,
+                                               const int32_t* targets, const float* lse, const float* coeff,
+                                               int64_t T, float grad_scale, void* dhidden_out, float* dW_accum,
+                                               void* stream) {
+  if (!ctx || !hidden || !W || !targets || !lse || !coeff) return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0");
+  return bwd_impl(ctx, 0, hidden, W, targets, lse, coeff, T, grad_scale, dhidden_out, dW_accum,
+                  static_cast<cudaStream_t>(stream));
+}
+
+// ------------------------------------------------------------------------------------- A0 / A7: CGP FIFO
+extern "C" int32_t grpo_cgp_plan(const int64_t* group_tokens, int32_t n_pending, int32_t U, int64_t token_budget,
+                                 int32_t flush, int32_t* launch_sizes_out, int32_t cap, int32_t* n_launches_out) {
+  if (!n_launches_out || n_pending < 0 || (n_pending > 0 && !group_tokens))
+    return fail(GRPO_ERR_INVALID_ARG, "bad arguments");
+  std::vector<int> sizes;
+  plan_update(group_tokens, n_pending, U, token_budget, flush != 0, sizes);
+  if (static_cast<int>(sizes.size()) > cap) return fail(GRPO_ERR_INVALID_ARG, "launch_sizes_out too small");
+  for (size_t i = 0; i < sizes.size(); ++i) launch_sizes_out[i] = sizes[i];
+  *n_launches_out = static_cast<int32_t>(sizes.size());
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_queue_state(const grpo_ctx* ctx, int32_t* pending_groups, int64_t* pending_tokens,
+                                    int32_t* consumed_groups, int32_t* round_complete) {
+  if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL");
+  if (pending_groups) *pending_groups = static_cast<int32_t>(ctx->fifo.size());
+  if (pending_tokens) {
+    int64_t s = 0;
+    for (const auto& g : ctx->fifo) s += g.tokens;
+    *pending_tokens = s;
+  }
+  if (consumed_groups) *consumed_groups = ctx->consumed;
+  if (round_complete) *round_complete = (ctx->cfg.groups_per_round > 0 && ctx->consumed >= ctx->cfg.groups_per_round) ? 1 : 0;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_reset_round(grpo_ctx* ctx) {
+  if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL");
+  ctx->fifo.clear();
+  ctx->consumed = 0;
+  return GRPO_OK;
+}
+
+__global__ void token_count_flat_kernel(const uint8_t* __restrict__ mask, const int32_t* __restrict__ targets, int V,
+                                        int64_t T, float* __restrict__ total) {
+  int c = 0;
+  for (int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; t < T;
+       t += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+    const int y = targets[t];
+    c += ((mask == nullptr || mask[t] != 0) && y >= 0 && y < V) ? 1 : 0;
+  }
+  const float cf = warp_sum(static_cast<float>(c));
+  if ((threadIdx.x & 31) == 0 && cf != 0.f) atomicAdd(total, cf);
+}
+__global__ void fill_u8_kernel(uint8_t* p, int64_t n, uint8_t v) {
+  for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n;
+       i += static_cast<int64_t>(gridDim.x) * blockDim.x)
+    p[i] = v;
+}
+
+static int32_t validate_group(const grpo_ctx* ctx, const grpo_group_desc& g) {
+  if (g.G <= 0 || (ctx->cfg.group_size > 0 && g.G != ctx->cfg.group_size))
+    return fail(GRPO_ERR_INCOMPLETE_GROUP, "group %lld has G=%d, expected %d complete responses", (long long)g.group_order,
+                g.G, ctx->cfg.group_size);
+  if (!g.seqlens_host || !g.hidden || !g.targets || !g.old_logp || !g.rewards)
+    return fail(GRPO_ERR_INCOMPLETE_GROUP, "group %lld is missing hidden/targets/old_logp/rewards/seqlens",
+                (long long)g.group_order);
+  for (int i = 0; i < g.G; ++i)
+    if (g.seqlens_host[i] <= 0)
+      return fail(GRPO_ERR_INCOMPLETE_GROUP, "group %lld response %d has no tokens", (long long)g.group_order, i);
+  return GRPO_OK;
+}
+
+// One launch = A1 -> A2/A3 -> A4-A6 over `k` whole groups packed into one token stream.
+static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, const void* W, float* dW_accum,
+                          float* loss_accum, float* metrics_accum, double loss_denom, const float* denom_dev, int slot,
+                          cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  const SlotLayout& L = ctx->lay;
+  int64_t T = 0;
+  int S = 0;
+  bool any_ref = false, all_ref = true, any_mask = false, any_dh = false;
+  for (int i = 0; i < k; ++i) {
+    T += groups[i].tokens;
+    S += groups[i].desc.G;
+    any_ref |= groups[i].desc.ref_logp != nullptr;
+    all_ref &= groups[i].desc.ref_logp != nullptr;
+    any_mask |= groups[i].desc.mask != nullptr;
+    any_dh |= groups[i].desc.dhidden_out != nullptr;
+  }
+  if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "launch of %lld tokens exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
+  if (S > L.s_max) return fail(GRPO_ERR_WORKSPACE, "too many sequences in one launch");
+  if (any_ref && !all_ref) return fail(GRPO_ERR_INVALID_ARG, "ref_logp must be given for all groups of a launch or none");
+
+  // small host-built index arrays
+  std::vector<int32_t> cu_seq(S + 1, 0), cu_grp(k + 1, 0);
+  int s = 0;
+  for (int i = 0; i < k; ++i) {
+    for (int j = 0; j < groups[i].desc.G; ++j, ++s) cu_seq[s + 1] = cu_seq[s] + groups[i].seqlens[j];
+    cu_grp[i + 1] = s;
+  }
+  int32_t* d_cu_seq = slot_ptr<int32_t>(ctx, slot, L.off_cu_seq);
+  int32_t* d_cu_grp = slot_ptr<int32_t>(ctx, slot, L.off_cu_grp);
+  float* d_rewards = slot_ptr<float>(ctx, slot, L.off_rewards);
+  float* d_adv = slot_ptr<float>(ctx, slot, L.off_adv);
+  CU_OK(cudaMemcpyAsync(d_cu_seq, cu_seq.data(), (S + 1) * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(d_cu_grp, cu_grp.data(), (k + 1) * 4, cudaMemcpyHostToDevice, st));
+  for (int i = 0; i < k; ++i)
+    CU_OK(cudaMemcpyAsync(d_rewards + cu_grp[i], groups[i].desc.rewards, groups[i].desc.G * 4, cudaMemcpyDeviceToDevice, st));
+
+  // pack the token stream (a single group is used in place)
+  const void* hidden;
+  const int32_t* targets;
+  const float *old_logp, *ref_logp;
+  const uint8_t* mask;
+  const int dh_elem = c.dhidden_fp32 ? 4 : 2;
+  if (k == 1) {
+    hidden = groups[0].desc.hidden; targets = groups[0].desc.targets; old_logp = groups[0].desc.old_logp;
+    ref_logp = groups[0].desc.ref_logp; mask = groups[0].desc.mask;
+  } else {
+    uint8_t* sh = slot_ptr<uint8_t>(ctx, slot, L.off_hidden);
+    int32_t* stg = slot_ptr<int32_t>(ctx, slot, L.off_targets);
+    float* so = slot_ptr<float>(ctx, slot, L.off_old);
+    float* sr = slot_ptr<float>(ctx, slot, L.off_ref);
+    uint8_t* sm = slot_ptr<uint8_t>(ctx, slot, L.off_mask);
+    int64_t off = 0;
+    for (int i = 0; i < k; ++i) {
+      const grpo_group_desc& g = groups[i].desc;
+      const int64_t n = groups[i].tokens;
+      CU_OK(cudaMemcpyAsync(sh + off * c.d * 2, g.hidden, n * c.d * 2, cudaMemcpyDeviceToDevice, st));
+      CU_OK(cudaMemcpyAsync(stg + off, g.targets, n * 4, cudaMemcpyDeviceToDevice, st));
+      CU_OK(cudaMemcpyAsync(so + off, g.old_logp, n * 4, cudaMemcpyDeviceToDevice, st));
+      if (any_ref) CU_OK(cudaMemcpyAsync(sr + off, g.ref_logp, n * 4, cudaMemcpyDeviceToDevice, st));
+      if (any_mask) {
+        if (g.mask) CU_OK(cudaMemcpyAsync(sm + off, g.mask, n, cudaMemcpyDeviceToDevice, st));
+        else { fill_u8_kernel<<<64, 256, 0, st>>>(sm + off, n, 1); CU_OK(cudaGetLastError()); }
+      }
+      off += n;
+    }
+    hidden = sh; targets = stg; old_logp = so; ref_logp = any_ref ? sr : nullptr; mask = any_mask ? sm : nullptr;
+  }
+
+  GRPO_TRY(grpo_group_advantage(ctx, d_rewards, d_cu_grp, k, 0, d_adv, nullptr, st));
+
+  float* logp = (k == 1 && groups[0].desc.logp_out) ? groups[0].desc.logp_out : slot_ptr<float>(ctx, slot, L.off_logp);
+  float* lse = slot_ptr<float>(ctx, slot, L.off_lse);
+  float* coeff = slot_ptr<float>(ctx, slot, L.off_coeff);
+  GRPO_TRY(fwd_impl(ctx, slot, hidden, W, targets, d_cu_seq, S, T, d_adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
+                    logp, lse, coeff, loss_accum, metrics_accum, st));
+  void* dh = nullptr;
+  if (any_dh) dh = (k == 1) ? groups[0].desc.dhidden_out : static_cast<void*>(slot_ptr<uint8_t>(ctx, slot, L.off_dh));
+  GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st));
+  if (k > 1) {
+    int64_t off = 0;
+    for (int i = 0; i < k; ++i) {
+      const grpo_group_desc& g = groups[i].desc;
+      const int64_t n = groups[i].tokens;
+      if (g.dhidden_out)
+        CU_OK(cudaMemcpyAsync(g.dhidden_out, static_cast<uint8_t*>(dh) + off * c.d * dh_elem, n * c.d * dh_elem,
+                              cudaMemcpyDeviceToDevice, st));
+      if (g.logp_out) CU_OK(cudaMemcpyAsync(g.logp_out, logp + off, n * 4, cudaMemcpyDeviceToDevice, st));
+      off += n;
+    }
+  }
+  return GRPO_OK;
+}
+
+static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float* dW_accum, float* loss_accum,
+                                float* metrics_accum, double loss_denom, void* const* streams, int32_t n_streams,
+                                int32_t* boundary) {
+  *boundary = 0;
+  if (ctx->fifo.empty()) return GRPO_OK;
+  std::vector<int64_t> tokens;
+  tokens.reserve(ctx->fifo.size());
+  for (const auto& g : ctx->fifo) tokens.push_back(g.tokens);
+  std::vector<int> sizes;
+  const int take = plan_update(tokens.data(), static_cast<int>(tokens.size()), ctx->cfg.groups_per_update,
+                               ctx->cfg.token_budget, flush, sizes);
+  if (take == 0) return GRPO_OK;
+  if (!W || !loss_accum) return fail(GRPO_ERR_INVALID_ARG, "W / loss_accum is NULL");
+  if (n_streams < 1 || n_streams > ctx->n_slots)
+    return fail(GRPO_ERR_WORKSPACE, "n_streams=%d but workspace has %d slots", n_streams, ctx->n_slots);
+  std::vector<PendingGroup> upd(ctx->fifo.begin(), ctx->fifo.begin() + take);
+
+  // implicit denominator of the whole update: count loss-bearing tokens of all its groups first
+  const float* denom_dev = nullptr;
+  if (ctx->cfg.loss_agg == 0 && !(loss_denom > 0.0) && sizes.size() > 1) {
+    float* dd = ctx->denom_ring + (ctx->denom_next++ % kDenomRing);
+    cudaStream_t s0 = static_cast<cudaStream_t>(streams ? streams[ctx->launches % n_streams] : nullptr);
+    CU_OK(cudaMemsetAsync(dd, 0, 4, s0));
+    for (const auto& g : upd) {
+      token_count_flat_kernel<<<64, 256, 0, s0>>>(g.desc.mask, g.desc.targets, ctx->cfg.V, g.tokens, dd);
+      CU_OK(cudaGetLastError());
+    }
+    CU_OK(cudaEventRecord(ctx->denom_event, s0));
+    for (int i = 0; i < n_streams; ++i)
+      if (streams && streams[i] != s0) CU_OK(cudaStreamWaitEvent(static_cast<cudaStream_t>(streams[i]), ctx->denom_event, 0));
+    denom_dev = dd;
+  }
+  int pos = 0;
+  for (int k : sizes) {
+    const int slot = static_cast<int>(ctx->launches % n_streams);
+    cudaStream_t st = static_cast<cudaStream_t>(streams ? streams[slot] : nullptr);
+    GRPO_TRY(run_launch(ctx, upd.data() + pos, k, W, dW_accum, loss_accum, metrics_accum, loss_denom, denom_dev, slot, st));
+    ctx->launches++;
+    pos += k;
+  }
+  ctx->fifo.erase(ctx->fifo.begin(), ctx->fifo.begin() + take);
+  ctx->consumed += take;
+  *boundary = 1;
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_enqueue_groups(grpo_ctx* ctx, const grpo_group_desc* groups, int32_t n, const void* W,
+                                       float* dW_accum, float* loss_accum, float* metrics_accum, double loss_denom,
+                                       void* const* streams, int32_t n_streams, int32_t* groups_consumed_out,
+                                       int32_t* update_boundary_out) {
+  if (!ctx || n < 0 || (n > 0 && !groups)) return fail(GRPO_ERR_INVALID_ARG, "bad ctx / groups / n");
+  for (int i = 0; i < n; ++i) GRPO_TRY(validate_group(ctx, groups[i]));
+  if (static_cast<int64_t>(ctx->fifo.size()) + n > ctx->cfg.max_pending_groups)
+    return fail(GRPO_ERR_QUEUE_FULL, "FIFO holds %zu groups, capacity %d", ctx->fifo.size(), ctx->cfg.max_pending_groups);
+  for (int i = 0; i < n; ++i) {
+    PendingGroup pg;
+    pg.desc = groups[i];
+    pg.seqlens.assign(groups[i].seqlens_host, groups[i].seqlens_host + groups[i].G);
+    pg.desc.seqlens_host = nullptr;
+    pg.tokens = 0;
+    for (int32_t l : pg.seqlens) pg.tokens += l;
+    ctx->fifo.push_back(std::move(pg));
+  }
+  int32_t boundary = 0;
+  int32_t st = drain_one_update(ctx, false, W, dW_accum, loss_accum, metrics_accum, loss_denom, streams, n_streams, &boundary);
+  if (groups_consumed_out) *groups_consumed_out = ctx->consumed;
+  if (update_boundary_out) *update_boundary_out = boundary;
+  return st;
+}
+
+extern "C" int32_t grpo_flush(grpo_ctx* ctx, const void* W, float* dW_accum, float* loss_accum, float* metrics_accum,
+                              double loss_denom, void* const* streams, int32_t n_streams, int32_t* groups_consumed_out,
+                              int32_t* update_boundary_out) {
+  if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL");
+  int32_t boundary = 0;
+  int32_t st = drain_one_update(ctx, true, W, dW_accum, loss_accum, metrics_accum, loss_denom, streams, n_streams, &boundary);
+  if (groups_consumed_out) *groups_consumed_out = ctx->consumed;
+  if (update_boundary_out) *update_boundary_out = boundary;
+  return st;
+}
+
+// ------------------------------------------------------------------------------------- end to end over host buffers
+extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const int32_t* targets_host,
+                                  const int32_t* cu_seqlens_host, const float* rewards_host,
+                                  const float* old_logp_host, const float* ref_logp_host, const uint8_t* mask_host,
+                                  int32_t n_groups, int32_t G, int64_t T, const void* W, float* dW_accum,
+                                  double loss_denom, float* loss_host, float* logp_host, void* dhidden_host,
+                                  void* stream) {
+  if (!ctx || !hidden_host || !targets_host || !cu_seqlens_host || !rewards_host || !old_logp_host || !W || !loss_host)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (n_groups <= 0 || G <= 0 || T <= 0) return fail(GRPO_ERR_SHAPE, "need n_groups, G, T > 0");
+  if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
+  if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T exceeds workspace max_T");
+  const grpo_config& c = ctx->cfg;
+  const SlotLayout& L = ctx->lay;
+  const int S = n_groups * G;
+  if (S > L.s_max) return fail(GRPO_ERR_WORKSPACE, "too many sequences");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  uint8_t* sh = slot_ptr<uint8_t>(ctx, 0, L.off_hidden);
+  int32_t* stg = slot_ptr<int32_t>(ctx, 0, L.off_targets);
+  float* so = slot_ptr<float>(ctx, 0, L.off_old);
+  float* sr = slot_ptr<float>(ctx, 0, L.off_ref);
+  uint8_t* sm = slot_ptr<uint8_t>(ctx, 0, L.off_mask);
+  int32_t* d_cu = slot_ptr<int32_t>(ctx, 0, L.off_cu_seq);
+  float* d_rw = slot_ptr<float>(ctx, 0, L.off_rewards);
+  float* d_adv = slot_ptr<float>(ctx, 0, L.off_adv);
+  float* logp = slot_ptr<float>(ctx, 0, L.off_logp);
+  float* lse = slot_ptr<float>(ctx, 0, L.off_lse);
+  float* coeff = slot_ptr<float>(ctx, 0, L.off_coeff);
+  uint8_t* dh = slot_ptr<uint8_t>(ctx, 0, L.off_dh);
+  float* loss_dev = slot_ptr<float>(ctx, 0, L.off_total) + 8;   // scratch scalar inside the 256-byte cell
+  const int dh_elem = c.dhidden_fp32 ? 4 : 2;
+  CU_OK(cudaMemcpyAsync(sh, hidden_host, T * c.d * 2, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(stg, targets_host, T * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(so, old_logp_host, T * 4, cudaMemcpyHostToDevice, st));
+  if (ref_logp_host) CU_OK(cudaMemcpyAsync(sr, ref_logp_host, T * 4, cudaMemcpyHostToDevice, st));
+  if (mask_host) CU_OK(cudaMemcpyAsync(sm, mask_host, T, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(d_cu, cu_seqlens_host, (S + 1) * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(d_rw, rewards_host, S * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemsetAsync(loss_dev, 0, 4, st));
+  GRPO_TRY(grpo_group_advantage(ctx, d_rw, nullptr, n_groups, G, d_adv, nullptr, st));
+  GRPO_TRY(fwd_impl(ctx, 0, sh, W, stg, d_cu, S, T, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr,
+                    loss_denom, nullptr, logp, lse, coeff, loss_dev, nullptr, st));
+  GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st));
+  CU_OK(cudaMemcpyAsync(loss_host, loss_dev, 4, cudaMemcpyDeviceToHost, st));
+  if (logp_host) CU_OK(cudaMemcpyAsync(logp_host, logp, T * 4, cudaMemcpyDeviceToHost, st));
+  if (dhidden_host) CU_OK(cudaMemcpyAsync(dhidden_host, dh, T * c.d * dh_elem, cudaMemcpyDeviceToHost, st));
+  CU_OK(cudaStreamSynchronize(st));
+  return GRPO_OK;
+}
+
+// ------------------------------------------------------------------------------------- test hook
+extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A, const void* B, float* C, int32_t M,
+                                   int32_t N, int32_t K, int32_t accumulate, void* stream) {
+  if (!ctx || !A || !B || !C) return fail(GRPO_ERR_INVALID_ARG, "NULL pointer");
+  if (M <= 0 || N <= 0 || K <= 0 || (M % 8) || (N % 8) || (K % 8)) return fail(GRPO_ERR_SHAPE, "M, N, K must be positive multiples of 8");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  CUtensorMap tmA, tmB;
+  GemmParams p;
+  std::memset(&p, 0, sizeof(p));
+  p.m_total = M; p.n_total = N;
+  p.m_tiles = (M + BM - 1) / BM; p.n_tiles = (N + BN - 1) / BN; p.k_blocks = (K + BK - 1) / BK;
+  p.n_fastest = 1;
+  p.c_out = C; p.c_pitch = N; p.c_fp32 = 1;
+  const int units = p.m_tiles * p.n_tiles;
+  const bool a_mn = layout == 2, b_mn = layout >= 1;
+  set_desc_defaults(p, a_mn, b_mn);
+  if (!a_mn) GRPO_TRY(make_tmap(ctx, &tmA, A, K, M, static_cast<uint64_t>(K) * 2, BK, BM));
+  else GRPO_TRY(make_tmap(ctx, &tmA, A, M, K, static_cast<uint64_t>(M) * 2, 64, BK));
+  if (!b_mn) GRPO_TRY(make_tmap(ctx, &tmB, B, K, N, static_cast<uint64_t>(K) * 2, BK, BN));
+  else GRPO_TRY(make_tmap(ctx, &tmB, B, N, K, static_cast<uint64_t>(N) * 2, 64, BK));
+  if (layout == 0) {
+    if (accumulate) return launch_gemm<false, false, EPI_RED_F32>(ctx, tmA, tmB, p, units, st);
+    return launch_gemm<false, false, EPI_STORE>(ctx, tmA, tmB, p, units, st);
+  } else if (layout == 1) {
+    if (accumulate) return launch_gemm<false, true, EPI_RED_F32>(ctx, tmA, tmB, p, units, st);
+    return launch_gemm<false, true, EPI_STORE>(ctx, tmA, tmB, p, units, st);
+  } else if (layout == 2) {
+    if (accumulate) return launch_gemm<true, true, EPI_RED_F32>(ctx, tmA, tmB, p, units, st);
+    return launch_gemm<true, true, EPI_STORE>(ctx, tmA, tmB, p, units, st);
+  }
+  return fail(GRPO_ERR_INVALID_ARG, "layout must be 0, 1 or 2");
+}

@@ -1,0 +1,185 @@
+// HBM-bound per-group / per-token kernels of the GRPO step: A1 (group advantage), the mask counts that
+// define the mean, and A3 (partial-LSE combine + clipped surrogate + k3 + coefficient for the backward).
+#pragma once
+#include "ptx_sm100.cuh"
+
+namespace grpo {
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// A1 — Eq. 1: one warp per group; two-pass mean / variance in fp32.
+// A group whose rewards are all equal gets advantages that are exactly 0 (max == min test), so the
+// zero-advantage path does not depend on the rounding of the mean.
+__global__ void group_advantage_kernel(const float* __restrict__ rewards, const int32_t* __restrict__ cu_groups,
+                                       int n_groups, int G, float eps_std, int ddof, float* __restrict__ adv,
+                                       uint8_t* __restrict__ zero_var) {
+  const int g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (g >= n_groups) return;
+  const int beg = cu_groups ? cu_groups[g] : g * G;
+  const int end = cu_groups ? cu_groups[g + 1] : beg + G;
+  const int n = end - beg;
+  float s = 0.f, mx = -INFINITY, mn = INFINITY;
+  for (int i = beg + lane; i < end; i += 32) {
+    const float r = rewards[i];
+    s += r;
+    mx = fmaxf(mx, r);
+    mn = fminf(mn, r);
+  }
+  s = warp_sum(s);
+  mx = warp_max(mx);
+  mn = warp_min(mn);
+  const float mu = n > 0 ? s / static_cast<float>(n) : 0.f;
+  float ss = 0.f;
+  for (int i = beg + lane; i < end; i += 32) {
+    const float dlt = rewards[i] - mu;
+    ss += dlt * dlt;
+  }
+  ss = warp_sum(ss);
+  const int div = n - ddof;
+  const bool flat = !(mx > mn) || div <= 0;
+  const float sigma = flat ? 0.f : sqrtf(ss / static_cast<float>(div));
+  const float inv = 1.f / (sigma + eps_std);
+  for (int i = beg + lane; i < end; i += 32) adv[i] = flat ? 0.f : (rewards[i] - mu) * inv;
+  if (zero_var && lane == 0) zero_var[g] = flat ? 1 : 0;
+}
+
+// Loss-bearing token counts: per sequence (loss_agg 1) and total (loss_agg 0 with implicit denominator).
+// One warp per sequence.  A token counts iff mask != 0 and 0 <= target < V.
+__global__ void token_count_kernel(const uint8_t* __restrict__ mask, const int32_t* __restrict__ targets, int V,
+                                   const int32_t* __restrict__ cu_seqlens, int S, float* __restrict__ seq_count,
+                                   float* __restrict__ total) {
+  const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (s >= S) return;
+  int c = 0;
+  for (int t = cu_seqlens[s] + lane; t < cu_seqlens[s + 1]; t += 32) {
+    const int y = targets[t];
+    c += ((mask == nullptr || mask[t] != 0) && y >= 0 && y < V) ? 1 : 0;
+  }
+  const float cf = warp_sum(static_cast<float>(c));
+  if (lane == 0) {
+    if (seq_count) seq_count[s] = cf;
+    if (total) atomicAdd(total, cf);
+  }
+}
+
+struct LossParams {
+  int64_t T;
+  int S, V;
+  int n_split;
+  int64_t part_stride;
+  const float* part_m;
+  const float* part_s;
+  const float* zy;
+  const int32_t* targets;
+  const int32_t* cu_seqlens;
+  const float* adv;
+  const float* old_logp;
+  const float* ref_logp;     // nullable
+  const uint8_t* mask;       // nullable
+  const float* seq_count;    // loss_agg 1
+  const float* total_count;  // loss_agg 0, implicit denominator (device scalar)
+  float denom_host;          // > 0: explicit
+  int loss_agg;
+  float clip_lo, clip_hi, kl_beta;
+  float* logp;
+  float* lse;
+  float* coeff;
+  float* loss_accum;
+  float* metrics_accum;      // nullable, [4]
+  int32_t* err_flag;
+};
+
+// A3.  One thread per packed token; block-level reduction, then one atomic per block and quantity.
+__global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) {
+  const int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  float loss_t = 0.f, m_cnt = 0.f, m_rho = 0.f, m_k3 = 0.f, m_clip = 0.f;
+  if (t < p.T) {
+    // combine the per-split (max, sum 2^(z2 - max)) pairs -> natural-log lse
+    float M = -INFINITY;
+    for (int i = 0; i < p.n_split; ++i) M = fmaxf(M, p.part_m[i * p.part_stride + t]);
+    float sum = 0.f;
+    for (int i = 0; i < p.n_split; ++i)
+      sum += p.part_s[i * p.part_stride + t] * exp2f(p.part_m[i * p.part_stride + t] - M);
+    const float lse = (M + log2f(sum)) * kLn2;
+    const int y = p.targets[t];
+    const bool valid = y >= 0 && y < p.V;
+    if (y >= p.V) atomicOr(p.err_flag, 1);
+    const float logp = valid ? p.zy[t] - lse : 0.f;
+    // sequence of this token: largest s with cu_seqlens[s] <= t
+    int lo = 0, hi = p.S;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (static_cast<int64_t>(p.cu_seqlens[mid]) <= t) lo = mid; else hi = mid;
+    }
+    const float A = p.adv[lo];
+    const float m = (valid && (p.mask == nullptr || p.mask[t] != 0)) ? 1.f : 0.f;
+    float w;
+    if (p.loss_agg == 0) {
+      const float denom = p.denom_host > 0.f ? p.denom_host : fmaxf(*p.total_count, 1.f);
+      w = m / denom;
+    } else {
+      w = m / (fmaxf(p.seq_count[lo], 1.f) * static_cast<float>(p.S));
+    }
+    float coeff = 0.f;
+    if (m != 0.f) {
+      const float rho = expf(logp - p.old_logp[t]);
+      const float lo_b = 1.f - p.clip_lo, hi_b = 1.f + p.clip_hi;
+      const float surr = fminf(rho * A, fminf(fmaxf(rho, lo_b), hi_b) * A);
+      const bool clipped = (A > 0.f && rho > hi_b) || (A < 0.f && rho < lo_b);
+      float k3 = 0.f, dk3 = 0.f;
+      if (p.kl_beta != 0.f && p.ref_logp != nullptr) {
+        const float delta = p.ref_logp[t] - logp;
+        const float e = expf(delta);
+        k3 = e - delta - 1.f;
+        dk3 = 1.f - e;
+      }
+      loss_t = w * (-surr + p.kl_beta * k3);
+      coeff = w * ((clipped ? 0.f : -A * rho) + p.kl_beta * dk3);
+      m_cnt = 1.f;
+      m_rho = rho;
+      m_k3 = k3;
+      m_clip = clipped ? 1.f : 0.f;
+    }
+    p.logp[t] = logp;
+    p.lse[t] = lse;
+    p.coeff[t] = coeff;
+  }
+  __shared__ float red[5][8];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float vals[5] = {loss_t, m_cnt, m_rho, m_k3, m_clip};
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    const float r = warp_sum(vals[q]);
+    if (lane == 0) red[q][warp] = r;
+  }
+  __syncthreads();
+  if (warp == 0) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      float r = lane < 8 ? red[q][lane] : 0.f;
+      r = warp_sum(r);
+      if (lane == 0 && r != 0.f) {
+        if (q == 0) atomicAdd(p.loss_accum, r);
+        else if (p.metrics_accum) atomicAdd(p.metrics_accum + (q - 1), r);
+      }
+    }
+  }
+}
+
+}  // namespace grpo

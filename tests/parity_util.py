@@ -1,0 +1,102 @@
+"""Helpers shared by the GPU parity tests: run the CUDA path through the C ABI, run the oracle on the
+same bits, and compute the gates of BASELINE.json north_star plus the sub-block gates of SURVEY §8(c)."""
+import numpy as np
+import torch
+
+from oracle.grpo_oracle import OracleConfig, grpo_step
+
+TOL_LOGP_ABS = 2e-3      # per-token log-prob abs err (north_star)
+TOL_LOSS_REL = 1e-3      # loss rel err, relative to max(|loss|, sum |w l|) (R21)
+TOL_GRAD_REL = 1e-2      # dHidden / dW rel L2 (north_star)
+
+
+def oracle_cfg(b, **kw):
+    return OracleConfig(eps_std=b.eps_std, clip_lo=b.clip_lo, clip_hi=b.clip_hi, kl_beta=b.kl_beta,
+                        loss_agg=b.loss_agg, **kw)
+
+
+def run_oracle(b, loss_denom=None, std_ddof=0, logit_scale=1.0, need_grads=True, chunk=1024):
+    x = b.numpy_f64()
+    cfg = oracle_cfg(b, std_ddof=std_ddof, logit_scale=logit_scale, chunk_tokens=chunk)
+    return grpo_step(x["H"], x["W"], x["y"], x["cu_seqlens"], x["rewards"], x["old_logp"], x["ref_logp"],
+                     mask=x["mask"], cfg=cfg, G=b.G, loss_denom=loss_denom, need_grads=need_grads)
+
+
+def make_ctx(b, **kw):
+    from paper_2606_26997_b200 import GrpoContext
+    args = dict(eps_std=b.eps_std, clip_lo=b.clip_lo, clip_hi=b.clip_hi, kl_beta=b.kl_beta, loss_agg=b.loss_agg,
+                group_size=b.G)
+    args.update(kw)
+    return GrpoContext(b.d, b.V, **args)
+
+
+def run_cuda(ctx, b, loss_denom=0.0, want_dw=True, want_dh=True, grad_scale=1.0):
+    dev = b.hidden.device
+    adv, zv = ctx.grpo_group_advantage(b.rewards, G=b.G, want_zero_var=True)
+    metrics = torch.zeros(4, dtype=torch.float32, device=dev)
+    f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                        b.mask, loss_denom=loss_denom, metrics_accum=metrics)
+    dW = torch.zeros(b.V, b.d, dtype=torch.float32, device=dev) if want_dw else None
+    dH = ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW,
+                                         grad_scale=grad_scale, want_dhidden=want_dh)
+    torch.cuda.synchronize()
+    return dict(adv=adv, zero_var=zv, metrics=metrics, dW=dW, dH=dH, **f)
+
+
+def rel_l2(a, r):
+    a = np.asarray(a, dtype=np.float64)
+    r = np.asarray(r, dtype=np.float64)
+    return float(np.linalg.norm(a - r) / max(np.linalg.norm(r), 1e-300))
+
+
+def to64(t):
+    return t.detach().double().cpu().numpy()
+
+
+def gates(b, out, ref, check_grads=True, logit_scale=1.0):
+    """Return dict of errors; caller asserts against the TOL_* constants."""
+    e = {}
+    e["adv_abs"] = float(np.abs(to64(out["adv"]) - ref["adv"]).max())
+    e["logp_abs"] = float(np.abs(to64(out["logp"]) - ref["logp"]).max())
+    e["lse_abs"] = float(np.abs(to64(out["lse"]) - ref["lse"]).max())
+    e["loss_rel"] = abs(out["loss"].item() - ref["loss"]) / max(abs(ref["loss"]), ref["abs_loss"], 1e-300)
+    cn = np.linalg.norm(ref["coeff"])
+    e["coeff_rel"] = rel_l2(to64(out["coeff"]), ref["coeff"]) if cn > 0 else float(np.abs(to64(out["coeff"])).max())
+    if check_grads:
+        dH, dW = to64(out["dH"]), to64(out["dW"])
+        e["dH_rel"] = rel_l2(dH, ref["dH"]) if np.linalg.norm(ref["dH"]) > 0 else float(np.abs(dH).max())
+        e["dW_rel"] = rel_l2(dW, ref["dW"]) if np.linalg.norm(ref["dW"]) > 0 else float(np.abs(dW).max())
+        # (i) rows of dW for vocab ids that never appear as a target: the dense softmax term alone
+        y = b.targets.cpu().numpy()
+        non_target = np.ones(b.V, dtype=bool)
+        non_target[y[(y >= 0) & (y < b.V)]] = False
+        if non_target.any() and np.linalg.norm(ref["dW"][non_target]) > 0:
+            e["dW_nontarget_rel"] = rel_l2(dW[non_target], ref["dW"][non_target])
+        # (ii) dH minus the one-hot part  c_t s W[y_t]: the sum_v p_tv W[v] part alone.  The bf16 rounding of
+        # the one-hot dZ entry (rel 2^-9 of the ONE-HOT part) bounds how well this can be resolved, so the
+        # error is reported relative to ||dense|| + 2.5e-3 ||onehot||; only meaningful for fp32 dH output.
+        if out["dH"].dtype == torch.float32:
+            W64 = b.W.double().cpu().numpy()
+            yy = np.clip(y, 0, b.V - 1)
+            onehot = (ref["coeff"] * ((y >= 0) & (y < b.V)))[:, None] * W64[yy] * logit_scale
+            dense_ref = ref["dH"] - onehot
+            if np.linalg.norm(dense_ref) > 0:
+                e["dH_dense_rel"] = float(np.linalg.norm((dH - onehot) - dense_ref) /
+                                          (np.linalg.norm(dense_ref) + 2.5e-3 * np.linalg.norm(onehot)))
+        # (iii) rows of dZ sum to zero => sum_v dW[v,:] = 0 (P7); scale: bf16 rounding of dZ entries
+        e["dW_colsum_rel"] = float(np.linalg.norm(dW.sum(0)) / max(np.linalg.norm(dW), 1e-300))
+    return e
+
+
+def assert_gates(e, check_grads=True):
+    assert e["adv_abs"] <= 1e-5, e
+    assert e["logp_abs"] <= TOL_LOGP_ABS, e
+    assert e["loss_rel"] <= TOL_LOSS_REL, e
+    assert e["coeff_rel"] <= 1e-3, e
+    if check_grads:
+        assert e["dH_rel"] <= TOL_GRAD_REL, e
+        assert e["dW_rel"] <= TOL_GRAD_REL, e
+        if "dW_nontarget_rel" in e:
+            assert e["dW_nontarget_rel"] <= TOL_GRAD_REL, e
+        if "dH_dense_rel" in e:
+            assert e["dH_dense_rel"] <= 1e-2, e

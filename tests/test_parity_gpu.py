@@ -1,0 +1,160 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the float64 oracle on the same seeded
+inputs, element by element.  Tolerances are BASELINE.json north_star's: per-token log-prob abs err
+<= 2e-3, loss rel err <= 1e-3, dHidden / dW rel-L2 <= 1e-2 (bf16 inputs, fp32 accumulation)."""
+import numpy as np
+import pytest
+import torch
+
+from tests.parity_util import (TOL_GRAD_REL, TOL_LOGP_ABS, assert_gates, gates, make_ctx, rel_l2, run_cuda,
+                               run_oracle, to64)
+from workloads.synth import make_config, slice_groups
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_2606_26997_b200.build import build
+    build()
+
+
+def _check(b, ctx_kw=None, oracle_kw=None, loss_denom=0.0, grad_scale=1.0):
+    ctx = make_ctx(b, **(ctx_kw or {}))
+    try:
+        out = run_cuda(ctx, b, loss_denom=loss_denom, grad_scale=grad_scale)
+        assert ctx.grpo_check_errors_sync() == 0
+    finally:
+        ctx.close()
+    okw = dict(oracle_kw or {})
+    ref = run_oracle(b, loss_denom=loss_denom if loss_denom > 0 else None, **okw)
+    if grad_scale != 1.0:
+        ref["dH"] *= grad_scale
+        ref["dW"] *= grad_scale
+    e = gates(b, out, ref, logit_scale=okw.get("logit_scale", 1.0))
+    assert_gates(e)
+    return out, ref, e
+
+
+# ------------------------------------------------------------------ BASELINE config 1 and variants
+def test_config1_exact_shape():
+    b = make_config(1, device="cuda")
+    out, ref, e = _check(b)
+    np.testing.assert_allclose(to64(out["metrics"]), ref["metrics"], rtol=1e-4, atol=1e-4)
+    assert e["dW_colsum_rel"] < 2e-3
+
+
+def test_config1b_clip_regions_populated():
+    b = make_config(1, device="cuda", variant="1b")
+    out, ref, e = _check(b)
+    frac = (ref["u"] == 0).mean()
+    assert 0.1 < frac < 0.9
+    assert to64(out["metrics"])[3] == ref["metrics"][3]          # same tokens clipped
+
+
+@pytest.mark.parametrize("kw", [
+    dict(mask_frac=0.25), dict(loss_agg=1), dict(loss_agg=1, mask_frac=0.3), dict(bad_target_frac=0.15),
+    dict(kl_beta=0.0), dict(kl_beta=0.05), dict(w_std=0.5), dict(w_std=1.5, variant="1b"),
+])
+def test_config1_variants(kw):
+    b = make_config(1, device="cuda", seed=3, variant=kw.pop("variant", "1b"), **kw)
+    _check(b, ctx_kw=dict(dhidden_fp32=1))
+
+
+def test_sample_std_and_temperature():
+    b = make_config(1, device="cuda", seed=4, variant="1b", w_std=0.3)
+    _check(b, ctx_kw=dict(std_ddof=1, logit_scale=0.7), oracle_kw=dict(std_ddof=1, logit_scale=0.7))
+    _check(b, ctx_kw=dict(logit_scale=1.9, dhidden_fp32=1), oracle_kw=dict(logit_scale=1.9), grad_scale=0.25)
+
+
+def test_explicit_denominator_and_homogeneity():
+    b = make_config(1, device="cuda", seed=5, variant="1b")
+    out1, _, _ = _check(b, loss_denom=float(b.T))
+    out2, _, _ = _check(b, loss_denom=float(b.T) / 4.0)
+    np.testing.assert_allclose(out2["loss"].item(), 4 * out1["loss"].item(), rtol=1e-5)
+    assert rel_l2(to64(out2["dW"]), 4 * to64(out1["dW"])) < 2e-3
+
+
+def test_zero_variance_groups_give_exact_zeros():
+    b = make_config(1, device="cuda", seed=6, kl_beta=0.0)
+    b.rewards = torch.tensor([1.0] * 4 + [0.0] * 4 + [1, 0, 1, 0] + [0.5] * 4, device="cuda")
+    out, ref, _ = _check(b)
+    zv = out["zero_var"].cpu().numpy()
+    np.testing.assert_array_equal(zv, [1, 1, 0, 1])
+    cu = b.cu_seqlens.cpu().numpy()
+    dH = out["dH"].float().cpu().numpy()
+    for g in (0, 1, 3):
+        assert np.all(to64(out["adv"])[4 * g:4 * g + 4] == 0.0)
+        assert np.all(dH[cu[4 * g]:cu[4 * g + 4]] == 0.0)          # zero advantage, beta = 0 => zero gradient
+    assert np.any(dH[cu[8]:cu[12]] != 0.0)
+
+
+def test_all_masked_gives_zero_loss_and_grads():
+    b = make_config(1, device="cuda", seed=7)
+    b.mask = torch.zeros(b.T, dtype=torch.uint8, device="cuda")
+    ctx = make_ctx(b)
+    out = run_cuda(ctx, b)
+    ctx.close()
+    assert out["loss"].item() == 0.0
+    assert torch.all(out["dW"] == 0) and torch.all(out["dH"].float() == 0)
+
+
+def test_out_of_range_target_sets_error_flag():
+    b = make_config(1, device="cuda", seed=8)
+    b.targets[5] = b.V + 7
+    ctx = make_ctx(b)
+    out = run_cuda(ctx, b)
+    assert ctx.grpo_check_errors_sync() == 1
+    assert ctx.grpo_check_errors_sync() == 0                         # cleared by the read
+    ctx.close()
+    ref = run_oracle(b)
+    assert abs(out["loss"].item() - ref["loss"]) <= 1e-3 * max(abs(ref["loss"]), ref["abs_loss"])
+
+
+# ------------------------------------------------------------------ several tiles, ragged tails, chunked backward
+@pytest.mark.parametrize("d,V,len_div,chunk", [(256, 5000, 20, 0), (72, 1000, 40, 0), (128, 3000, 10, 1024),
+                                               (512, 2504, 30, 512)])
+def test_config3_shaped_midsize(d, V, len_div, chunk):
+    b = make_config(3, device="cuda", d=d, V=V, len_div=len_div, w_std=0.08)
+    assert b.zero_var_frac > 0
+    kw = dict(bwd_chunk_tokens=chunk) if chunk else {}
+    _check(b, ctx_kw=kw)
+
+
+def test_config4_shaped_large_groups():
+    b = make_config(4, device="cuda", d=128, V=4096, len_div=40)
+    _check(b)
+
+
+def test_single_token_and_tiny():
+    b = make_config(1, device="cuda", seed=9, n_groups=1, G=2, len_div=100.0)   # every response 1 token
+    assert b.T == 2
+    _check(b)
+
+
+# ------------------------------------------------------------------ determinism of the forward, run-to-run
+def test_forward_is_deterministic():
+    b = make_config(3, device="cuda", d=256, V=5000, len_div=20)
+    ctx = make_ctx(b)
+    a = run_cuda(ctx, b, want_dw=False, want_dh=False)
+    c = run_cuda(ctx, b, want_dw=False, want_dh=False)
+    ctx.close()
+    assert torch.equal(a["logp"], c["logp"]) and torch.equal(a["coeff"], c["coeff"])
+
+
+# ------------------------------------------------------------------ end-to-end over host buffers == device path
+def test_step_host_matches_device_path():
+    b = make_config(3, device="cuda", d=256, V=5000, len_div=20)
+    ctx = make_ctx(b)
+    out = run_cuda(ctx, b)
+    pin = lambda t: None if t is None else t.cpu().pin_memory()
+    dW = torch.zeros_like(out["dW"])
+    logp_h = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    dh_h = torch.empty(b.T, b.d, dtype=torch.bfloat16).pin_memory()
+    loss_h = ctx.grpo_step_host(pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards), pin(b.old_logp),
+                                b.n_groups, b.G, b.W, dW, ref_logp_h=pin(b.ref_logp), mask_h=pin(b.mask),
+                                logp_h=logp_h, dhidden_h=dh_h)
+    ctx.close()
+    assert torch.equal(logp_h, out["logp"].cpu())
+    np.testing.assert_allclose(loss_h.item(), out["loss"].item(), rtol=1e-5)
+    assert torch.equal(dh_h, out["dH"].cpu())
+    assert rel_l2(to64(dW), to64(out["dW"])) < 1e-5

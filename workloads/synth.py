@@ -148,7 +148,8 @@ def base_logp_and_targets(H, W, gen, sample: str, chunk: int = 2048):
 def make_config(cfg: int, seed: int = 0, device="cpu", *, d: int | None = None, V: int | None = None,
                 n_groups: int | None = None, G: int | None = None, len_div: float = 1.0,
                 old_sigma: float | None = None, kl_beta: float | None = None,
-                mask_frac: float = 0.0, loss_agg: int = 0, variant: str = "") -> GrpoBatch:
+                mask_frac: float = 0.0, loss_agg: int = 0, variant: str = "", w_std: float = 0.02,
+                bad_target_frac: float = 0.0) -> GrpoBatch:
     """Build config ``cfg`` (1-5).  Keyword overrides shrink it for CPU-sized parity cases.
 
     variant "1b": config 1 with old-logprob noise sigma = 0.3 so both clip regions are
@@ -169,7 +170,7 @@ def make_config(cfg: int, seed: int = 0, device="cpu", *, d: int | None = None, 
     dev = torch.device(device)
     gen = torch.Generator(device=dev)
     gen.manual_seed(base_seed)
-    W = (torch.randn(V, d, generator=gen, device=dev, dtype=torch.float32) * 0.02).to(torch.bfloat16)
+    W = (torch.randn(V, d, generator=gen, device=dev, dtype=torch.float32) * w_std).to(torch.bfloat16)
     Hf = torch.randn(T, d, generator=gen, device=dev, dtype=torch.float32)
     if cfg != 1:   # "after RMSNorm-like scaling": unit-RMS rows (R16)
         Hf = Hf * torch.rsqrt(Hf.pow(2).mean(dim=1, keepdim=True) + 1e-12)
@@ -185,6 +186,9 @@ def make_config(cfg: int, seed: int = 0, device="cpu", *, d: int | None = None, 
     mask = None
     if mask_frac > 0.0:
         mask = (torch.rand(T, generator=gen, device=dev) >= mask_frac).to(torch.uint8)
+    if bad_target_frac > 0.0:   # ignored tokens (y < 0) — exercises DESIGN.md R13
+        bad = torch.rand(T, generator=gen, device=dev) < bad_target_frac
+        y = torch.where(bad, torch.full_like(y, -100), y)
     cu = np.concatenate([[0], np.cumsum(seqlens)]).astype(np.int32)
     arrival = rng.permutation(n_groups) if cfg == 5 else None
     return GrpoBatch(
