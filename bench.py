@@ -1,0 +1,366 @@
+#!/usr/bin/env python
+"""bench.py — GRPO loss fwd+bwd tokens/s at d=2048, V=151936 on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path (group advantage, LM-head
+contraction + online log-sum-exp, loss epilogue, backward recompute + dZ, dH, dW accumulation) over one
+batch of synthetic input.  At N=1 the workload is BASELINE.json configs[1]: one complete group, G=8
+responses of 512..4096 tokens, d=2048, V=151936 (Qwen3-1.7B LM-head shape), on-policy old log-probs,
+no KL.  With N>1 (torchrun, one rank per GPU) every rank runs its own complete group (weak scaling over
+independent groups; the path has no collective — DESIGN.md §7); the only torch.distributed traffic is
+the barrier and the max/sum of the measurements.
+
+Output: ONE JSON line on rank 0 (keys documented in DESIGN.md §6).
+`--impl reference` times the float64 CPU oracle (oracle/) on the host cores, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "GRPO loss fwd+bwd tokens/sec at d=2048,V=151936; % of B200 BF16 tensor peak"
+UNIT = "tokens/s"
+SAMPLE_LEN_DIV = 32.0          # oracle sample: configs[1] with response lengths / 32 (T ~ 570), full d and V
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback"
+    return d
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event reasons of one GPU with NVML while the timed region runs."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+               0x10: "sync_boost"}
+
+    def __init__(self, torch_index: int, period_s: float = 0.05):
+        self.period = period_s
+        self.samples = []
+        self.mask = 0
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        self.h = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = "GPU-" + str(torch.cuda.get_device_properties(torch_index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:      # NVML missing: report that, never fake a clock
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    self.mask |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.h is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr is not None:
+            self._stop.set()
+            self._thr.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        reasons = [name for bit, name in self.REASONS.items() if self.mask & bit]
+        return {"sm_mhz": int(statistics.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "sm_min_mhz": min(self.samples), "samples": len(self.samples), "reasons": reasons}
+
+
+# ----------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(device="cpu"):
+    """Bounded sample of the timed workload for the CPU oracle: configs[1] with lengths / SAMPLE_LEN_DIV."""
+    from workloads.synth import make_config
+    b = make_config(2, seed=0, device=device, len_div=SAMPLE_LEN_DIV)
+    return b.to("cpu") if device != "cpu" else b
+
+
+def time_oracle_step(b):
+    """One fwd+bwd of the oracle as it stands on sample `b`; returns seconds."""
+    from oracle.grpo_oracle import OracleConfig, grpo_step
+    x = b.numpy_f64()
+    cfg = OracleConfig(eps_std=b.eps_std, clip_lo=b.clip_lo, clip_hi=b.clip_hi, kl_beta=b.kl_beta, loss_agg=b.loss_agg)
+    t0 = time.perf_counter()
+    out = grpo_step(x["H"], x["W"], x["y"], x["cu_seqlens"], x["rewards"], x["old_logp"], x["ref_logp"],
+                    mask=x["mask"], cfg=cfg, G=b.G)
+    dt = time.perf_counter() - t0
+    assert out["dW"].shape == x["W"].shape
+    return dt
+
+
+def oracle_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 0) for p in threadpool_info() if p.get("user_api") == "blas"]
+        if n:
+            return int(max(n))
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def sample_desc(b):
+    return (f"configs[1] with response lengths/{SAMPLE_LEN_DIV:g}: 1 group x G={b.G}, T={b.T} tokens, d={b.d}, "
+            f"V={b.V}; one oracle fwd+bwd (float64, numpy/OpenBLAS) per step")
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    b = oracle_sample("cpu")
+    for _ in range(args.warmup):
+        time_oracle_step(b)
+    times = [time_oracle_step(b) for _ in range(args.steps)]
+    total = sum(times)
+    value = b.T * args.steps / total
+    cores = oracle_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[1]: one complete group G=8, lengths U[512,4096], d=2048, V=151936 "
+                               "(bounded sample, see cpu_baseline.sample)", "tokens_per_step": b.T},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_desc(b)},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------- CUDA arm
+GEMM_KINDS = ("gemm_lse", "gemm_dz", "gemm_dh", "gemm_dw")
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_26997_b200 import GrpoContext
+    from paper_2606_26997_b200.build import build
+    from workloads.synth import make_config
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference "
+                         "for the oracle baseline)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if local == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
+    b = make_config(2, seed=rank, device=dev)
+    T, d, V = b.T, b.d, b.V
+    ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi)
+    dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
+    loss = torch.zeros(1, dtype=torch.float32, device=dev)
+    dH = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
+
+    def step():
+        adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+        f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                            b.mask, loss_accum=loss)
+        ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW, dhidden_out=dH)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    assert ctx.grpo_check_errors_sync() == 0
+    dW.zero_()
+    loss.zero_()
+
+    # ---- timed region: K steps, CUDA events on the launch stream, per-kernel events inside the library
+    sampler = ClockSampler(local)
+    n0 = ctx.grpo_kernel_launches()
+    ctx.grpo_profile_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    prof = ctx.grpo_profile_read_sync()
+    ctx.grpo_profile_enable(False)
+    n1 = ctx.grpo_kernel_launches()
+    launches = sum(n1.values()) - sum(n0.values())
+    loss_val = loss.item()
+    assert loss_val == loss_val, "loss is NaN"
+
+    # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step
+    pin = lambda t: None if t is None else t.cpu().pin_memory()
+    h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
+                                                   pin(b.old_logp))
+    h_logp = torch.empty(T, dtype=torch.float32).pin_memory()
+    h_dh = torch.empty(T, d, dtype=torch.bfloat16).pin_memory()
+    h_loss = torch.zeros(1, dtype=torch.float32).pin_memory()
+
+    def step_host():
+        ctx.grpo_step_host(h_hidden, h_targets, h_cu, h_rewards, h_old, b.n_groups, b.G, b.W, dW, loss_h=h_loss,
+                           logp_h=h_logp, dhidden_h=h_dh)
+
+    for _ in range(2):
+        step_host()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_host()                     # synchronises its stream before returning: the host has the results
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    barrier()
+    h2d = sum(t.numel() * t.element_size() for t in (h_hidden, h_targets, h_cu, h_rewards, h_old))
+    d2h = sum(t.numel() * t.element_size() for t in (h_logp, h_dh, h_loss))
+
+    # ---- reduce over ranks: max time, sum tokens
+    stats = torch.tensor([ms_total, e2e_s], dtype=torch.float64, device=dev)
+    toks = torch.tensor([float(T)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
+        dist.all_reduce(toks, op=dist.ReduceOp.SUM)
+    ms_total, e2e_s = stats.tolist()
+    tokens_all = toks.item()
+    value = tokens_all * args.steps / (ms_total * 1e-3)
+    e2e_value = tokens_all * args.steps / e2e_s
+
+    if rank == 0:
+        peaks = load_peaks()
+        line = build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, prof, clocks, peaks,
+                          tokens_all, loss_val)
+        if world == 1 and not args.no_cpu_baseline:
+            sb = oracle_sample(dev)
+            dt = time_oracle_step(sb)
+            line["cpu_baseline"] = {"value": sb.T / dt, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
+                                    "sample": sample_desc(sb), "seconds": dt}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, prof, clocks, peaks, tokens_all,
+               loss_val):
+    T, d, V = b.T, b.d, b.V
+    steps = args.steps
+    flops_per_gemm_step = 2.0 * T * V * d                 # each of A2, A4, A5, A6 (rank 0's tokens)
+    # the kernels are timed inside a long step (hundreds of ms of back-to-back tensor work), so the
+    # denominator is the SUSTAINED measured bf16 matmul rate; the burst figure is reported beside it
+    peak = float(peaks.get("bf16_tflops_sustained") or peaks["bf16_tflops"])
+    peak_burst = float(peaks["bf16_tflops"])
+    kernels = {}
+    for k, v in prof.items():
+        if v["launches"] == 0:
+            continue
+        e = {"ms_per_step": v["ms"] / steps, "launches_per_step": v["launches"] / steps}
+        if k in GEMM_KINDS:
+            e["tflops"] = flops_per_gemm_step * steps / (v["ms"] * 1e-3) / 1e12
+            e["frac_of_peak"] = e["tflops"] / peak
+        kernels[k] = e
+    gemm_ms = sum(prof[k]["ms"] for k in GEMM_KINDS)
+    dom = max(GEMM_KINDS, key=lambda k: prof[k]["ms"])
+    dom_tflops = kernels[dom]["tflops"]
+    path_tflops = 4 * flops_per_gemm_step * steps / (gemm_ms * 1e-3) / 1e12
+    step_tflops = 4 * flops_per_gemm_step * steps / (ms_total * 1e-3) / 1e12 if world == 1 else None
+    roofline = {
+        "bound": "tensor", "kernel": dom, "achieved": dom_tflops, "peak": peak, "unit": "TFLOP/s",
+        "frac": dom_tflops / peak, "traffic": NCU_TRAFFIC_BYTES.get(dom),
+        "peak_source": f"{peaks['_source']} bf16_tflops_sustained (MEASURED_PEAKS.json); burst {peak_burst:g}",
+        "frac_of_burst": dom_tflops / peak_burst,
+        "flops_per_launch": flops_per_gemm_step / kernels[dom]["launches_per_step"],
+        "all_gemms": {"achieved": path_tflops, "frac": path_tflops / peak, "share_of_step": gemm_ms / ms_total},
+        "whole_step": None if step_tflops is None else {"achieved": step_tflops, "frac": step_tflops / peak,
+                                                        "flops_basis": "8*T*V*d executed (4 contractions)"},
+    }
+    return {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "configs[1]: one complete group G=8, lengths U[512,4096], d=2048, V=151936, "
+                               "on-policy old log-probs, no KL; one such group per GPU",
+                   "tokens_per_step": int(tokens_all), "tokens_rank0": T, "d": d, "V": V, "G": b.G,
+                   "parallelism": f"replicas x{world}: independent complete groups, no collective",
+                   "l2": "inputs larger than L2 (W 622 MB, dW 1.2 GB, dZ chunk 2.9 GB vs 126 MB L2); no flush needed",
+                   "bwd_chunk_tokens": 9472},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "api": "grpo_step_host (C ABI, pinned host buffers; W and dW resident on the device)"},
+        "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
+        "loss_after_steps": loss_val,
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: launch with torch.distributed.run --nproc-per-node "
+                             f"{args.gpus} (one rank per GPU)")
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -174,6 +174,29 @@ int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const int32_t* ta
                        int64_t T, const void* W, float* dW_accum, double loss_denom, float* loss_host,
                        float* logp_host, void* dhidden_host, void* stream);
 
+/* Kernel accounting.  Every kernel this library launches belongs to one kind. */
+enum {
+  GRPO_KERNEL_ADVANTAGE = 0,   /* A1 */
+  GRPO_KERNEL_TOKEN_COUNT = 1, /* mask counts / fills that define the mean */
+  GRPO_KERNEL_GEMM_LSE = 2,    /* A2: z = H W^T with the online log-sum-exp epilogue */
+  GRPO_KERNEL_LOSS = 3,        /* A3 */
+  GRPO_KERNEL_GEMM_DZ = 4,     /* A4: recompute z, dZ epilogue */
+  GRPO_KERNEL_GEMM_DH = 5,     /* A5: dH = dZ W */
+  GRPO_KERNEL_GEMM_DW = 6,     /* A6: dW += dZ^T H */
+  GRPO_KERNEL_DEBUG = 7,       /* grpo_debug_gemm */
+  GRPO_NUM_KERNEL_KINDS = 8
+};
+
+/* counts_out HOST int64 [GRPO_NUM_KERNEL_KINDS]: kernels launched by this context since creation. */
+int32_t grpo_kernel_launches(const grpo_ctx* ctx, int64_t* counts_out);
+
+/* While enabled, every kernel launch is bracketed by CUDA events recorded on its launch stream.
+ * grpo_profile_read_sync synchronises the device, sums the elapsed milliseconds per kind into
+ * ms_out (HOST double [GRPO_NUM_KERNEL_KINDS]) with the number of timed launches in launches_out
+ * (HOST int64 [GRPO_NUM_KERNEL_KINDS]), and clears the records.  Disabling discards records. */
+int32_t grpo_profile_enable(grpo_ctx* ctx, int32_t on);
+int32_t grpo_profile_read_sync(grpo_ctx* ctx, double* ms_out, int64_t* launches_out);
+
 /* Test hook: C[M,N] (fp32, row-major, pitch N) = A * B with the production tcgen05 kernel.
  * layout 0: A [M,K] K-major, B [N,K] K-major;  1: A [M,K] K-major, B [K,N] MN-major;
  * 2: A [K,M] MN-major, B [K,N] MN-major.  accumulate != 0: C += (atomic).  bf16 inputs.

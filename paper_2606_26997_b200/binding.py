@@ -21,8 +21,10 @@ EXPORTS = [
     "grpo_default_config", "grpo_create", "grpo_destroy", "grpo_last_error", "grpo_workspace_bytes",
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
-    "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm",
+    "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
+    "grpo_profile_enable", "grpo_profile_read_sync",
 ]
+KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug"]
 
 
 class GrpoError(RuntimeError):
@@ -81,6 +83,9 @@ def load_library() -> C.CDLL:
     lib.grpo_check_errors_sync.argtypes = [vp, C.POINTER(i32)]
     lib.grpo_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i64, vp, vp, f64, vp, vp, vp, vp]
     lib.grpo_debug_gemm.argtypes = [vp, i32, vp, vp, vp, i32, i32, i32, i32, vp]
+    lib.grpo_kernel_launches.argtypes = [vp, C.POINTER(i64)]
+    lib.grpo_profile_enable.argtypes = [vp, i32]
+    lib.grpo_profile_read_sync.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
     _LIB = lib
     return lib
 
@@ -303,6 +308,21 @@ class GrpoContext:
             _dev(dW_accum, torch.float32, "dW_accum"), float(loss_denom), _host(loss_h, torch.float32, "loss_h"),
             _host(logp_h, torch.float32, "logp_h"), dh_ptr, _stream(stream)))
         return loss_h
+
+    # ------------------------------------------------------------------ accounting / profiling
+    def grpo_kernel_launches(self) -> dict:
+        arr = (C.c_int64 * len(KERNEL_KINDS))()
+        _check(self.lib.grpo_kernel_launches(self.h, arr))
+        return {k: arr[i] for i, k in enumerate(KERNEL_KINDS)}
+
+    def grpo_profile_enable(self, on: bool = True):
+        _check(self.lib.grpo_profile_enable(self.h, int(on)))
+
+    def grpo_profile_read_sync(self) -> dict:
+        ms = (C.c_double * len(KERNEL_KINDS))()
+        n = (C.c_int64 * len(KERNEL_KINDS))()
+        _check(self.lib.grpo_profile_read_sync(self.h, ms, n))
+        return {k: dict(ms=ms[i], launches=n[i]) for i, k in enumerate(KERNEL_KINDS)}
 
     # ------------------------------------------------------------------ test hook
     def grpo_debug_gemm(self, layout: int, A, B, M: int, N: int, K: int, C_out=None, accumulate: bool = False,

@@ -81,8 +81,35 @@ struct grpo_ctx {
   std::deque<PendingGroup> fifo;
   int64_t launches = 0;
   int32_t consumed = 0;
+  // kernel accounting (always) and per-launch CUDA-event timing (only while profiling is on)
+  int64_t kernel_count[GRPO_NUM_KERNEL_KINDS] = {0};
+  bool profiling = false;
+  struct ProfRec { int kind; cudaEvent_t beg, end; };
+  std::vector<ProfRec> prof;
+};
+
+// Brackets one kernel launch: counts it and, while profiling, records events on the launch stream.
+struct LaunchScope {
+  grpo_ctx* ctx; cudaStream_t st; cudaEvent_t end = nullptr;
+  LaunchScope(grpo_ctx* c, int kind, cudaStream_t s) : ctx(c), st(s) {
+    ctx->kernel_count[kind]++;
+    if (ctx->profiling) {
+      grpo_ctx::ProfRec r{kind, nullptr, nullptr};
+      if (cudaEventCreate(&r.beg) == cudaSuccess && cudaEventCreate(&r.end) == cudaSuccess) {
+        cudaEventRecord(r.beg, st);
+        end = r.end;
+        ctx->prof.push_back(r);
+      }
+    }
+  }
+  ~LaunchScope() { if (end) cudaEventRecord(end, st); }
 };
 static const int kDenomRing = 64;
+static void prof_clear(grpo_ctx* ctx) {
+  for (auto& r : ctx->prof) { cudaEventDestroy(r.beg); cudaEventDestroy(r.end); }
+  ctx->prof.clear();
+}
+
 
 static int64_t chunk_tokens(const grpo_config& c) { return c.bwd_chunk_tokens > 0 ? c.bwd_chunk_tokens : 9472; }
 
@@ -154,7 +181,7 @@ static void set_desc_defaults(GemmParams& p, bool a_mn, bool b_mn) {
 }
 
 template <bool A_MN, bool B_MN, int EPI>
-static int32_t launch_gemm(const grpo_ctx* ctx, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
+static int32_t launch_gemm(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
                            int n_units, cudaStream_t st) {
   static bool attr_set = false;
   auto kern = grpo_gemm_kernel<A_MN, B_MN, EPI>;
@@ -164,7 +191,10 @@ static int32_t launch_gemm(const grpo_ctx* ctx, const CUtensorMap& tmA, const CU
   }
   if (n_units <= 0) return GRPO_OK;
   const int grid = std::min(n_units, ctx->num_sms);
-  kern<<<grid, kGemmThreads, kSmemBytes, st>>>(tmA, tmB, p, n_units);
+  {
+    LaunchScope ls(ctx, kind, st);
+    kern<<<grid, kGemmThreads, kSmemBytes, st>>>(tmA, tmB, p, n_units);
+  }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
 }
@@ -241,6 +271,7 @@ extern "C" int32_t grpo_destroy(grpo_ctx* ctx) {
   if (!ctx) return GRPO_OK;
   cudaFree(ctx->err_dev);
   cudaFree(ctx->denom_ring);
+  prof_clear(ctx);
   if (ctx->denom_event) cudaEventDestroy(ctx->denom_event);
   delete ctx;
   return GRPO_OK;
@@ -274,6 +305,34 @@ extern "C" int32_t grpo_check_errors_sync(grpo_ctx* ctx, int32_t* flags_out) {
   return GRPO_OK;
 }
 
+// ------------------------------------------------------------------------------------- accounting / profiling
+extern "C" int32_t grpo_kernel_launches(const grpo_ctx* ctx, int64_t* counts_out) {
+  if (!ctx || !counts_out) return fail(GRPO_ERR_INVALID_ARG, "ctx/counts_out is NULL");
+  for (int i = 0; i < GRPO_NUM_KERNEL_KINDS; ++i) counts_out[i] = ctx->kernel_count[i];
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_profile_enable(grpo_ctx* ctx, int32_t on) {
+  if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL");
+  ctx->profiling = on != 0;
+  if (!on) prof_clear(ctx);
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_profile_read_sync(grpo_ctx* ctx, double* ms_out, int64_t* launches_out) {
+  if (!ctx || !ms_out || !launches_out) return fail(GRPO_ERR_INVALID_ARG, "NULL pointer");
+  CU_OK(cudaDeviceSynchronize());
+  for (int i = 0; i < GRPO_NUM_KERNEL_KINDS; ++i) { ms_out[i] = 0.0; launches_out[i] = 0; }
+  for (auto& r : ctx->prof) {
+    float ms = 0.f;
+    CU_OK(cudaEventElapsedTime(&ms, r.beg, r.end));
+    ms_out[r.kind] += ms;
+    launches_out[r.kind]++;
+  }
+  prof_clear(ctx);
+  return GRPO_OK;
+}
+
 // ------------------------------------------------------------------------------------- A1
 extern "C" int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, const int32_t* cu_groups,
                                         int32_t n_groups, int32_t G, float* adv_out, uint8_t* zero_var_out,
@@ -283,8 +342,11 @@ extern "C" int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, con
   if (n_groups == 0) return GRPO_OK;
   const int threads = 128;
   const int blocks = (n_groups * 32 + threads - 1) / threads;
-  group_advantage_kernel<<<blocks, threads, 0, static_cast<cudaStream_t>(stream)>>>(
-      rewards, cu_groups, n_groups, G, ctx->cfg.eps_std, ctx->cfg.std_ddof, adv_out, zero_var_out);
+  {
+    LaunchScope ls(ctx, GRPO_KERNEL_ADVANTAGE, static_cast<cudaStream_t>(stream));
+    group_advantage_kernel<<<blocks, threads, 0, static_cast<cudaStream_t>(stream)>>>(
+        rewards, cu_groups, n_groups, G, ctx->cfg.eps_std, ctx->cfg.std_ddof, adv_out, zero_var_out);
+  }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
 }
@@ -312,7 +374,10 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     CU_OK(cudaMemsetAsync(total, 0, 4, st));
     const int threads = 128;
     const int blocks = (S * 32 + threads - 1) / threads;
-    token_count_kernel<<<blocks, threads, 0, st>>>(mask, targets, c.V, cu_seqlens, S, seq_count, total);
+    {
+      LaunchScope ls(ctx, GRPO_KERNEL_TOKEN_COUNT, st);
+      token_count_kernel<<<blocks, threads, 0, st>>>(mask, targets, c.V, cu_seqlens, S, seq_count, total);
+    }
     CU_OK(cudaGetLastError());
   }
 
@@ -336,7 +401,7 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   p.part_s = part_s;
   p.part_stride = T;
   p.zy = zy;
-  GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, tmH, tmW, p, p.m_tiles * p.n_split, st)));
+  GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
 
   LossParams lp;
   std::memset(&lp, 0, sizeof(lp));
@@ -350,7 +415,10 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   lp.metrics_accum = metrics_accum; lp.err_flag = ctx->err_dev;
   const int threads = 256;
   const int blocks = static_cast<int>((T + threads - 1) / threads);
-  loss_epilogue_kernel<<<blocks, threads, 0, st>>>(lp);
+  {
+    LaunchScope ls(ctx, GRPO_KERNEL_LOSS, st);
+    loss_epilogue_kernel<<<blocks, threads, 0, st>>>(lp);
+  }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
 }
@@ -409,7 +477,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.scale_log2e = c.logit_scale * kLog2e; p.logit_scale = c.logit_scale;
       p.lse = lse; p.coeff = coeff; p.coeff_mul = c.logit_scale * grad_scale;
       p.dz = dz; p.dz_pitch = L.v_pad;
-      GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
+      GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, GRPO_KERNEL_GEMM_DZ, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
     }
     if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d]
       GemmParams p;
@@ -419,7 +487,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
       p.n_fastest = 1;
       p.c_out = static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem; p.c_pitch = c.d; p.c_fp32 = c.dhidden_fp32;
-      GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
+      GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
     }
     if (dW_accum) {  // A6: dW[V, d] += dZ^T[V, rows] H[rows, d]
       GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
@@ -432,7 +500,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
       p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1;
-      GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st)));
+      GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_GEMM_DW, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st)));
     }
   }
   return GRPO_OK;
@@ -574,7 +642,10 @@ static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, cons
       if (any_ref) CU_OK(cudaMemcpyAsync(sr + off, g.ref_logp, n * 4, cudaMemcpyDeviceToDevice, st));
       if (any_mask) {
         if (g.mask) CU_OK(cudaMemcpyAsync(sm + off, g.mask, n, cudaMemcpyDeviceToDevice, st));
-        else { fill_u8_kernel<<<64, 256, 0, st>>>(sm + off, n, 1); CU_OK(cudaGetLastError()); }
+        else {
+          { LaunchScope ls(ctx, GRPO_KERNEL_TOKEN_COUNT, st); fill_u8_kernel<<<64, 256, 0, st>>>(sm + off, n, 1); }
+          CU_OK(cudaGetLastError());
+        }
       }
       off += n;
     }
@@ -630,7 +701,10 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
     cudaStream_t s0 = static_cast<cudaStream_t>(streams ? streams[ctx->launches % n_streams] : nullptr);
     CU_OK(cudaMemsetAsync(dd, 0, 4, s0));
     for (const auto& g : upd) {
-      token_count_flat_kernel<<<64, 256, 0, s0>>>(g.desc.mask, g.desc.targets, ctx->cfg.V, g.tokens, dd);
+      {
+        LaunchScope ls(ctx, GRPO_KERNEL_TOKEN_COUNT, s0);
+        token_count_flat_kernel<<<64, 256, 0, s0>>>(g.desc.mask, g.desc.targets, ctx->cfg.V, g.tokens, dd);
+      }
       CU_OK(cudaGetLastError());
     }
     CU_OK(cudaEventRecord(ctx->denom_event, s0));
@@ -758,14 +832,14 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   if (!b_mn) GRPO_TRY(make_tmap(ctx, &tmB, B, K, N, static_cast<uint64_t>(K) * 2, BK, BN));
   else GRPO_TRY(make_tmap(ctx, &tmB, B, N, K, static_cast<uint64_t>(N) * 2, 64, BK));
   if (layout == 0) {
-    if (accumulate) return launch_gemm<false, false, EPI_RED_F32>(ctx, tmA, tmB, p, units, st);
-    return launch_gemm<false, false, EPI_STORE>(ctx, tmA, tmB, p, units, st);
+    if (accumulate) return launch_gemm<false, false, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
+    return launch_gemm<false, false, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   } else if (layout == 1) {
-    if (accumulate) return launch_gemm<false, true, EPI_RED_F32>(ctx, tmA, tmB, p, units, st);
-    return launch_gemm<false, true, EPI_STORE>(ctx, tmA, tmB, p, units, st);
+    if (accumulate) return launch_gemm<false, true, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
+    return launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   } else if (layout == 2) {
-    if (accumulate) return launch_gemm<true, true, EPI_RED_F32>(ctx, tmA, tmB, p, units, st);
-    return launch_gemm<true, true, EPI_STORE>(ctx, tmA, tmB, p, units, st);
+    if (accumulate) return launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
+    return launch_gemm<true, true, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   }
   return fail(GRPO_ERR_INVALID_ARG, "layout must be 0, 1 or 2");
 }

@@ -72,17 +72,18 @@ def gates(b, out, ref, check_grads=True, logit_scale=1.0):
         non_target[y[(y >= 0) & (y < b.V)]] = False
         if non_target.any() and np.linalg.norm(ref["dW"][non_target]) > 0:
             e["dW_nontarget_rel"] = rel_l2(dW[non_target], ref["dW"][non_target])
-        # (ii) dH minus the one-hot part  c_t s W[y_t]: the sum_v p_tv W[v] part alone.  The bf16 rounding of
-        # the one-hot dZ entry (rel 2^-9 of the ONE-HOT part) bounds how well this can be resolved, so the
-        # error is reported relative to ||dense|| + 2.5e-3 ||onehot||; only meaningful for fp32 dH output.
+        # (ii) dH minus the one-hot part  c_t s W[y_t]: the sum_v p_tv W[v] part alone.  The one-hot dZ entry
+        # c_t (1 - p_ty) is rounded to bf16 before the dH contraction (rel err <= 2^-9, rms 2^-9/sqrt(3) = 1.1e-3
+        # of the ONE-HOT part), which bounds how well the dense part can be resolved from dH.  Gate:
+        # ||err|| <= 1e-2 ||dense|| + 2.5e-3 ||onehot||, reported as the ratio; fp32 dH output only.
         if out["dH"].dtype == torch.float32:
             W64 = b.W.double().cpu().numpy()
             yy = np.clip(y, 0, b.V - 1)
             onehot = (ref["coeff"] * ((y >= 0) & (y < b.V)))[:, None] * W64[yy] * logit_scale
             dense_ref = ref["dH"] - onehot
             if np.linalg.norm(dense_ref) > 0:
-                e["dH_dense_rel"] = float(np.linalg.norm((dH - onehot) - dense_ref) /
-                                          (np.linalg.norm(dense_ref) + 2.5e-3 * np.linalg.norm(onehot)))
+                e["dH_dense_ratio"] = float(np.linalg.norm((dH - onehot) - dense_ref) /
+                                            (1e-2 * np.linalg.norm(dense_ref) + 2.5e-3 * np.linalg.norm(onehot)))
         # (iii) rows of dZ sum to zero => sum_v dW[v,:] = 0 (P7); scale: bf16 rounding of dZ entries
         e["dW_colsum_rel"] = float(np.linalg.norm(dW.sum(0)) / max(np.linalg.norm(dW), 1e-300))
     return e
@@ -98,5 +99,5 @@ def assert_gates(e, check_grads=True):
         assert e["dW_rel"] <= TOL_GRAD_REL, e
         if "dW_nontarget_rel" in e:
             assert e["dW_nontarget_rel"] <= TOL_GRAD_REL, e
-        if "dH_dense_rel" in e:
-            assert e["dH_dense_rel"] <= 1e-2, e
+        if "dH_dense_ratio" in e:
+            assert e["dH_dense_ratio"] <= 1.0, e

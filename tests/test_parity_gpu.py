@@ -47,7 +47,7 @@ def test_config1b_clip_regions_populated():
     b = make_config(1, device="cuda", variant="1b")
     out, ref, e = _check(b)
     frac = (ref["u"] == 0).mean()
-    assert 0.1 < frac < 0.9
+    assert 0.03 < frac < 0.9          # zero-advantage groups and |log rho| < log 1.28 tokens are never clipped
     assert to64(out["metrics"])[3] == ref["metrics"][3]          # same tokens clipped
 
 
