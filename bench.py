@@ -30,7 +30,11 @@ if ROOT not in sys.path:
 
 METRIC = "GRPO loss fwd+bwd tokens/sec at d=2048,V=151936; % of B200 BF16 tensor peak"
 UNIT = "tokens/s"
-SAMPLE_LEN_DIV = 32.0          # oracle sample: configs[1] with response lengths / 32 (T ~ 570), full d and V
+# Oracle samples: configs[1] with response lengths / div at full d and V.  The cpu_baseline leg times ONE
+# oracle step (~10-20 s of CPU work); the --impl reference arm times steps+warmup of them, so its sample is
+# smaller (~3 s per step) to keep the whole run within a few minutes.
+SAMPLE_LEN_DIV = 8.0           # cpu_baseline leg: T ~ 2.3k tokens
+REF_SAMPLE_LEN_DIV = 32.0      # --impl reference arm: T ~ 580 tokens per step
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
@@ -108,10 +112,10 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------- oracle legs
-def oracle_sample(device="cpu"):
-    """Bounded sample of the timed workload for the CPU oracle: configs[1] with lengths / SAMPLE_LEN_DIV."""
+def oracle_sample(device="cpu", len_div=SAMPLE_LEN_DIV):
+    """Bounded sample of the timed workload for the CPU oracle: configs[1] with lengths / len_div."""
     from workloads.synth import make_config
-    b = make_config(2, seed=0, device=device, len_div=SAMPLE_LEN_DIV)
+    b = make_config(2, seed=0, device=device, len_div=len_div)
     return b.to("cpu") if device != "cpu" else b
 
 
@@ -139,8 +143,8 @@ def oracle_threads():
     return os.cpu_count() or 1
 
 
-def sample_desc(b):
-    return (f"configs[1] with response lengths/{SAMPLE_LEN_DIV:g}: 1 group x G={b.G}, T={b.T} tokens, d={b.d}, "
+def sample_desc(b, len_div=SAMPLE_LEN_DIV):
+    return (f"configs[1] with response lengths/{len_div:g}: 1 group x G={b.G}, T={b.T} tokens, d={b.d}, "
             f"V={b.V}; one oracle fwd+bwd (float64, numpy/OpenBLAS) per step")
 
 
@@ -148,7 +152,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    b = oracle_sample("cpu")
+    b = oracle_sample("cpu", REF_SAMPLE_LEN_DIV)
     for _ in range(args.warmup):
         time_oracle_step(b)
     times = [time_oracle_step(b) for _ in range(args.steps)]
@@ -161,7 +165,8 @@ def run_reference(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "configs[1]: one complete group G=8, lengths U[512,4096], d=2048, V=151936 "
                                "(bounded sample, see cpu_baseline.sample)", "tokens_per_step": b.T},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_desc(b)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample_desc(b, REF_SAMPLE_LEN_DIV)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -170,6 +175,26 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------- CUDA arm
+def rank_seed(rank: int) -> int:
+    """Rank r times its own complete group (weak scaling over independent groups)."""
+    return int(rank)
+
+
+def reduce_over_ranks(ms_total: float, e2e_s: float, tokens: int, world: int, device):
+    """Whole-job figures: the timed regions' MAX over ranks and the SUM of the tokens all ranks processed.
+    The only torch.distributed traffic of the benchmark besides the barriers (the path has no collective)."""
+    if world <= 1:
+        return float(ms_total), float(e2e_s), float(tokens)
+    import torch
+    import torch.distributed as dist
+    stats = torch.tensor([ms_total, e2e_s], dtype=torch.float64, device=device)
+    toks = torch.tensor([float(tokens)], dtype=torch.float64, device=device)
+    dist.all_reduce(stats, op=dist.ReduceOp.MAX)
+    dist.all_reduce(toks, op=dist.ReduceOp.SUM)
+    ms, e2e = stats.tolist()
+    return ms, e2e, toks.item()
+
+
 GEMM_KINDS = ("gemm_lse", "gemm_dz", "gemm_dh", "gemm_dw")
 
 
@@ -201,7 +226,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
-    b = make_config(2, seed=rank, device=dev)
+    b = make_config(2, seed=rank_seed(rank), device=dev)
     T, d, V = b.T, b.d, b.V
     ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi)
     dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
@@ -268,13 +293,7 @@ def run_ours(args):
     d2h = sum(t.numel() * t.element_size() for t in (h_logp, h_dh, h_loss))
 
     # ---- reduce over ranks: max time, sum tokens
-    stats = torch.tensor([ms_total, e2e_s], dtype=torch.float64, device=dev)
-    toks = torch.tensor([float(T)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
-        dist.all_reduce(toks, op=dist.ReduceOp.SUM)
-    ms_total, e2e_s = stats.tolist()
-    tokens_all = toks.item()
+    ms_total, e2e_s, tokens_all = reduce_over_ranks(ms_total, e2e_s, T, world, dev)
     value = tokens_all * args.steps / (ms_total * 1e-3)
     e2e_value = tokens_all * args.steps / e2e_s
 

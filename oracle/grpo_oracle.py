@@ -32,6 +32,7 @@ import numpy as np
 __all__ = [
     "OracleConfig", "bf16_bits_to_f64", "group_advantage", "token_advantage",
     "token_logprobs", "loss_terms", "backward", "grpo_step", "grpo_step_loops",
+    "token_rows", "dH_rows", "dW_rows",
 ]
 
 
@@ -202,6 +203,58 @@ def backward(H, W, y, lse, coeff, logit_scale=1.0, chunk_tokens=1024, grad_scale
         dH[t0:t1] = logit_scale * (dz @ W)
         dW += logit_scale * (dz.T @ H[t0:t1])
     return dH, dW
+
+
+# ------------------------------------------------------- single outputs, one by one
+# For inputs too large to run the whole step in float64 (T x V x d at the Qwen3 shape), the same
+# definitions evaluated for a SAMPLE of outputs: a token's (lse, logp), a row of dH, a row of dW.
+# Each is the formula of steps 3, 4 and 9 written for one index; nothing is shared with `backward`
+# beyond numpy (tests/test_oracle_pins.py checks they reproduce its rows).
+def token_rows(H, W, y, rows, logit_scale=1.0):
+    """(lse_t, logp_t) for t in ``rows``: the full logit row z_t = s W h_t is materialised."""
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    V = W.shape[0]
+    lse = np.zeros(len(rows))
+    logp = np.zeros(len(rows))
+    for i, t in enumerate(rows):
+        z = logit_scale * (W @ H[t])
+        m = z.max()
+        lse[i] = m + np.log(np.exp(z - m).sum())
+        yt = int(y[t])
+        logp[i] = z[yt] - lse[i] if 0 <= yt < V else 0.0
+    return lse, logp
+
+
+def dH_rows(H, W, y, lse_rows, coeff_rows, rows, logit_scale=1.0):
+    """dH[t,:] = s sum_v c_t (1[v = y_t] - p_tv) W[v,:] for t in ``rows`` (lse/coeff given for those t)."""
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    V = W.shape[0]
+    out = np.zeros((len(rows), H.shape[1]))
+    for i, t in enumerate(rows):
+        z = logit_scale * (W @ H[t])
+        dz = -np.exp(z - lse_rows[i])
+        yt = int(y[t])
+        if 0 <= yt < V:
+            dz[yt] += 1.0
+        out[i] = logit_scale * coeff_rows[i] * (dz @ W)
+    return out
+
+
+def dW_rows(H, W, y, lse, coeff, vocab_ids, logit_scale=1.0):
+    """dW[v,:] = s sum_t c_t (1[v = y_t] - p_tv) H[t,:] for v in ``vocab_ids`` (lse/coeff for ALL t)."""
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    y = np.asarray(y, dtype=np.int64)
+    lse = np.asarray(lse, dtype=np.float64)
+    c = np.asarray(coeff, dtype=np.float64)
+    out = np.zeros((len(vocab_ids), H.shape[1]))
+    for i, v in enumerate(vocab_ids):
+        z = logit_scale * (H @ W[v])                      # column v of the logits, all tokens
+        dz = c * ((y == v).astype(np.float64) - np.exp(z - lse))
+        out[i] = logit_scale * (dz @ H)
+    return out
 
 
 # ------------------------------------------------------------------------ whole step

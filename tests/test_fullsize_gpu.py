@@ -1,0 +1,186 @@
+"""Parity at BASELINE.json's FULL sizes (d=2048, V=151936), in the launch configuration bench.py times.
+
+The float64 oracle cannot run the whole step at these sizes in test time (SURVEY.md §7 hard part 7), so:
+  * configs[1] (the bench workload, T ~ 18.7k): the oracle's full forward (lse, logp of EVERY token, loss,
+    coeff) is affordable (~1 min on the host cores); dH and dW are compared on sampled rows the oracle computes
+    one by one (oracle.dH_rows / dW_rows), plus the size-independent property sum_v dW[v,:] = 0 (P7).
+  * configs[2], [3], [4] (64k .. 500k tokens): sampled tokens (lse, logp, coeff, dH rows) against the oracle,
+    with the full-batch denominator so every sampled term is exactly the full-batch term; dW through
+    properties that hold at any size (P7; exact zeros; additivity of streamed vs batched launches, P12).
+No oracle input or expected value comes from the CUDA path."""
+import numpy as np
+import pytest
+import torch
+
+from oracle.grpo_oracle import (OracleConfig, dH_rows, dW_rows, group_advantage, loss_terms, token_advantage,
+                                token_logprobs, token_rows)
+from tests.parity_util import TOL_GRAD_REL, TOL_LOGP_ABS, TOL_LOSS_REL, make_ctx, rel_l2, run_cuda, to64
+from workloads.synth import make_config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_2606_26997_b200.build import build
+    build()
+
+
+def _ocfg(b):
+    return OracleConfig(eps_std=b.eps_std, clip_lo=b.clip_lo, clip_hi=b.clip_hi, kl_beta=b.kl_beta,
+                        loss_agg=b.loss_agg)
+
+
+def _sample_tokens(b, n, seed):
+    rng = np.random.default_rng(seed)
+    rows = set(rng.choice(b.T, size=min(n, b.T), replace=False).tolist())
+    cu = b.cu_seqlens.cpu().numpy()
+    rows |= {0, b.T - 1, int(cu[1]) - 1, int(cu[1])}                  # stream ends and a sequence boundary
+    rows |= {t for t in (127, 128, b.T - b.T % 128 - 1, b.T - b.T % 128) if 0 <= t < b.T}   # tile edges, ragged tail
+    return np.array(sorted(rows))
+
+
+def _oracle_sampled(b, rows, denom):
+    """Oracle (lse, logp, coeff, dH) of the sampled tokens; every term is the full-batch term."""
+    Hs = b.hidden[torch.from_numpy(rows).to(b.hidden.device)].double().cpu().numpy()
+    W64 = b.W.double().cpu().numpy()
+    y = b.targets.cpu().numpy().astype(np.int64)[rows]
+    idx = np.arange(len(rows))
+    lse, logp = token_rows(Hs, W64, y, idx)
+    adv, _ = group_advantage(b.rewards.double().cpu().numpy(), G=b.G, eps_std=b.eps_std)
+    A_tok = token_advantage(adv, b.cu_seqlens.cpu().numpy())[rows]
+    pick = lambda t: None if t is None else t.double().cpu().numpy()[rows]
+    lt = loss_terms(logp, pick(b.old_logp), pick(b.ref_logp), None if b.mask is None else b.mask.cpu().numpy()[rows],
+                    A_tok, np.array([0, len(rows)]), _ocfg(b), loss_denom=denom, valid=(y >= 0) & (y < b.V))
+    dH = dH_rows(Hs, W64, y, lse, lt["coeff"], idx)
+    return dict(lse=lse, logp=logp, coeff=lt["coeff"], dH=dH, adv=adv)
+
+
+def _check_sampled(b, out, rows, ref):
+    r = torch.from_numpy(rows).to(b.hidden.device)
+    assert np.abs(to64(out["adv"]) - ref["adv"]).max() <= 1e-5
+    assert np.abs(to64(out["logp"][r]) - ref["logp"]).max() <= TOL_LOGP_ABS
+    assert np.abs(to64(out["lse"][r]) - ref["lse"]).max() <= TOL_LOGP_ABS
+    assert rel_l2(to64(out["coeff"][r]), ref["coeff"]) <= 1e-3
+    dH = to64(out["dH"][r])
+    assert rel_l2(dH, ref["dH"]) <= TOL_GRAD_REL
+    worst = max(rel_l2(dH[i], ref["dH"][i]) for i in range(len(rows)) if np.linalg.norm(ref["dH"][i]) > 0)
+    assert worst <= 2 * TOL_GRAD_REL, worst                           # no single row is off either
+
+
+def _colsum_rel(dW):
+    return float(dW.sum(0, dtype=torch.float64).norm() / dW.double().norm().clamp_min(1e-300))
+
+
+# ------------------------------------------------------------------ configs[1]: the workload bench.py times
+def test_config2_full_size_bench_workload():
+    b = make_config(2, seed=0, device="cuda")
+    assert (b.d, b.V, b.G, b.n_groups) == (2048, 151936, 8, 1) and 4096 <= b.T <= 32768
+    ctx = make_ctx(b, max_tokens=b.T)                                  # defaults = bench.py's launch configuration
+    out = run_cuda(ctx, b)
+    assert ctx.grpo_check_errors_sync() == 0
+    ctx.close()
+    x = b.numpy_f64()
+    # full forward in float64: every token's lse / logp, the loss and the backward coefficients
+    lse, logp = token_logprobs(x["H"], x["W"], x["y"])
+    adv, _ = group_advantage(x["rewards"], G=b.G, eps_std=b.eps_std)
+    lt = loss_terms(logp, x["old_logp"], None, None, token_advantage(adv, x["cu_seqlens"]), x["cu_seqlens"], _ocfg(b))
+    assert np.abs(to64(out["logp"]) - logp).max() <= TOL_LOGP_ABS
+    assert np.abs(to64(out["lse"]) - lse).max() <= TOL_LOGP_ABS
+    assert abs(out["loss"].item() - lt["loss"]) <= TOL_LOSS_REL * max(abs(lt["loss"]), lt["abs_loss"])
+    assert rel_l2(to64(out["coeff"]), lt["coeff"]) <= 1e-3
+    # on-policy: rho = 1 +- 1e-5 (R15), nothing clipped
+    assert abs(to64(out["metrics"])[1] / b.T - 1.0) < 1e-4 and to64(out["metrics"])[3] == 0
+    # sampled dH rows
+    rows = _sample_tokens(b, 48, seed=1)
+    dH_ref = dH_rows(x["H"], x["W"], x["y"], lse[rows], lt["coeff"][rows], rows)
+    dH = to64(out["dH"][torch.from_numpy(rows).cuda()])
+    assert rel_l2(dH, dH_ref) <= TOL_GRAD_REL
+    # sampled dW rows: target ids (one-hot + dense part), ids that are never a target (dense part alone),
+    # the first / last vocab rows and the rows around the last 256-wide vocab tile (151936 = 593.5 x 256)
+    rng = np.random.default_rng(2)
+    tgt = np.unique(x["y"])
+    non = np.setdiff1d(np.arange(b.V), tgt)
+    vids = np.unique(np.concatenate([rng.choice(tgt, 24, replace=False), rng.choice(non, 24, replace=False),
+                                     [0, 1, 255, 256, 151807, 151808, b.V - 2, b.V - 1]]))
+    dW_ref = dW_rows(x["H"], x["W"], x["y"], lse, lt["coeff"], vids)
+    dW = to64(out["dW"][torch.from_numpy(vids).cuda()])
+    is_t = np.isin(vids, tgt)
+    assert rel_l2(dW[is_t], dW_ref[is_t]) <= TOL_GRAD_REL
+    assert rel_l2(dW[~is_t], dW_ref[~is_t]) <= TOL_GRAD_REL            # dense softmax term on its own
+    assert _colsum_rel(out["dW"]) <= 2e-3                              # P7 on the whole [V, d] gradient
+    assert torch.isfinite(out["dW"]).all() and torch.isfinite(out["dH"].float()).all()
+
+
+# ------------------------------------------------------------------ configs[2]: 4 x G=8, KL, zero-variance groups
+def test_config3_full_size_sampled():
+    b = make_config(3, seed=0, device="cuda")
+    assert b.zero_var_frac > 0 and b.kl_beta > 0
+    ctx = make_ctx(b, max_tokens=b.T)
+    out = run_cuda(ctx, b)
+    assert ctx.grpo_check_errors_sync() == 0
+    ctx.close()
+    rows = _sample_tokens(b, 40, seed=3)
+    _check_sampled(b, out, rows, _oracle_sampled(b, rows, float(b.T)))
+    assert _colsum_rel(out["dW"]) <= 2e-3
+    assert to64(out["metrics"])[0] == b.T
+
+
+# ------------------------------------------------------------------ configs[3]: 8 x G=16 long tail, ~0.5M tokens
+def test_config4_full_size_sampled_and_zero_rows():
+    b = make_config(4, seed=0, device="cuda")
+    assert b.T > 300_000 and b.kl_beta == 0.0
+    ctx = make_ctx(b, max_tokens=b.T)
+    out = run_cuda(ctx, b)
+    assert ctx.grpo_check_errors_sync() == 0
+    ctx.close()
+    rows = _sample_tokens(b, 40, seed=4)
+    _check_sampled(b, out, rows, _oracle_sampled(b, rows, float(b.T)))
+    assert _colsum_rel(out["dW"]) <= 2e-3
+    # beta = 0: tokens of zero-variance groups have exactly zero gradient rows (R4)
+    r = b.rewards.view(b.n_groups, b.G)
+    for g in torch.nonzero(r.max(1).values == r.min(1).values).flatten().tolist():
+        t0, t1 = b.group_token_range(g)
+        assert torch.all(out["dH"][t0:t1] == 0)
+
+
+# ------------------------------------------------------------------ configs[4]: streaming CGP arrival, 32 groups
+def test_config5_full_size_streamed_equals_batched():
+    b = make_config(5, seed=0, device="cuda")
+    assert b.n_groups == 32 and b.T > 300_000
+    rows = _sample_tokens(b, 32, seed=5)
+    ref = _oracle_sampled(b, rows, float(b.T))
+    results = []
+    gtok = [int(b.seqlens[g * b.G:(g + 1) * b.G].sum()) for g in b.arrival_order]
+    for U, n_streams in ((1, 1), (4, 2)):                              # per-group launches; 4-group batches, 2 streams
+        max_T = max(sum(gtok[i:i + U]) for i in range(0, b.n_groups, U))
+        ctx = make_ctx(b, groups_per_update=U, groups_per_round=b.n_groups, max_tokens=max_T, n_slots=n_streams)
+        streams = [torch.cuda.Stream() for _ in range(n_streams)]
+        dW = torch.zeros(b.V, b.d, dtype=torch.float32, device="cuda")
+        loss = torch.zeros(1, dtype=torch.float32, device="cuda")
+        dH = torch.zeros(b.T, b.d, dtype=torch.bfloat16, device="cuda")
+        logp = torch.zeros(b.T, dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        boundaries = 0
+        for g in b.arrival_order:                                      # one complete group at a time, FIFO
+            g = int(g)
+            t0, t1 = b.group_token_range(g)
+            desc = ctx.make_group_desc(g, b.seqlens[g * b.G:(g + 1) * b.G], b.hidden[t0:t1], b.targets[t0:t1],
+                                       b.old_logp[t0:t1], b.rewards[g * b.G:(g + 1) * b.G].contiguous(), None, None,
+                                       dH[t0:t1], logp[t0:t1])
+            _, boundary = ctx.grpo_enqueue_groups([desc], b.W, dW, loss, loss_denom=float(b.T), streams=streams)
+            boundaries += int(boundary)
+        torch.cuda.synchronize()
+        assert ctx.grpo_check_errors_sync() == 0
+        st = ctx.grpo_queue_state()
+        assert st["pending_groups"] == 0 and st["round_complete"] and boundaries == b.n_groups // U
+        ctx.close()
+        r = torch.from_numpy(rows).cuda()
+        assert np.abs(to64(logp[r]) - ref["logp"]).max() <= TOL_LOGP_ABS
+        assert rel_l2(to64(dH[r]), ref["dH"]) <= TOL_GRAD_REL
+        assert _colsum_rel(dW) <= 2e-3
+        results.append((dW, loss, logp))
+    (dW1, loss1, lp1), (dW4, loss4, lp4) = results
+    assert (lp1 - lp4).abs().max().item() <= 2e-5
+    assert float((dW1.double() - dW4.double()).norm() / dW4.double().norm()) <= 5e-4
+    np.testing.assert_allclose(loss1.item(), loss4.item(), rtol=1e-4)

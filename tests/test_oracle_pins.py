@@ -390,3 +390,28 @@ def test_bf16_widening_is_exact():
     x = torch.randn(1000).to(torch.bfloat16)
     bits = x.view(torch.int16).numpy().view(np.uint16)
     np.testing.assert_array_equal(bf16_bits_to_f64(bits), x.to(torch.float64).numpy())
+
+
+def test_single_output_helpers_reproduce_rows_of_the_full_step():
+    """token_rows / dH_rows / dW_rows (used to sample outputs at the full Qwen3 shape) against the pinned
+    whole-step oracle, and against the explicit-loop oracle, on config 1b with masked and ignored tokens."""
+    from oracle.grpo_oracle import dH_rows, dW_rows, token_rows
+    from workloads.synth import make_config
+    b = make_config(1, seed=11, variant="1b", mask_frac=0.2, bad_target_frac=0.1, n_groups=2, G=3, V=300, d=16)
+    x = b.numpy_f64()
+    cfg = OracleConfig(kl_beta=b.kl_beta, logit_scale=0.8)
+    ref = grpo_step(x["H"], x["W"], x["y"], x["cu_seqlens"], x["rewards"], x["old_logp"], x["ref_logp"],
+                    mask=x["mask"], cfg=cfg, G=b.G)
+    loops = grpo_step_loops(x["H"], x["W"], x["y"], x["cu_seqlens"], x["rewards"], x["old_logp"], x["ref_logp"],
+                            mask=x["mask"], cfg=cfg, G=b.G)
+    rows = list(range(0, b.T, 7))
+    lse, logp = token_rows(x["H"], x["W"], x["y"], rows, 0.8)
+    np.testing.assert_allclose(lse, ref["lse"][rows], rtol=0, atol=1e-12)
+    np.testing.assert_allclose(logp, ref["logp"][rows], rtol=0, atol=1e-12)
+    dh = dH_rows(x["H"], x["W"], x["y"], lse, ref["coeff"][rows], rows, 0.8)
+    np.testing.assert_allclose(dh, ref["dH"][rows], rtol=1e-10, atol=1e-15)
+    np.testing.assert_allclose(dh, loops["dH"][rows], rtol=1e-9, atol=1e-14)
+    vids = sorted(set(int(v) for v in x["y"][:20] if v >= 0) | {0, 1, 150, 299})
+    dw = dW_rows(x["H"], x["W"], x["y"], ref["lse"], ref["coeff"], vids, 0.8)
+    np.testing.assert_allclose(dw, ref["dW"][vids], rtol=1e-10, atol=1e-15)
+    np.testing.assert_allclose(dw, loops["dW"][vids], rtol=1e-9, atol=1e-14)
