@@ -228,7 +228,8 @@ def run_ours(args):
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
     b = make_config(2, seed=rank_seed(rank), device=dev)
     T, d, V = b.T, b.d, b.V
-    ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi)
+    ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
+                      gemm_cta_group=args.cta_group)
     dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
     loss = torch.zeros(1, dtype=torch.float32, device=dev)
     dH = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
@@ -369,6 +370,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--cta-group", type=int, default=0, choices=[0, 1, 2],
+                    help="grpo_config.gemm_cta_group: 0 = library default (CTA pairs), 1 = single-CTA tiles")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":

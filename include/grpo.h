@@ -66,6 +66,8 @@ typedef struct {
   int64_t token_budget;      /* feasible-batch token budget per launch; 0 = unlimited */
   int64_t bwd_chunk_tokens;  /* tokens per backward dZ chunk; 0 = default (9472) */
   int32_t max_pending_groups;/* FIFO capacity; 0 = default (4096) */
+  int32_t gemm_cta_group;    /* CTAs cooperating on one tcgen05 MMA: 0 = default (2: CTA pairs, 256x256 pair
+                                tiles), 1 = single-CTA 128x256 tiles (kept as an A/B reference) */
 } grpo_config;
 
 /* Fill *cfg with the defaults above (d, V must still be set). */

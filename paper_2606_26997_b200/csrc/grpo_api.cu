@@ -69,6 +69,7 @@ struct grpo_ctx {
   grpo_config cfg;
   int device = 0;
   int num_sms = 0;
+  int cg = 2;                    // CTAs per MMA: 1 (cta_group::1) or 2 (CTA pairs, cta_group::2)
   EncodeTiledFn encode = nullptr;
   int32_t* err_dev = nullptr;
   float* denom_ring = nullptr;   // device scalars for implicit per-update denominators
@@ -180,23 +181,45 @@ static void set_desc_defaults(GemmParams& p, bool a_mn, bool b_mn) {
   p.lbo_b = b_mn ? 8192 : 16; p.sbo_b = 1024; p.kadv_b = b_mn ? 2048 : 32;
 }
 
-template <bool A_MN, bool B_MN, int EPI>
-static int32_t launch_gemm(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
-                           int n_units, cudaStream_t st) {
+template <int CG, bool A_MN, bool B_MN, int EPI>
+static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB,
+                              const GemmParams& p, int n_units, cudaStream_t st) {
   static bool attr_set = false;
-  auto kern = grpo_gemm_kernel<A_MN, B_MN, EPI>;
+  auto kern = grpo_gemm_kernel<CG, A_MN, B_MN, EPI>;
+  constexpr int smem = GemmShape<CG>::kSmemBytes;
   if (!attr_set) {
-    CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     attr_set = true;
   }
   if (n_units <= 0) return GRPO_OK;
-  const int grid = std::min(n_units, ctx->num_sms);
+  // persistent: one CTA (CG = 1) or one CTA pair (CG = 2, a 2-CTA cluster) per SM / SM pair
+  const int grid = CG * std::min(n_units, ctx->num_sms / CG);
+  cudaLaunchConfig_t lc;
+  std::memset(&lc, 0, sizeof(lc));
+  lc.gridDim = dim3(grid);
+  lc.blockDim = dim3(kGemmThreads);
+  lc.dynamicSmemBytes = smem;
+  lc.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CG;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
   {
     LaunchScope ls(ctx, kind, st);
-    kern<<<grid, kGemmThreads, kSmemBytes, st>>>(tmA, tmB, p, n_units);
+    CU_OK(cudaLaunchKernelEx(&lc, kern, tmA, tmB, p, n_units));
   }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
+}
+
+template <bool A_MN, bool B_MN, int EPI>
+static int32_t launch_gemm(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
+                           int n_units, cudaStream_t st) {
+  if (ctx->cg == 2) return launch_gemm_cg<2, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st);
+  return launch_gemm_cg<1, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st);
 }
 
 static int choose_n_split(int m_tiles, int n_tiles, int sms, int64_t max_split) {
@@ -234,6 +257,8 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
   if (!cfg || !out) return fail(GRPO_ERR_INVALID_ARG, "cfg/out is NULL");
   if (cfg->d <= 0 || cfg->V <= 0 || cfg->d % 8 != 0)
     return fail(GRPO_ERR_SHAPE, "need d > 0, d %% 8 == 0, V > 0 (got d=%d V=%d)", cfg->d, cfg->V);
+  if (cfg->gemm_cta_group < 0 || cfg->gemm_cta_group > 2)
+    return fail(GRPO_ERR_INVALID_ARG, "gemm_cta_group must be 0 (default), 1 or 2");
   if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
     return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
   int dev = 0;
@@ -249,6 +274,7 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
   if (ctx->cfg.max_pending_groups <= 0) ctx->cfg.max_pending_groups = 4096;
   ctx->device = dev;
   ctx->num_sms = prop.multiProcessorCount;
+  ctx->cg = cfg->gemm_cta_group == 1 ? 1 : 2;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -383,16 +409,17 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
 
   CUtensorMap tmH, tmW;
   GRPO_TRY(make_tmap(ctx, &tmH, hidden, c.d, T, static_cast<uint64_t>(c.d) * 2, BK, BM));
-  GRPO_TRY(make_tmap(ctx, &tmW, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN));
+  const int TM = BM * ctx->cg;                      // rows of C per scheduling unit (CTA or CTA pair)
+  GRPO_TRY(make_tmap(ctx, &tmW, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN / ctx->cg));
   GemmParams p;
   std::memset(&p, 0, sizeof(p));
   set_desc_defaults(p, false, false);
   p.m_total = static_cast<int>(T);
   p.n_total = c.V;
-  p.m_tiles = static_cast<int>((T + BM - 1) / BM);
+  p.m_tiles = static_cast<int>((T + TM - 1) / TM);
   p.n_tiles = (c.V + BN - 1) / BN;
   p.k_blocks = (c.d + BK - 1) / BK;
-  p.n_split = choose_n_split(p.m_tiles, p.n_tiles, ctx->num_sms, std::max<int64_t>(1, L.part_cap / T));
+  p.n_split = choose_n_split(p.m_tiles, p.n_tiles, ctx->num_sms / ctx->cg, std::max<int64_t>(1, L.part_cap / T));
   p.tiles_per_split = (p.n_tiles + p.n_split - 1) / p.n_split;
   p.targets = targets;
   p.scale_log2e = c.logit_scale * kLog2e;
@@ -450,18 +477,19 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   const int64_t Tc = L.chunk_rows;
   const int n_chunks = static_cast<int>((T + Tc - 1) / Tc);
   // equalise chunks (whole 128-row tiles) so the last one is not a sliver
-  const int64_t rows_per_chunk = std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, BM));
+  const int64_t rows_per_chunk = std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, BM * ctx->cg));
   const uint8_t* Hb = static_cast<const uint8_t*>(hidden);
   const int dh_elem = c.dhidden_fp32 ? 4 : 2;
 
   CUtensorMap tmW_k, tmW_mn;
-  GRPO_TRY(make_tmap(ctx, &tmW_k, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN));
+  const int TM = BM * ctx->cg;
+  GRPO_TRY(make_tmap(ctx, &tmW_k, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN / ctx->cg));
   GRPO_TRY(make_tmap(ctx, &tmW_mn, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, 64, BK));
 
   for (int64_t t0 = 0; t0 < T; t0 += rows_per_chunk) {
     const int64_t rows = std::min<int64_t>(rows_per_chunk, T - t0);
     const void* Hc = Hb + t0 * c.d * 2;
-    const int m_tiles = static_cast<int>((rows + BM - 1) / BM);
+    const int m_tiles = static_cast<int>((rows + TM - 1) / TM);
     CUtensorMap tmH_k, tmH_mn, tmDZ_k, tmDZ_mn;
     GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
     GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
@@ -496,7 +524,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       std::memset(&p, 0, sizeof(p));
       set_desc_defaults(p, true, true);
       p.m_total = c.V; p.n_total = c.d;
-      p.m_tiles = (c.V + BM - 1) / BM; p.n_tiles = (c.d + BN - 1) / BN;
+      p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
       p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1;
@@ -821,7 +849,8 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   GemmParams p;
   std::memset(&p, 0, sizeof(p));
   p.m_total = M; p.n_total = N;
-  p.m_tiles = (M + BM - 1) / BM; p.n_tiles = (N + BN - 1) / BN; p.k_blocks = (K + BK - 1) / BK;
+  const int TM = BM * ctx->cg;
+  p.m_tiles = (M + TM - 1) / TM; p.n_tiles = (N + BN - 1) / BN; p.k_blocks = (K + BK - 1) / BK;
   p.n_fastest = 1;
   p.c_out = C; p.c_pitch = N; p.c_fp32 = 1;
   const int units = p.m_tiles * p.n_tiles;
@@ -829,7 +858,7 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   set_desc_defaults(p, a_mn, b_mn);
   if (!a_mn) GRPO_TRY(make_tmap(ctx, &tmA, A, K, M, static_cast<uint64_t>(K) * 2, BK, BM));
   else GRPO_TRY(make_tmap(ctx, &tmA, A, M, K, static_cast<uint64_t>(M) * 2, 64, BK));
-  if (!b_mn) GRPO_TRY(make_tmap(ctx, &tmB, B, K, N, static_cast<uint64_t>(K) * 2, BK, BN));
+  if (!b_mn) GRPO_TRY(make_tmap(ctx, &tmB, B, K, N, static_cast<uint64_t>(K) * 2, BK, BN / ctx->cg));
   else GRPO_TRY(make_tmap(ctx, &tmB, B, N, K, static_cast<uint64_t>(N) * 2, 64, BK));
   if (layout == 0) {
     if (accumulate) return launch_gemm<false, false, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);

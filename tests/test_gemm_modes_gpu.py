@@ -6,12 +6,13 @@ import torch
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def ctx():
+@pytest.fixture(scope="module", params=[2, 1], ids=["cta_pair", "single_cta"])
+def ctx(request):
+    """Both tcgen05 variants of the kernel: cta_group::2 pair tiles (the default) and cta_group::1."""
     from paper_2606_26997_b200 import GrpoContext
     from paper_2606_26997_b200.build import build
     build()
-    c = GrpoContext(64, 1000)
+    c = GrpoContext(64, 1000, gemm_cta_group=request.param)
     yield c
     c.close()
 
@@ -25,9 +26,10 @@ def _ref(A, B, layout):
     return A64.T @ B64              # A [K,M], B [K,N]
 
 
-# shapes span several 128x256 tiles, ragged M/N tails, K tails (not a multiple of 64) and tiny K
+# shapes span several 128x256 / 256x256 tiles, ragged M/N tails (including a pair whose second CTA is
+# entirely out of range), K tails (not a multiple of 64), tiny K, and more k blocks than ring stages
 SHAPES = [(128, 256, 64), (256, 512, 128), (200, 264, 72), (1000, 2048, 320), (136, 64, 1000), (8, 8, 8),
-          (384, 1000, 2048)]
+          (384, 1000, 2048), (2048, 136, 4096)]
 
 
 @pytest.mark.parametrize("layout", [0, 1, 2])

@@ -125,6 +125,13 @@ def test_config4_shaped_large_groups():
     _check(b)
 
 
+@pytest.mark.parametrize("cfg_id,kw", [(1, dict(variant="1b")), (3, dict(d=256, V=5000, len_div=20, w_std=0.08))])
+def test_single_cta_variant_parity(cfg_id, kw):
+    """gemm_cta_group = 1 (cta_group::1, 128x256 tiles) stays a supported A/B reference of the default pair kernel."""
+    b = make_config(cfg_id, device="cuda", **kw)
+    _check(b, ctx_kw=dict(gemm_cta_group=1))
+
+
 def test_single_token_and_tiny():
     b = make_config(1, device="cuda", seed=9, n_groups=1, G=2, len_div=100.0)   # every response 1 token
     assert b.T == 2
