@@ -229,7 +229,7 @@ def run_ours(args):
     b = make_config(2, seed=rank_seed(rank), device=dev)
     T, d, V = b.T, b.d, b.V
     ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
-                      gemm_cta_group=args.cta_group)
+                      gemm_cta_group=args.cta_group, **({"bwd_chunk_tokens": args.bwd_chunk} if args.bwd_chunk else {}))
     dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
     loss = torch.zeros(1, dtype=torch.float32, device=dev)
     dH = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
@@ -356,7 +356,7 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
                    "tokens_per_step": int(tokens_all), "tokens_rank0": T, "d": d, "V": V, "G": b.G,
                    "parallelism": f"replicas x{world}: independent complete groups, no collective",
                    "l2": "inputs larger than L2 (W 622 MB, dW 1.2 GB, dZ chunk 2.9 GB vs 126 MB L2); no flush needed",
-                   "bwd_chunk_tokens": 9472},
+                   "bwd_chunk_tokens": args.bwd_chunk or "library default"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "api": "grpo_step_host (C ABI, pinned host buffers; W and dW resident on the device)"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
@@ -372,6 +372,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--cta-group", type=int, default=0, choices=[0, 1, 2],
                     help="grpo_config.gemm_cta_group: 0 = library default (CTA pairs), 1 = single-CTA tiles")
+    ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":

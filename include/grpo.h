@@ -68,6 +68,10 @@ typedef struct {
   int32_t max_pending_groups;/* FIFO capacity; 0 = default (4096) */
   int32_t gemm_cta_group;    /* CTAs cooperating on one tcgen05 MMA: 0 = default (2: CTA pairs, 256x256 pair
                                 tiles), 1 = single-CTA 128x256 tiles (kept as an A/B reference) */
+  int32_t gemm_drift_epoch_kb; /* drift gate of the contraction kernels: the CTA pairs of a launch stay within
+                                one epoch of this many k blocks of each other so that the operand panels they
+                                share are fetched from HBM once.  0 = default (32),
+                                < 0 = off.  Performance only: results do not depend on it. */
 } grpo_config;
 
 /* Fill *cfg with the defaults above (d, V must still be set). */

@@ -38,7 +38,8 @@ class GrpoConfig(C.Structure):
                 ("clip_lo", C.c_float), ("clip_hi", C.c_float), ("kl_beta", C.c_float), ("loss_agg", C.c_int32),
                 ("logit_scale", C.c_float), ("dhidden_fp32", C.c_int32), ("group_size", C.c_int32),
                 ("groups_per_update", C.c_int32), ("groups_per_round", C.c_int32), ("token_budget", C.c_int64),
-                ("bwd_chunk_tokens", C.c_int64), ("max_pending_groups", C.c_int32), ("gemm_cta_group", C.c_int32)]
+                ("bwd_chunk_tokens", C.c_int64), ("max_pending_groups", C.c_int32), ("gemm_cta_group", C.c_int32),
+                ("gemm_drift_epoch_kb", C.c_int32)]
 
 
 class GroupDesc(C.Structure):

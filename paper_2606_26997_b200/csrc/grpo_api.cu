@@ -55,7 +55,7 @@ struct SlotLayout {
   int64_t v_pad = 0;
   int64_t off_part_m = 0, off_part_s = 0, off_zy = 0, off_total = 0, off_seq_count = 0, off_dz = 0;
   int64_t off_hidden = 0, off_targets = 0, off_old = 0, off_ref = 0, off_mask = 0, off_rewards = 0, off_adv = 0,
-          off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0;
+          off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0, off_sync = 0;
   int64_t bytes = 0;
 };
 
@@ -112,6 +112,7 @@ static void prof_clear(grpo_ctx* ctx) {
 }
 
 
+static const int kSyncCap = 1 << 15;   // drift-gate epoch counters per workspace slot
 static int64_t chunk_tokens(const grpo_config& c) { return c.bwd_chunk_tokens > 0 ? c.bwd_chunk_tokens : 9472; }
 
 static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
@@ -145,6 +146,7 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.off_lse = take(max_T * 4);
   L.off_coeff = take(max_T * 4);
   L.off_dh = take(max_T * c.d * (c.dhidden_fp32 ? 4 : 2));
+  L.off_sync = take(kSyncCap * 4);
   L.bytes = off;
   return L;
 }
@@ -194,6 +196,21 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   if (n_units <= 0) return GRPO_OK;
   // persistent: one CTA (CG = 1) or one CTA pair (CG = 2, a 2-CTA cluster) per SM / SM pair
   const int grid = CG * std::min(n_units, ctx->num_sms / CG);
+  GemmParams pl = p;
+  // drift gate (gemm_sm100.cuh): epoch counters live in the launch's workspace slot, zeroed on the stream
+  const int xsync = ctx->cfg.gemm_drift_epoch_kb == 0 ? 32 : ctx->cfg.gemm_drift_epoch_kb;
+  if (pl.sync != nullptr && xsync > 0 && grid / CG > 1) {
+    const int64_t n_pairs = grid / CG;
+    const int64_t kb_unit = static_cast<int64_t>(p.k_blocks) * (EPI == EPI_LSE ? p.tiles_per_split : 1);
+    const int64_t max_kb = (n_units + n_pairs - 1) / n_pairs * kb_unit;
+    int64_t E = xsync;
+    while ((max_kb + E - 1) / E + 1 > kSyncCap) E *= 2;
+    pl.sync_epoch_kb = static_cast<int>(E);
+    pl.sync_epochs = static_cast<int>((max_kb + E - 1) / E + 1);
+    CU_OK(cudaMemsetAsync(pl.sync, 0, static_cast<size_t>(pl.sync_epochs) * 4, st));
+  } else {
+    pl.sync = nullptr;
+  }
   cudaLaunchConfig_t lc;
   std::memset(&lc, 0, sizeof(lc));
   lc.gridDim = dim3(grid);
@@ -209,7 +226,7 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   lc.numAttrs = 1;
   {
     LaunchScope ls(ctx, kind, st);
-    CU_OK(cudaLaunchKernelEx(&lc, kern, tmA, tmB, p, n_units));
+    CU_OK(cudaLaunchKernelEx(&lc, kern, tmA, tmB, pl, n_units));
   }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
@@ -428,6 +445,7 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   p.part_s = part_s;
   p.part_stride = T;
   p.zy = zy;
+  p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
   GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
 
   LossParams lp;
@@ -505,6 +523,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.scale_log2e = c.logit_scale * kLog2e; p.logit_scale = c.logit_scale;
       p.lse = lse; p.coeff = coeff; p.coeff_mul = c.logit_scale * grad_scale;
       p.dz = dz; p.dz_pitch = L.v_pad;
+      p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, GRPO_KERNEL_GEMM_DZ, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
     }
     if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d]
@@ -515,6 +534,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
       p.n_fastest = 1;
       p.c_out = static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem; p.c_pitch = c.d; p.c_fp32 = c.dhidden_fp32;
+      p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
     }
     if (dW_accum) {  // A6: dW[V, d] += dZ^T[V, rows] H[rows, d]
@@ -528,6 +548,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
       p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1;
+      p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_GEMM_DW, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st)));
     }
   }
@@ -853,6 +874,7 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   p.m_tiles = (M + TM - 1) / TM; p.n_tiles = (N + BN - 1) / BN; p.k_blocks = (K + BK - 1) / BK;
   p.n_fastest = 1;
   p.c_out = C; p.c_pitch = N; p.c_fp32 = 1;
+  if (ctx->ws) p.sync = slot_ptr<unsigned int>(ctx, 0, ctx->lay.off_sync);
   const int units = p.m_tiles * p.n_tiles;
   const bool a_mn = layout == 2, b_mn = layout >= 1;
   set_desc_defaults(p, a_mn, b_mn);

@@ -6,13 +6,17 @@ import torch
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module", params=[2, 1], ids=["cta_pair", "single_cta"])
+@pytest.fixture(scope="module", params=[(2, 0), (1, 0), (2, 1), (2, -1)],
+                ids=["cta_pair", "single_cta", "cta_pair_gate_every_kblock", "cta_pair_gate_off"])
 def ctx(request):
-    """Both tcgen05 variants of the kernel: cta_group::2 pair tiles (the default) and cta_group::1."""
+    """Both tcgen05 variants of the kernel: cta_group::2 pair tiles (the default) and cta_group::1; the
+    drift gate (a performance-only producer throttle) at its default epoch, at the
+    tightest epoch (every k block: the gate is exercised on every iteration) and off."""
     from paper_2606_26997_b200 import GrpoContext
     from paper_2606_26997_b200.build import build
     build()
-    c = GrpoContext(64, 1000, gemm_cta_group=request.param)
+    cg, drift = request.param
+    c = GrpoContext(64, 1000, max_tokens=256, gemm_cta_group=cg, gemm_drift_epoch_kb=drift)
     yield c
     c.close()
 
