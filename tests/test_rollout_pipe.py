@@ -150,3 +150,98 @@ def test_modes_do_the_same_training_work_and_cgp_is_never_later():
         assert sorted(g for u in r.update_groups for g in u) == list(range(R))
         assert all(s >= rd for s, rd in zip(r.start, r.ready))
         assert all(r.start[j + 1] >= r.end[j] for j in range(len(r.start) - 1))
+
+
+# ------------------------------------------------------------------------------------------- C ABI vs oracle
+@pytest.fixture(scope="module")
+def rp():
+    from paper_2606_26997_b200.build import build
+    build()
+    from paper_2606_26997_b200 import rollout_pipe
+    return rollout_pipe
+
+
+def test_abi_exports_every_declared_symbol(rp):
+    import re
+    root = os.path.dirname(os.path.dirname(__file__))
+    header = open(os.path.join(root, "include", "rollout_pipe.h")).read()
+    declared = set(re.findall(r"^int32_t\s+(rp_\w+)\s*\(", header, flags=re.M))
+    assert declared == set(rp.RP_EXPORTS)
+    from paper_2606_26997_b200.binding import load_library
+    lib = load_library()
+    for name in declared:
+        getattr(lib, name)
+
+
+def test_abi_paper_examples(rp):
+    assert rp.rp_fgd_frontier([5, 3, 1, 2, 4, 6], 2) == [1, 2]                       # Eq. 5
+    K = 4
+    work = np.array([[10.0] * K] + [[20.0] * K] * 5)
+    _, gdone, trace = rp.rp_rollout(work, 8.0, 0.0, F_w=2, trace_cap=16)
+    assert trace[0][1] == [0, 1] and trace[1][1] == [1, 2]
+    tl = rp.rp_cgp_timeline([210.0, 250.0], [10.0, 10.0], 2, rp.MODE_CGP)
+    assert tl["t_first_U"] == 250.0 and tl["start"][0] - 210.0 == 40.0
+    ts = rp.rp_cgp_timeline(np.linspace(200.0, 400.0, 96), np.ones(96), 2, rp.MODE_SLIME)
+    assert ts["t_start"] == 400.0 and all(r == 400.0 for r in ts["ready"])
+
+
+def _round(seed, R, K):
+    """Seeded synthetic round with the paper's shape parameters (K = 8, U = 2, F_w = 2, responses of a few
+    thousand tokens); stands in for its workloads."""
+    rng = np.random.default_rng(seed)
+    work = np.minimum(rng.geometric(1.0 / 2000.0, size=(R, K)), 8192).astype(np.float64)
+    mat = rng.uniform(0.2, 3.0, size=R)
+    train = work.sum(axis=1) / 4500.0          # ~4.5k response tokens/s whole-trainer rate (SURVEY.md section 6)
+    return work, mat, train
+
+
+@pytest.mark.parametrize("seed,R,K,U,F_w,cap", [(0, 32, 8, 2, 2, 0.0), (1, 96, 8, 2, 2, 0.0), (2, 17, 5, 3, 4, 40.0),
+                                                (3, 64, 8, 2, 1, 0.0), (4, 6, 2, 4, 9, 25.0), (5, 1, 8, 2, 2, 0.0)])
+def test_abi_matches_oracle(rp, seed, R, K, U, F_w, cap):
+    work, mat, train = _round(seed, R, K)
+    C_tok = 6000.0
+    for fw in (0, F_w):
+        rd_o, gd_o, tr_o = O.rollout(work, C_tok, cap, fw)
+        rd, gd, tr = rp.rp_rollout(work, C_tok, cap, fw, trace_cap=4 * R)
+        np.testing.assert_allclose(rd, rd_o, rtol=1e-10, atol=1e-9)
+        np.testing.assert_allclose(gd, gd_o, rtol=1e-10, atol=1e-9)
+        if fw > 0:                     # distinct geometric lengths: no simultaneous group completions
+            assert [F for _, F in tr] == [F for _, F in tr_o]
+            np.testing.assert_allclose([t for t, _ in tr], [t for t, _ in tr_o], rtol=1e-10, atol=1e-9)
+    for mode in (O.MODE_SLIME, O.MODE_CGP, O.MODE_CGP_FGD):
+        o = O.simulate(work, C_tok, cap, F_w, U, mode, mat, train)
+        c = rp.rp_simulate(work, C_tok, cap, F_w, U, mode, mat, train)
+        assert c["fifo_order"] == o.fifo_order
+        for k in ("t_first_U", "t_complete", "dt_cgp", "t_start", "t_train_end", "compute", "wait", "w_train_eq4",
+                  "w_train_alt"):
+            assert c[k] == pytest.approx(getattr(o, k), rel=1e-10, abs=1e-9), k
+        np.testing.assert_allclose(c["ready"], o.ready, rtol=1e-10, atol=1e-9)
+        np.testing.assert_allclose(c["start"], o.start, rtol=1e-10, atol=1e-9)
+        np.testing.assert_allclose(c["end"], o.end, rtol=1e-10, atol=1e-9)
+        assert c["n_updates"] == len(o.update_groups)
+
+
+def test_abi_edge_cases(rp):
+    tl = rp.rp_cgp_timeline([], [], 2, rp.MODE_CGP)                                   # empty round
+    assert tl["n_updates"] == 0 and tl["t_train_end"] == 0.0
+    rd, gd, _ = rp.rp_rollout(np.zeros((3, 2)), 10.0)                                 # zero-length responses
+    assert np.all(rd == 0.0) and np.all(gd == 0.0)
+    with pytest.raises(ValueError):
+        rp.rp_rollout(np.ones((2, 2)), 0.0)                                           # capacity must be > 0
+    with pytest.raises(ValueError):
+        rp.rp_cgp_timeline([1.0], [1.0], 0, rp.MODE_CGP)                              # U >= 1
+
+
+def test_paper_trend_cgp_gain_grows_with_R(rp):
+    """Qualitative claim of section 5.2: the reduction of rollout-to-train-end time over Slime
+    grows with R; CGP+FGD starts the trainer earlier than Slime at every R.  Model-level check only."""
+    gains = []
+    for R in (32, 64, 96):
+        work, mat, train = _round(100 + R, R, 8)
+        cap_tok = work.sum() / (train.sum())          # rollout and training take about equally long
+        s = rp.rp_simulate(work, cap_tok, 0.0, 2, 2, rp.MODE_SLIME, mat, train)
+        f = rp.rp_simulate(work, cap_tok, 0.0, 2, 2, rp.MODE_CGP_FGD, mat, train)
+        assert f["t_start"] < s["t_start"] and f["compute"] == pytest.approx(s["compute"])
+        gains.append(1.0 - f["t_train_end"] / s["t_train_end"])
+    assert gains[0] < gains[1] < gains[2]
+    assert 0.2 < gains[2] < 0.5
