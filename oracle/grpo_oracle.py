@@ -45,6 +45,8 @@ class OracleConfig:
     kl_beta: float = 0.0         # 0 disables the k3 term
     loss_agg: int = 0            # 0 token mean over the logical update, 1 per-sequence mean
     logit_scale: float = 1.0     # 1 / temperature
+    kl_type: int = 0             # NEXT-2: 0 = k3 (north_star), 1 = k1, 2 = k2 (R26)
+    dual_clip: float = 0.0       # NEXT-2: 0 = off; c > 1: for A < 0 the surrogate is max(s, c A) (R27)
     chunk_tokens: int = 1024     # memory bound only; results do not depend on it
 
 
@@ -154,14 +156,28 @@ def loss_terms(logp, old_logp, ref_logp, mask, adv_tok, cu_seqlens, cfg: OracleC
     surr = np.minimum(rho * A, np.clip(rho, lo, hi) * A)
     use_kl = cfg.kl_beta != 0.0 and ref_logp is not None
     if use_kl:
+        # per-sample estimators of KL(pi || pi_ref) on samples from pi, with r = pi_ref / pi = exp(delta):
+        #   k1 = -log r,   k2 = (log r)^2 / 2,   k3 = (r - 1) - log r      (R8, R26)
         delta = np.asarray(ref_logp, dtype=np.float64) - logp
-        k3 = np.exp(delta) - delta - 1.0
-        dk3 = 1.0 - np.exp(delta)                      # d k3 / d logp
+        if cfg.kl_type == 1:
+            k3 = -delta
+            dk3 = np.ones(T)                           # d k1 / d logp
+        elif cfg.kl_type == 2:
+            k3 = 0.5 * delta * delta
+            dk3 = -delta                               # d k2 / d logp
+        else:
+            k3 = np.exp(delta) - delta - 1.0
+            dk3 = 1.0 - np.exp(delta)                  # d k3 / d logp
     else:
         k3 = np.zeros(T)
         dk3 = np.zeros(T)
-    ell = -surr + cfg.kl_beta * k3
     clipped = ((A > 0) & (rho > hi)) | ((A < 0) & (rho < lo))
+    if cfg.dual_clip > 0.0:
+        # dual clip (R27): a negative-advantage token whose ratio exceeds c contributes the
+        # constant c A instead of rho A, so its policy gradient vanishes
+        surr = np.where(A < 0, np.maximum(surr, cfg.dual_clip * A), surr)
+        clipped = clipped | ((A < 0) & (rho > cfg.dual_clip))
+    ell = -surr + cfg.kl_beta * k3
     u = np.where(clipped, 0.0, 1.0)
     coeff = w * (-A * rho * u + cfg.kl_beta * dk3)
     # w == 0 tokens (masked / invalid) contribute exact zeros even if ell is inf/nan-free
@@ -337,9 +353,17 @@ def grpo_step_loops(H, W, y, cu_seqlens, rewards, old_logp, ref_logp=None, mask=
         k3 = dk3 = 0.0
         if cfg.kl_beta != 0.0 and ref_logp is not None:
             delta = float(ref_logp[t]) - logp[t]
-            k3 = math.exp(delta) - delta - 1.0
-            dk3 = 1.0 - math.exp(delta)
+            if cfg.kl_type == 1:
+                k3, dk3 = -delta, 1.0
+            elif cfg.kl_type == 2:
+                k3, dk3 = 0.5 * delta * delta, -delta
+            else:
+                k3 = math.exp(delta) - delta - 1.0
+                dk3 = 1.0 - math.exp(delta)
         clipped = (A > 0 and rho > hi) or (A < 0 and rho < lo)
+        if cfg.dual_clip > 0.0 and A < 0:
+            surr = max(surr, cfg.dual_clip * A)
+            clipped = clipped or rho > cfg.dual_clip
         if w[t] != 0.0:
             loss += w[t] * (-surr + cfg.kl_beta * k3)
             coeff[t] = w[t] * (-A * rho * (0.0 if clipped else 1.0) + cfg.kl_beta * dk3)
