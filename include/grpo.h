@@ -72,6 +72,15 @@ typedef struct {
                                 one epoch of this many k blocks of each other so that the operand panels they
                                 share are fetched from HBM once.  0 = default (32),
                                 < 0 = off.  Performance only: results do not depend on it. */
+  int32_t kl_type;           /* KL estimator weighted by kl_beta (R8, R26): 0 = k3 (default),
+                                1 = k1 = logp - ref, 2 = k2 = (logp - ref)^2 / 2 */
+  float   dual_clip;         /* 0 = off; c > 1: for A < 0 the surrogate is max(min(rho A, clip(rho) A), c A)
+                                (R27) */
+  int32_t bwd_skip_zero_tiles; /* 0 = default (on), < 0 = off.  The backward skips every token tile whose
+                                coefficients dloss/dlogp are all exactly zero (zero-variance groups at
+                                kl_beta = 0, masked spans): their dHidden rows are written as zeros and they
+                                add nothing to dW, which is what the dense computation gives (DESIGN.md
+                                section 10).  Decided on the device; no host synchronisation. */
 } grpo_config;
 
 /* Fill *cfg with the defaults above (d, V must still be set). */
@@ -190,8 +199,13 @@ enum {
   GRPO_KERNEL_GEMM_DH = 5,     /* A5: dH = dZ W */
   GRPO_KERNEL_GEMM_DW = 6,     /* A6: dW += dZ^T H */
   GRPO_KERNEL_DEBUG = 7,       /* grpo_debug_gemm */
-  GRPO_NUM_KERNEL_KINDS = 8
+  GRPO_KERNEL_TILE_SCAN = 8,   /* backward: zero-coefficient tile scan + zero fill of skipped dHidden rows */
+  GRPO_NUM_KERNEL_KINDS = 9
 };
+
+/* Token tiles the backward calls of workspace slot 0 walked (active) and saw (total) since the last call
+ * of this function; both 0 when bwd_skip_zero_tiles is off.  Synchronises. */
+int32_t grpo_bwd_tile_stats_sync(grpo_ctx* ctx, int64_t* active_out /*HOST*/, int64_t* total_out /*HOST*/);
 
 /* counts_out HOST int64 [GRPO_NUM_KERNEL_KINDS]: kernels launched by this context since creation. */
 int32_t grpo_kernel_launches(const grpo_ctx* ctx, int64_t* counts_out);

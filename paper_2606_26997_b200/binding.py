@@ -22,9 +22,9 @@ EXPORTS = [
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
-    "grpo_profile_enable", "grpo_profile_read_sync",
+    "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
 ]
-KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug"]
+KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan"]
 
 
 class GrpoError(RuntimeError):
@@ -39,7 +39,8 @@ class GrpoConfig(C.Structure):
                 ("logit_scale", C.c_float), ("dhidden_fp32", C.c_int32), ("group_size", C.c_int32),
                 ("groups_per_update", C.c_int32), ("groups_per_round", C.c_int32), ("token_budget", C.c_int64),
                 ("bwd_chunk_tokens", C.c_int64), ("max_pending_groups", C.c_int32), ("gemm_cta_group", C.c_int32),
-                ("gemm_drift_epoch_kb", C.c_int32)]
+                ("gemm_drift_epoch_kb", C.c_int32), ("kl_type", C.c_int32), ("dual_clip", C.c_float),
+                ("bwd_skip_zero_tiles", C.c_int32)]
 
 
 class GroupDesc(C.Structure):
@@ -87,6 +88,7 @@ def load_library() -> C.CDLL:
     lib.grpo_kernel_launches.argtypes = [vp, C.POINTER(i64)]
     lib.grpo_profile_enable.argtypes = [vp, i32]
     lib.grpo_profile_read_sync.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
+    lib.grpo_bwd_tile_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     _LIB = lib
     return lib
 
@@ -324,6 +326,11 @@ class GrpoContext:
         n = (C.c_int64 * len(KERNEL_KINDS))()
         _check(self.lib.grpo_profile_read_sync(self.h, ms, n))
         return {k: dict(ms=ms[i], launches=n[i]) for i, k in enumerate(KERNEL_KINDS)}
+
+    def grpo_bwd_tile_stats_sync(self):
+        a, t = C.c_int64(0), C.c_int64(0)
+        _check(self.lib.grpo_bwd_tile_stats_sync(self.h, C.byref(a), C.byref(t)))
+        return a.value, t.value
 
     # ------------------------------------------------------------------ test hook
     def grpo_debug_gemm(self, layout: int, A, B, M: int, N: int, K: int, C_out=None, accumulate: bool = False,

@@ -73,6 +73,11 @@ struct GemmParams {
   void* c_out;
   int64_t c_pitch;                   // elements
   int c_fp32;
+  // zero-coefficient tile skipping (A4-A6): device list written by
+  // active_tiles_kernel: [0] = number of active token tiles, [1] = tiles in the chunk, [2 ..] = their
+  // indices (ascending).  nullptr: every tile is active.  A4/A5 walk only active m tiles; A6 walks only the
+  // k blocks (token rows) of active tiles.
+  const int* tile_list;
   // drift bound between the CTA pairs of one launch (see the producer loop); sync == nullptr: off
   unsigned int* sync;
   int sync_epoch_kb;                 // k blocks per epoch
@@ -88,21 +93,51 @@ struct alignas(8) GemmBarriers {
   int gate_open;                     // highest epoch the producer may enter (written by the gate warp)
 };
 
-__device__ __forceinline__ void unit_to_tiles(const GemmParams& p, int u, int epi, int& m_tile, int& n0, int& n1) {
-  if (epi == EPI_LSE) {
+// Effective extent of a launch under tile skipping: the number of m tiles walked (A4/A5), the k blocks
+// per unit (A6) and the unit count.  Uniform over the grid (one global load each).
+struct Extent { int m_tiles, k_blocks, n_units; };
+template <int CG, int EPI>
+__device__ __forceinline__ Extent launch_extent(const GemmParams& p, int n_units) {
+  Extent e{p.m_tiles, p.k_blocks, n_units};
+  if (p.tile_list != nullptr) {
+    const int n_active = p.tile_list[0];
+    if constexpr (EPI == EPI_RED_F32) {
+      e.k_blocks = min(p.k_blocks, n_active * (BM * CG / BK));
+      if (e.k_blocks == 0) e.n_units = 0;            // nothing to add: no MMA, so no epilogue either
+    } else {
+      e.m_tiles = n_active;
+      e.n_units = n_active * p.n_tiles;
+    }
+  }
+  return e;
+}
+// k block (in units of BK token rows) the kb-th walked k block of A6 maps to
+template <int CG>
+__device__ __forceinline__ int walked_k_block(const GemmParams& p, int kb) {
+  constexpr int kPerTile = BM * CG / BK;
+  return p.tile_list == nullptr ? kb : p.tile_list[2 + kb / kPerTile] * kPerTile + kb % kPerTile;
+}
+
+template <int EPI>
+__device__ __forceinline__ void unit_to_tiles(const GemmParams& p, const Extent& e, int u, int& m_tile, int& n0,
+                                              int& n1) {
+  if constexpr (EPI == EPI_LSE) {
     m_tile = u % p.m_tiles;
     int split = u / p.m_tiles;
     n0 = split * p.tiles_per_split;
     n1 = min(p.n_tiles, n0 + p.tiles_per_split);
-  } else if (p.n_fastest) {
-    n0 = u % p.n_tiles;
-    m_tile = u / p.n_tiles;
-    n1 = n0 + 1;
-  } else {
-    m_tile = u % p.m_tiles;
-    n0 = u / p.m_tiles;
-    n1 = n0 + 1;
+    return;
   }
+  int m_idx;
+  if (p.n_fastest) {
+    n0 = u % p.n_tiles;
+    m_idx = u / p.n_tiles;
+  } else {
+    m_idx = u % e.m_tiles;
+    n0 = u / e.m_tiles;
+  }
+  n1 = n0 + 1;
+  m_tile = (EPI != EPI_RED_F32 && p.tile_list != nullptr) ? p.tile_list[2 + m_idx] : m_idx;
 }
 
 // Drift bound.  The CTA pairs of a launch that share operand panels through L2 (the 8 d-tiles of one dZ
@@ -131,7 +166,7 @@ __device__ __forceinline__ void st_volatile_shared_i32(int* p, int v) {
 template <int CG, bool A_MN, bool B_MN, int EPI>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                 const GemmParams p, const int n_units) {
+                 const GemmParams p, const int n_units_dense) {
   using Shape = GemmShape<CG>;
   constexpr int kStages = Shape::kStages;
   constexpr int kStageBytes = Shape::kStageBytes;
@@ -149,6 +184,8 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   const uint32_t cta_rank = CG == 2 ? cluster_ctarank() : 0u;   // 0 = leader (issues the MMAs)
   const int unit0 = blockIdx.x / CG;                             // CTA pairs walk the unit list together
   const int unit_step = gridDim.x / CG;
+  const Extent ext = launch_extent<CG, EPI>(p, n_units_dense);
+  const int n_units = ext.n_units;
 
   if (warp == kProducerWarp && lane == 0) {
     prefetch_tmap(&tmA);
@@ -179,11 +216,12 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       int epoch = 0, to_epoch = 1;
       for (int u = unit0; u < n_units; u += unit_step) {
         int m_tile, n0, n1;
-        unit_to_tiles(p, u, EPI, m_tile, n0, n1);
+        unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
         const int a_row = (m_tile * CG + static_cast<int>(cta_rank)) * BM;
         for (int n_tile = n0; n_tile < n1; ++n_tile) {
           const int b_row = n_tile * BN + static_cast<int>(cta_rank) * kBRows;
-          for (int kb = 0; kb < p.k_blocks; ++kb) {
+          for (int kbw = 0; kbw < ext.k_blocks; ++kbw) {
+            const int kb = EPI == EPI_RED_F32 ? walked_k_block<CG>(p, kbw) : kbw;
             if (sync_on && cta_rank == 0 && --to_epoch == 0) {
               to_epoch = p.sync_epoch_kb;
               red_add_u32(p.sync + epoch, 1u);
@@ -239,12 +277,12 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       uint32_t acc_phase = 0;
       for (int u = unit0; u < n_units; u += unit_step) {
         int m_tile, n0, n1;
-        unit_to_tiles(p, u, EPI, m_tile, n0, n1);
+        unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
         for (int n_tile = n0; n_tile < n1; ++n_tile) {
           mbar_wait(&bars->tmem_empty[acc], acc_phase ^ 1);
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + acc * BN;
-          for (int kb = 0; kb < p.k_blocks; ++kb) {
+          for (int kb = 0; kb < ext.k_blocks; ++kb) {
             mbar_wait(&bars->full[stage], phase);
             tc_fence_after();
             if (leader_lane) {
@@ -273,8 +311,8 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       long long my_kb = 0;
       for (int u = unit0; u < n_units; u += unit_step) {
         int m_tile, n0, n1;
-        unit_to_tiles(p, u, EPI, m_tile, n0, n1);
-        my_kb += static_cast<long long>(n1 - n0) * p.k_blocks;
+        unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
+        my_kb += static_cast<long long>(n1 - n0) * ext.k_blocks;
       }
       const int my_epochs = static_cast<int>((my_kb + p.sync_epoch_kb - 1) / p.sync_epoch_kb);
       const unsigned int n_pairs = gridDim.x / CG;
@@ -297,7 +335,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     uint32_t acc_phase = 0;
     for (int u = unit0; u < n_units; u += unit_step) {
       int m_tile, n0, n1;
-      unit_to_tiles(p, u, EPI, m_tile, n0, n1);
+      unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
       const int row_local = (m_tile * CG + static_cast<int>(cta_rank)) * BM + row_in_tile;   // row within this launch's C
       const bool row_ok = row_local < p.m_total;
       const int64_t row_g = p.row_offset + row_local;            // index into per-token arrays

@@ -55,7 +55,9 @@ struct SlotLayout {
   int64_t v_pad = 0;
   int64_t off_part_m = 0, off_part_s = 0, off_zy = 0, off_total = 0, off_seq_count = 0, off_dz = 0;
   int64_t off_hidden = 0, off_targets = 0, off_old = 0, off_ref = 0, off_mask = 0, off_rewards = 0, off_adv = 0,
-          off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0, off_sync = 0;
+          off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0, off_sync = 0,
+          off_tiles = 0, off_tile_stats = 0;
+  int64_t tile_cap = 0;   // token tiles per backward chunk
   int64_t bytes = 0;
 };
 
@@ -147,6 +149,9 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.off_coeff = take(max_T * 4);
   L.off_dh = take(max_T * c.d * (c.dhidden_fp32 ? 4 : 2));
   L.off_sync = take(kSyncCap * 4);
+  L.tile_cap = L.chunk_rows / BM + 1;
+  L.off_tiles = take((2 + 2 * L.tile_cap) * 4);
+  L.off_tile_stats = take(16);
   L.bytes = off;
   return L;
 }
@@ -278,6 +283,8 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
     return fail(GRPO_ERR_INVALID_ARG, "gemm_cta_group must be 0 (default), 1 or 2");
   if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
     return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
+  if (cfg->kl_type < 0 || cfg->kl_type > 2 || (cfg->dual_clip != 0.f && !(cfg->dual_clip > 1.f)))
+    return fail(GRPO_ERR_INVALID_ARG, "kl_type must be 0, 1 or 2 and dual_clip 0 or > 1");
   int dev = 0;
   CU_OK(cudaGetDevice(&dev));
   cudaDeviceProp prop;
@@ -337,6 +344,7 @@ extern "C" int32_t grpo_set_workspace(grpo_ctx* ctx, void* dev_ptr, int64_t byte
   ctx->ws_max_T = max_T;
   ctx->n_slots = n_slots;
   ctx->lay = L;
+  for (int i = 0; i < n_slots; ++i) CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_tile_stats), 0, 16));
   return GRPO_OK;
 }
 
@@ -373,6 +381,20 @@ extern "C" int32_t grpo_profile_read_sync(grpo_ctx* ctx, double* ms_out, int64_t
     launches_out[r.kind]++;
   }
   prof_clear(ctx);
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_bwd_tile_stats_sync(grpo_ctx* ctx, int64_t* active_out, int64_t* total_out) {
+  if (!ctx || !active_out || !total_out) return fail(GRPO_ERR_INVALID_ARG, "NULL pointer");
+  *active_out = *total_out = 0;
+  if (!ctx->ws) return GRPO_OK;
+  int h[2] = {0, 0};
+  int* stats = slot_ptr<int>(ctx, 0, ctx->lay.off_tile_stats);
+  CU_OK(cudaDeviceSynchronize());
+  CU_OK(cudaMemcpy(h, stats, 8, cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemset(stats, 0, 8));
+  *active_out = h[0];
+  *total_out = h[1];
   return GRPO_OK;
 }
 
@@ -456,6 +478,7 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   lp.seq_count = seq_count; lp.total_count = denom_dev ? denom_dev : total;
   lp.denom_host = loss_denom > 0.0 ? static_cast<float>(loss_denom) : 0.f;
   lp.loss_agg = c.loss_agg; lp.clip_lo = c.clip_lo; lp.clip_hi = c.clip_hi; lp.kl_beta = c.kl_beta;
+  lp.kl_type = c.kl_type; lp.dual_clip = c.dual_clip;
   lp.logp = logp_out; lp.lse = lse_out; lp.coeff = coeff_out; lp.loss_accum = loss_accum;
   lp.metrics_accum = metrics_accum; lp.err_flag = ctx->err_dev;
   const int threads = 256;
@@ -512,6 +535,25 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
     GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
 
+    // zero-coefficient tile skipping: scan this chunk's coefficients on the device
+    const int* tile_list = nullptr;
+    if (c.bwd_skip_zero_tiles >= 0) {
+      int* list = slot_ptr<int>(ctx, slot, L.off_tiles);
+      {
+        LaunchScope ls(ctx, GRPO_KERNEL_TILE_SCAN, st);
+        active_tiles_kernel<<<1, 1024, 0, st>>>(coeff + t0, static_cast<int>(rows), TM, static_cast<int>(L.tile_cap), list,
+                                                slot_ptr<int>(ctx, slot, L.off_tile_stats));
+      }
+      CU_OK(cudaGetLastError());
+      if (dhidden_out) {
+        LaunchScope ls(ctx, GRPO_KERNEL_TILE_SCAN, st);
+        zero_inactive_rows_kernel<<<m_tiles, 256, 0, st>>>(static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem,
+                                                           static_cast<int64_t>(c.d) * dh_elem, static_cast<int>(rows), TM,
+                                                           list + 2 + L.tile_cap);
+        CU_OK(cudaGetLastError());
+      }
+      tile_list = list;
+    }
     {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
@@ -522,7 +564,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.row_offset = t0; p.targets = targets;
       p.scale_log2e = c.logit_scale * kLog2e; p.logit_scale = c.logit_scale;
       p.lse = lse; p.coeff = coeff; p.coeff_mul = c.logit_scale * grad_scale;
-      p.dz = dz; p.dz_pitch = L.v_pad;
+      p.dz = dz; p.dz_pitch = L.v_pad; p.tile_list = tile_list;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, GRPO_KERNEL_GEMM_DZ, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
     }
@@ -534,6 +576,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
       p.n_fastest = 1;
       p.c_out = static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem; p.c_pitch = c.d; p.c_fp32 = c.dhidden_fp32;
+      p.tile_list = tile_list;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
     }
@@ -547,7 +590,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
-      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1;
+      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.tile_list = tile_list;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_GEMM_DW, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st)));
     }

@@ -97,6 +97,8 @@ struct LossParams {
   float denom_host;          // > 0: explicit
   int loss_agg;
   float clip_lo, clip_hi, kl_beta;
+  int kl_type;               // 0 = k3, 1 = k1, 2 = k2 (R26)
+  float dual_clip;           // 0 = off (R27)
   float* logp;
   float* lse;
   float* coeff;
@@ -140,14 +142,26 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
     if (m != 0.f) {
       const float rho = expf(logp - p.old_logp[t]);
       const float lo_b = 1.f - p.clip_lo, hi_b = 1.f + p.clip_hi;
-      const float surr = fminf(rho * A, fminf(fmaxf(rho, lo_b), hi_b) * A);
-      const bool clipped = (A > 0.f && rho > hi_b) || (A < 0.f && rho < lo_b);
+      float surr = fminf(rho * A, fminf(fmaxf(rho, lo_b), hi_b) * A);
+      bool clipped = (A > 0.f && rho > hi_b) || (A < 0.f && rho < lo_b);
+      if (p.dual_clip > 0.f && A < 0.f) {
+        surr = fmaxf(surr, p.dual_clip * A);
+        clipped = clipped || rho > p.dual_clip;
+      }
       float k3 = 0.f, dk3 = 0.f;
       if (p.kl_beta != 0.f && p.ref_logp != nullptr) {
         const float delta = p.ref_logp[t] - logp;
-        const float e = expf(delta);
-        k3 = e - delta - 1.f;
-        dk3 = 1.f - e;
+        if (p.kl_type == 1) {
+          k3 = -delta;
+          dk3 = 1.f;
+        } else if (p.kl_type == 2) {
+          k3 = 0.5f * delta * delta;
+          dk3 = -delta;
+        } else {
+          const float e = expf(delta);
+          k3 = e - delta - 1.f;
+          dk3 = 1.f - e;
+        }
       }
       loss_t = w * (-surr + p.kl_beta * k3);
       coeff = w * ((clipped ? 0.f : -A * rho) + p.kl_beta * dk3);
@@ -180,6 +194,45 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
       }
     }
   }
+}
+
+// Zero-coefficient tile scan.  One block; warp w scans token tiles w, w + nwarps, ...
+// of `tile_rows` rows: a tile is active iff any coeff in it is non-zero.  Output list: [0] = n_active,
+// [1] = n_tiles, [2 .. 2 + n_active) = active tile indices ascending, [2 + cap .. 2 + cap + n_tiles) =
+// per-tile flags.  stats (nullable): [0] += n_active, [1] += n_tiles.
+__global__ void __launch_bounds__(1024) active_tiles_kernel(const float* __restrict__ coeff, int rows, int tile_rows,
+                                                            int cap, int* __restrict__ list, int* __restrict__ stats) {
+  const int n_tiles = (rows + tile_rows - 1) / tile_rows;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+  int* flags = list + 2 + cap;
+  for (int tile = warp; tile < n_tiles; tile += n_warps) {
+    const int beg = tile * tile_rows, end = min(rows, beg + tile_rows);
+    bool any = false;
+    for (int r = beg + lane; r < end; r += 32) any |= coeff[r] != 0.f;
+    any = __any_sync(0xffffffffu, any);
+    if (lane == 0) flags[tile] = any ? 1 : 0;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int n = 0;
+    for (int tile = 0; tile < n_tiles; ++tile)
+      if (flags[tile]) list[2 + n++] = tile;
+    list[0] = n;
+    list[1] = n_tiles;
+    if (stats) { atomicAdd(stats, n); atomicAdd(stats + 1, n_tiles); }
+  }
+}
+
+// dHidden rows of skipped tiles are zeros (what the dense A5 would have produced from an all-zero dZ
+// panel).  One block per tile; 16-byte stores (row_bytes is a multiple of 16: d % 8 == 0).
+__global__ void __launch_bounds__(256) zero_inactive_rows_kernel(uint8_t* __restrict__ out, int64_t row_bytes, int rows,
+                                                                 int tile_rows, const int* __restrict__ flags) {
+  const int tile = blockIdx.x;
+  if (flags[tile]) return;
+  const int beg = tile * tile_rows, end = min(rows, beg + tile_rows);
+  uint4* dst = reinterpret_cast<uint4*>(out + static_cast<int64_t>(beg) * row_bytes);
+  const int64_t n = static_cast<int64_t>(end - beg) * row_bytes / 16;
+  for (int64_t i = threadIdx.x; i < n; i += blockDim.x) dst[i] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 }  // namespace grpo

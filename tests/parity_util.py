@@ -15,9 +15,11 @@ def oracle_cfg(b, **kw):
                         loss_agg=b.loss_agg, **kw)
 
 
-def run_oracle(b, loss_denom=None, std_ddof=0, logit_scale=1.0, need_grads=True, chunk=1024):
+def run_oracle(b, loss_denom=None, std_ddof=0, logit_scale=1.0, need_grads=True, chunk=1024, kl_type=0,
+               dual_clip=0.0):
     x = b.numpy_f64()
-    cfg = oracle_cfg(b, std_ddof=std_ddof, logit_scale=logit_scale, chunk_tokens=chunk)
+    cfg = oracle_cfg(b, std_ddof=std_ddof, logit_scale=logit_scale, chunk_tokens=chunk, kl_type=kl_type,
+                     dual_clip=dual_clip)
     return grpo_step(x["H"], x["W"], x["y"], x["cu_seqlens"], x["rewards"], x["old_logp"], x["ref_logp"],
                      mask=x["mask"], cfg=cfg, G=b.G, loss_denom=loss_denom, need_grads=need_grads)
 
