@@ -196,6 +196,13 @@ def reduce_over_ranks(ms_total: float, e2e_s: float, tokens: int, world: int, de
 
 
 GEMM_KINDS = ("gemm_lse", "gemm_dz", "gemm_dh", "gemm_dw")
+WORKLOADS = {
+    2: "configs[1]: one complete group G=8, lengths U[512,4096], d=2048, V=151936, on-policy old log-probs, "
+       "no KL; one such group per GPU",
+    3: "configs[2] (informational): 4 groups x G=8, lognormal lengths, zero-variance groups kept, KL beta=0.001",
+    4: "configs[3] (informational): 8 groups x G=16, lognormal long-tail lengths, Beta-Bernoulli rewards, no KL",
+    5: "configs[4] as ONE full-batch step (informational): 32 groups x G=8, geometric lengths, no KL",
+}
 
 
 def run_ours(args):
@@ -226,10 +233,15 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
-    b = make_config(2, seed=rank_seed(rank), device=dev)
+    b = make_config(args.config, seed=rank_seed(rank), device=dev)
     T, d, V = b.T, b.d, b.V
+    extra = {}
+    if args.no_tile_skip:
+        extra["bwd_skip_zero_tiles"] = -1
+    if args.no_drift_gate:
+        extra["gemm_drift_epoch_kb"] = -1
     ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
-                      gemm_cta_group=args.cta_group, **({"bwd_chunk_tokens": args.bwd_chunk} if args.bwd_chunk else {}))
+                      gemm_cta_group=args.cta_group, **extra, **({"bwd_chunk_tokens": args.bwd_chunk} if args.bwd_chunk else {}))
     dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
     loss = torch.zeros(1, dtype=torch.float32, device=dev)
     dH = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
@@ -249,6 +261,7 @@ def run_ours(args):
 
     # ---- timed region: K steps, CUDA events on the launch stream, per-kernel events inside the library
     sampler = ClockSampler(local)
+    ctx.grpo_bwd_tile_stats_sync()          # clear
     n0 = ctx.grpo_kernel_launches()
     ctx.grpo_profile_enable(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -264,12 +277,26 @@ def run_ours(args):
     ms_total = e0.elapsed_time(e1)
     prof = ctx.grpo_profile_read_sync()
     ctx.grpo_profile_enable(False)
+    tiles_walked, tiles_total = ctx.grpo_bwd_tile_stats_sync()
+    args.bwd_active_frac = tiles_walked / tiles_total if tiles_total > 0 else 1.0
+    args.bwd_tiles = {"walked": tiles_walked, "total": tiles_total}
     n1 = ctx.grpo_kernel_launches()
     launches = sum(n1.values()) - sum(n0.values())
     loss_val = loss.item()
     assert loss_val == loss_val, "loss is NaN"
 
     # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step
+    # (headline workload only; --config 3/4/5 are informational device-resident runs)
+    if args.config != 2:
+        ms_total, _, tokens_all = reduce_over_ranks(ms_total, 0.0, T, world, dev)
+        if rank == 0:
+            line = build_line(args, b, world, tokens_all * args.steps / (ms_total * 1e-3), ms_total, None, 0, 0,
+                              launches, prof, clocks, load_peaks(), tokens_all, loss_val)
+            print(json.dumps(line), flush=True)
+        ctx.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
     pin = lambda t: None if t is None else t.cpu().pin_memory()
     h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
                                                    pin(b.old_logp))
@@ -324,41 +351,47 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
     peak = float(peaks.get("bf16_tflops_sustained") or peaks["bf16_tflops"])
     peak_burst = float(peaks["bf16_tflops"])
     kernels = {}
+    # executed FLOPs: the backward contractions walk only token tiles with a non-zero coefficient
+    act = getattr(args, "bwd_active_frac", 1.0)
+    kind_flops = {k: flops_per_gemm_step * (1.0 if k == "gemm_lse" else act) for k in GEMM_KINDS}
     for k, v in prof.items():
         if v["launches"] == 0:
             continue
         e = {"ms_per_step": v["ms"] / steps, "launches_per_step": v["launches"] / steps}
         if k in GEMM_KINDS:
-            e["tflops"] = flops_per_gemm_step * steps / (v["ms"] * 1e-3) / 1e12
+            e["tflops"] = kind_flops[k] * steps / (v["ms"] * 1e-3) / 1e12
             e["frac_of_peak"] = e["tflops"] / peak
         kernels[k] = e
     gemm_ms = sum(prof[k]["ms"] for k in GEMM_KINDS)
     dom = max(GEMM_KINDS, key=lambda k: prof[k]["ms"])
     dom_tflops = kernels[dom]["tflops"]
-    path_tflops = 4 * flops_per_gemm_step * steps / (gemm_ms * 1e-3) / 1e12
-    step_tflops = 4 * flops_per_gemm_step * steps / (ms_total * 1e-3) / 1e12 if world == 1 else None
+    exec_flops = sum(kind_flops.values())
+    path_tflops = exec_flops * steps / (gemm_ms * 1e-3) / 1e12
+    step_tflops = exec_flops * steps / (ms_total * 1e-3) / 1e12 if world == 1 else None
     roofline = {
         "bound": "tensor", "kernel": dom, "achieved": dom_tflops, "peak": peak, "unit": "TFLOP/s",
         "frac": dom_tflops / peak, "traffic": NCU_TRAFFIC_BYTES.get(dom),
         "peak_source": f"{peaks['_source']} bf16_tflops_sustained (MEASURED_PEAKS.json); burst {peak_burst:g}",
         "frac_of_burst": dom_tflops / peak_burst,
-        "flops_per_launch": flops_per_gemm_step / kernels[dom]["launches_per_step"],
+        "flops_per_launch": kind_flops[dom] / kernels[dom]["launches_per_step"],
         "all_gemms": {"achieved": path_tflops, "frac": path_tflops / peak, "share_of_step": gemm_ms / ms_total},
         "whole_step": None if step_tflops is None else {"achieved": step_tflops, "frac": step_tflops / peak,
-                                                        "flops_basis": "8*T*V*d executed (4 contractions)"},
+                                                        "flops_basis": "executed: 2*T*V*d (A2) + 3*2*T_walked*V*d (A4-A6); "
+                                                                       "= 8*T*V*d when no tile is skipped"},
     }
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": "configs[1]: one complete group G=8, lengths U[512,4096], d=2048, V=151936, "
-                               "on-policy old log-probs, no KL; one such group per GPU",
+        "config": {"workload": WORKLOADS[args.config],
                    "tokens_per_step": int(tokens_all), "tokens_rank0": T, "d": d, "V": V, "G": b.G,
                    "parallelism": f"replicas x{world}: independent complete groups, no collective",
                    "l2": "inputs larger than L2 (W 622 MB, dW 1.2 GB, dZ chunk 2.9 GB vs 126 MB L2); no flush needed",
                    "bwd_chunk_tokens": args.bwd_chunk or "library default"},
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "api": "grpo_step_host (C ABI, pinned host buffers; W and dW resident on the device)"},
+        "e2e": None if e2e_value is None else {
+            "value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "api": "grpo_step_host (C ABI, pinned host buffers; W and dW resident on the device)"},
+        "bwd_tiles": getattr(args, "bwd_tiles", None),
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
         "loss_after_steps": loss_val,
     }
@@ -372,6 +405,11 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--cta-group", type=int, default=0, choices=[0, 1, 2],
                     help="grpo_config.gemm_cta_group: 0 = library default (CTA pairs), 1 = single-CTA tiles")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5],
+                    help="workload = workloads.synth.make_config index (2 = BASELINE configs[1], the headline; "
+                         "3-5 are informational device-resident runs without the e2e / cpu_baseline legs)")
+    ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
+    ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     args = ap.parse_args()
