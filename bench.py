@@ -240,17 +240,26 @@ def run_ours(args):
         extra["bwd_skip_zero_tiles"] = -1
     if args.no_drift_gate:
         extra["gemm_drift_epoch_kb"] = -1
+    if args.stash:
+        extra["stash_logits"] = 1           # grpo_step_host (the e2e leg) then uses the same variant
     ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
                       gemm_cta_group=args.cta_group, **extra, **({"bwd_chunk_tokens": args.bwd_chunk} if args.bwd_chunk else {}))
     dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
     loss = torch.zeros(1, dtype=torch.float32, device=dev)
     dH = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
 
-    def step():
+    def step_recompute():       # north_star: forward, then backward with the logits recomputed chunk by chunk
         adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
         f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
                                             b.mask, loss_accum=loss)
         ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW, dhidden_out=dH)
+
+    def step_stash():           # 3-contraction variant: logits stashed per chunk
+        adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+        ctx.grpo_fused_logprob_loss_fwd_bwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                            b.mask, loss_accum=loss, dW_accum=dW, dhidden_out=dH)
+
+    step = step_stash if args.stash else step_recompute
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -284,6 +293,25 @@ def run_ours(args):
     launches = sum(n1.values()) - sum(n0.values())
     loss_val = loss.item()
     assert loss_val == loss_val, "loss is NaN"
+
+    # ---- the other variant of the step, timed the same way (reported beside the headline, never as it)
+    args.other_variant = None
+    if not args.no_variants:
+        other = step_recompute if args.stash else step_stash
+        for _ in range(3):
+            other()
+        barrier()
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        v0.record()
+        for _ in range(args.steps):
+            other()
+        v1.record()
+        torch.cuda.synchronize()
+        barrier()
+        v_ms, _, v_tok = reduce_over_ranks(v0.elapsed_time(v1), 0.0, T, world, dev)
+        args.other_variant = {"variant": "recompute (north_star)" if args.stash else "stash_logits (3 contractions)",
+                              "value": v_tok * args.steps / (v_ms * 1e-3), "unit": UNIT,
+                              "ms_per_step": v_ms / args.steps}
 
     # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step
     # (headline workload only; --config 3/4/5 are informational device-resident runs)
@@ -353,7 +381,8 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
     kernels = {}
     # executed FLOPs: the backward contractions walk only token tiles with a non-zero coefficient
     act = getattr(args, "bwd_active_frac", 1.0)
-    kind_flops = {k: flops_per_gemm_step * (1.0 if k == "gemm_lse" else act) for k in GEMM_KINDS}
+    kind_flops = {k: flops_per_gemm_step * (1.0 if k == "gemm_lse" else act) * (prof[k]["launches"] > 0)
+                  for k in GEMM_KINDS}
     for k, v in prof.items():
         if v["launches"] == 0:
             continue
@@ -361,6 +390,9 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         if k in GEMM_KINDS:
             e["tflops"] = kind_flops[k] * steps / (v["ms"] * 1e-3) / 1e12
             e["frac_of_peak"] = e["tflops"] / peak
+        if k == "stash_dz":     # HBM-bound: 2 B read + 2 B written per logit of the walked rows
+            e["gbps"] = 4.0 * T * V * act * steps / (v["ms"] * 1e-3) / 1e9
+            e["frac_of_hbm_peak"] = e["gbps"] / float(peaks["hbm_gbs"])
         kernels[k] = e
     gemm_ms = sum(prof[k]["ms"] for k in GEMM_KINDS)
     dom = max(GEMM_KINDS, key=lambda k: prof[k]["ms"])
@@ -376,14 +408,17 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         "flops_per_launch": kind_flops[dom] / kernels[dom]["launches_per_step"],
         "all_gemms": {"achieved": path_tflops, "frac": path_tflops / peak, "share_of_step": gemm_ms / ms_total},
         "whole_step": None if step_tflops is None else {"achieved": step_tflops, "frac": step_tflops / peak,
-                                                        "flops_basis": "executed: 2*T*V*d (A2) + 3*2*T_walked*V*d (A4-A6); "
-                                                                       "= 8*T*V*d when no tile is skipped"},
+                                                        "flops_basis": "executed: 2*T*V*d (A2) + 2*T_walked*V*d per backward "
+                                                                       "contraction (3 recompute / 2 stash); 8*T*V*d for "
+                                                                       "the north_star path when no tile is skipped"},
     }
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config],
+                   "variant": "stash_logits (3 contractions, DESIGN.md section 11)" if args.stash
+                   else "recompute (north_star: 4 contractions)",
                    "tokens_per_step": int(tokens_all), "tokens_rank0": T, "d": d, "V": V, "G": b.G,
                    "parallelism": f"replicas x{world}: independent complete groups, no collective",
                    "l2": "inputs larger than L2 (W 622 MB, dW 1.2 GB, dZ chunk 2.9 GB vs 126 MB L2); no flush needed",
@@ -392,6 +427,7 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
             "value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "api": "grpo_step_host (C ABI, pinned host buffers; W and dW resident on the device)"},
         "bwd_tiles": getattr(args, "bwd_tiles", None),
+        "other_variant": getattr(args, "other_variant", None),
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
         "loss_after_steps": loss_val,
     }
@@ -408,6 +444,10 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5],
                     help="workload = workloads.synth.make_config index (2 = BASELINE configs[1], the headline; "
                          "3-5 are informational device-resident runs without the e2e / cpu_baseline legs)")
+    ap.add_argument("--stash", action="store_true",
+                    help="time grpo_fused_logprob_loss_fwd_bwd (3-contraction variant) as the step instead of the "
+                         "north_star forward + recomputing backward")
+    ap.add_argument("--no-variants", action="store_true", help="do not time the other variant beside the headline")
     ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")

@@ -81,6 +81,9 @@ typedef struct {
                                 kl_beta = 0, masked spans): their dHidden rows are written as zeros and they
                                 add nothing to dW, which is what the dense computation gives (DESIGN.md
                                 section 10).  Decided on the device; no host synchronisation. */
+  int32_t stash_logits;      /* 0 = default: grpo_enqueue_groups / grpo_step_host run forward then backward with
+                                the logits RECOMPUTED chunk by chunk (north_star, 4 contractions); 1 = they run
+                                grpo_fused_logprob_loss_fwd_bwd instead (3 contractions) */
 } grpo_config;
 
 /* Fill *cfg with the defaults above (d, V must still be set). */
@@ -129,6 +132,22 @@ int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden, const voi
                                     void* dhidden_out, float* dW_accum, void* stream);
 
 /* One COMPLETE group (all K responses present, rewards verified). */
+/* 3-contraction variant of forward + backward in ONE call.
+ * Per chunk of bwd_chunk_tokens tokens: the forward contraction (A2) also writes the chunk's scaled logits as
+ * fp16 into the workspace chunk buffer, A3 runs on the chunk, an HBM-bound pass turns the stashed logits into
+ * dZ in place, then A5 and A6 run as in the backward.  The [T, V] logits are still never materialised (one
+ * [Tc, V] chunk lives in the workspace) but nothing is recomputed: 6 T V d FLOPs instead of 8 T V d.
+ * Arguments and outputs are those of grpo_fused_logprob_loss_fwd followed by grpo_fused_logprob_loss_bwd
+ * (dhidden_out / dW_accum may each be NULL); results agree with that pair within the parity tolerances
+ * (the stashed logit is rounded to fp16, the recomputed one is not).  The denominator of the mean must be
+ * known before the first chunk: loss_denom > 0, or it is counted from mask / targets of this call first. */
+int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hidden, const void* W, const int32_t* targets,
+                                        const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv,
+                                        const float* old_logp, const float* ref_logp, const uint8_t* mask,
+                                        double loss_denom, float grad_scale, float* logp_out, float* lse_out,
+                                        float* coeff_out, float* loss_accum, float* metrics_accum, void* dhidden_out,
+                                        float* dW_accum, void* stream);
+
 typedef struct {
   int64_t group_order;          /* submission order; informational, FIFO is by arrival */
   int32_t G;                    /* responses in the group */
@@ -200,7 +219,8 @@ enum {
   GRPO_KERNEL_GEMM_DW = 6,     /* A6: dW += dZ^T H */
   GRPO_KERNEL_DEBUG = 7,       /* grpo_debug_gemm */
   GRPO_KERNEL_TILE_SCAN = 8,   /* backward: zero-coefficient tile scan + zero fill of skipped dHidden rows */
-  GRPO_NUM_KERNEL_KINDS = 9
+  GRPO_KERNEL_STASH_DZ = 9,    /* 3-contraction variant: stashed logits -> dZ in place */
+  GRPO_NUM_KERNEL_KINDS = 10
 };
 
 /* Token tiles the backward calls of workspace slot 0 walked (active) and saw (total) since the last call

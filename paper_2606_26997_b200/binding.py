@@ -20,11 +20,12 @@ STATUS_NAMES = {0: "GRPO_OK", 1: "GRPO_ERR_INVALID_ARG", 2: "GRPO_ERR_SHAPE", 3:
 EXPORTS = [
     "grpo_default_config", "grpo_create", "grpo_destroy", "grpo_last_error", "grpo_workspace_bytes",
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
+    "grpo_fused_logprob_loss_fwd_bwd",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
     "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
 ]
-KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan"]
+KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan", "stash_dz"]
 
 
 class GrpoError(RuntimeError):
@@ -40,7 +41,7 @@ class GrpoConfig(C.Structure):
                 ("groups_per_update", C.c_int32), ("groups_per_round", C.c_int32), ("token_budget", C.c_int64),
                 ("bwd_chunk_tokens", C.c_int64), ("max_pending_groups", C.c_int32), ("gemm_cta_group", C.c_int32),
                 ("gemm_drift_epoch_kb", C.c_int32), ("kl_type", C.c_int32), ("dual_clip", C.c_float),
-                ("bwd_skip_zero_tiles", C.c_int32)]
+                ("bwd_skip_zero_tiles", C.c_int32), ("stash_logits", C.c_int32)]
 
 
 class GroupDesc(C.Structure):
@@ -76,6 +77,8 @@ def load_library() -> C.CDLL:
     lib.grpo_fused_logprob_loss_fwd.argtypes = [vp, vp, vp, vp, vp, i32, i64, vp, vp, vp, vp, f64, vp, vp, vp, vp,
                                                 vp, vp]
     lib.grpo_fused_logprob_loss_bwd.argtypes = [vp, vp, vp, vp, vp, vp, i64, f32, vp, vp, vp]
+    lib.grpo_fused_logprob_loss_fwd_bwd.argtypes = [vp, vp, vp, vp, vp, i32, i64, vp, vp, vp, vp, f64, f32, vp, vp, vp,
+                                                    vp, vp, vp, vp, vp]
     lib.grpo_enqueue_groups.argtypes = [vp, C.POINTER(GroupDesc), i32, vp, vp, vp, vp, f64, C.POINTER(vp), i32,
                                         C.POINTER(i32), C.POINTER(i32)]
     lib.grpo_flush.argtypes = [vp, vp, vp, vp, vp, f64, C.POINTER(vp), i32, C.POINTER(i32), C.POINTER(i32)]
@@ -235,6 +238,35 @@ class GrpoContext:
             _dev(coeff, torch.float32, "coeff", T), T, float(grad_scale), dh_ptr,
             _dev(dW_accum, torch.float32, "dW_accum", self.cfg.V * self.cfg.d), _stream(stream)))
         return dhidden_out
+
+    # ------------------------------------------------------------------ A2 - A6 in one call (3-contraction variant)
+    def grpo_fused_logprob_loss_fwd_bwd(self, hidden, W, targets, cu_seqlens, adv, old_logp, ref_logp=None, mask=None,
+                                        loss_denom: float = 0.0, grad_scale: float = 1.0, loss_accum=None,
+                                        metrics_accum=None, dW_accum=None, want_dhidden: bool = True,
+                                        dhidden_out=None, stream=None):
+        T, d = hidden.shape
+        S = cu_seqlens.numel() - 1
+        self.ensure_workspace(T, 1)
+        dev = hidden.device
+        logp = torch.empty(T, dtype=torch.float32, device=dev)
+        lse = torch.empty(T, dtype=torch.float32, device=dev)
+        coeff = torch.empty(T, dtype=torch.float32, device=dev)
+        if loss_accum is None:
+            loss_accum = torch.zeros(1, dtype=torch.float32, device=dev)
+        if want_dhidden and dhidden_out is None:
+            dhidden_out = torch.empty(T, d, dtype=torch.float32 if self.cfg.dhidden_fp32 else torch.bfloat16,
+                                      device=dev)
+        dh_ptr = None if dhidden_out is None else C.c_void_p(dhidden_out.data_ptr())
+        _check(self.lib.grpo_fused_logprob_loss_fwd_bwd(
+            self.h, _dev(hidden, torch.bfloat16, "hidden", T * self.cfg.d), _dev(W, torch.bfloat16, "W", self.cfg.V * self.cfg.d),
+            _dev(targets, torch.int32, "targets", T), _dev(cu_seqlens, torch.int32, "cu_seqlens"), S, T,
+            _dev(adv, torch.float32, "adv", S), _dev(old_logp, torch.float32, "old_logp", T),
+            _dev(ref_logp, torch.float32, "ref_logp", T), _dev(mask, torch.uint8, "mask", T), float(loss_denom),
+            float(grad_scale), _dev(logp, torch.float32, "logp"), _dev(lse, torch.float32, "lse"),
+            _dev(coeff, torch.float32, "coeff"), _dev(loss_accum, torch.float32, "loss_accum"),
+            _dev(metrics_accum, torch.float32, "metrics_accum"), dh_ptr,
+            _dev(dW_accum, torch.float32, "dW_accum", self.cfg.V * self.cfg.d), _stream(stream)))
+        return dict(logp=logp, lse=lse, coeff=coeff, loss=loss_accum, dH=dhidden_out)
 
     # ------------------------------------------------------------------ A0 / A7
     def make_group_desc(self, order: int, seqlens, hidden, targets, old_logp, rewards, ref_logp=None, mask=None,

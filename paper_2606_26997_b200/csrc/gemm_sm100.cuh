@@ -44,7 +44,10 @@ template <int CG> struct GemmShape {
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
-enum Epi : int { EPI_LSE = 0, EPI_DZ = 1, EPI_STORE = 2, EPI_RED_F32 = 3 };
+enum Epi : int { EPI_LSE = 0, EPI_DZ = 1, EPI_STORE = 2, EPI_RED_F32 = 3, EPI_LSE_STASH = 4 };
+// EPI_LSE_STASH (3-contraction variant): EPI_LSE that also writes the scaled logits
+// z s log2(e) as fp16 into the chunk buffer `dz`, which stash_to_dz_kernel later turns into dZ in place.
+__host__ __device__ constexpr bool is_lse(int epi) { return epi == EPI_LSE || epi == EPI_LSE_STASH; }
 
 struct GemmParams {
   int m_total, n_total;              // valid rows / cols of C
@@ -99,7 +102,7 @@ struct Extent { int m_tiles, k_blocks, n_units; };
 template <int CG, int EPI>
 __device__ __forceinline__ Extent launch_extent(const GemmParams& p, int n_units) {
   Extent e{p.m_tiles, p.k_blocks, n_units};
-  if (p.tile_list != nullptr) {
+  if (p.tile_list != nullptr && !is_lse(EPI)) {
     const int n_active = p.tile_list[0];
     if constexpr (EPI == EPI_RED_F32) {
       e.k_blocks = min(p.k_blocks, n_active * (BM * CG / BK));
@@ -121,7 +124,7 @@ __device__ __forceinline__ int walked_k_block(const GemmParams& p, int kb) {
 template <int EPI>
 __device__ __forceinline__ void unit_to_tiles(const GemmParams& p, const Extent& e, int u, int& m_tile, int& n0,
                                               int& n1) {
-  if constexpr (EPI == EPI_LSE) {
+  if constexpr (is_lse(EPI)) {
     m_tile = u % p.m_tiles;
     int split = u / p.m_tiles;
     n0 = split * p.tiles_per_split;
@@ -343,7 +346,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       [[maybe_unused]] int y = -1;
       [[maybe_unused]] float run_m = -INFINITY, run_s = 0.f;     // EPI_LSE running stats (log2 domain)
       [[maybe_unused]] float lse2 = 0.f, kcoef = 0.f;            // EPI_DZ per-row constants
-      if constexpr (EPI == EPI_LSE || EPI == EPI_DZ) {
+      if constexpr (is_lse(EPI) || EPI == EPI_DZ) {
         if (row_ok) {
           y = p.targets[row_g];
           if (y >= p.n_total) y = -1;
@@ -370,7 +373,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           tmem_ld_wait();
           const int nvalid = p.n_total - cbase;                   // >= 1; columns >= nvalid are padding
 
-          if constexpr (EPI == EPI_LSE) {
+          if constexpr (is_lse(EPI)) {
             float cmax = -INFINITY;
             if (nvalid >= 32) {
 #pragma unroll
@@ -380,6 +383,15 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               for (int i = 0; i < 32; ++i) {
                 v[i] = i < nvalid ? v[i] * p.scale_log2e : -INFINITY;
                 cmax = fmaxf(cmax, v[i]);
+              }
+            }
+            if constexpr (EPI == EPI_LSE_STASH) {
+              if (row_ok) {   // scaled logits (log2 domain) as fp16; padding columns hold -inf
+                __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
+#pragma unroll
+                for (int g = 0; g < 4; ++g)
+                  st_global_v4(dst + g * 8, pack_f16x2(v[g * 8 + 0], v[g * 8 + 1]), pack_f16x2(v[g * 8 + 2], v[g * 8 + 3]),
+                               pack_f16x2(v[g * 8 + 4], v[g * 8 + 5]), pack_f16x2(v[g * 8 + 6], v[g * 8 + 7]));
               }
             }
             const float new_m = fmaxf(run_m, cmax);
@@ -403,13 +415,13 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll
               for (int i = 0; i < 32; ++i) dzv[i] = (y - cbase == i) ? dzv[i] + kcoef : dzv[i];
             }
+            uint32_t pk[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) pk[j] = pack_bf16x2(dzv[2 * j], dzv[2 * j + 1]);
             if (row_ok) {
               __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
 #pragma unroll
-              for (int g = 0; g < 4; ++g)
-                st_global_v4(dst + g * 8, pack_bf16x2(dzv[g * 8 + 0], dzv[g * 8 + 1]),
-                             pack_bf16x2(dzv[g * 8 + 2], dzv[g * 8 + 3]), pack_bf16x2(dzv[g * 8 + 4], dzv[g * 8 + 5]),
-                             pack_bf16x2(dzv[g * 8 + 6], dzv[g * 8 + 7]));
+              for (int g = 0; g < 4; ++g) st_global_v4(dst + g * 8, pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
             }
           } else if constexpr (EPI == EPI_STORE) {
             if (row_ok) {
@@ -451,11 +463,11 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         if (acc == 0) acc_phase ^= 1;
       }
 
-      if constexpr (EPI == EPI_LSE) {
+      if constexpr (is_lse(EPI)) {
         if (row_ok) {
           const int split = u / p.m_tiles;
-          p.part_m[split * p.part_stride + row_g] = run_m;
-          p.part_s[split * p.part_stride + row_g] = run_s;
+          p.part_m[split * p.part_stride + row_local] = run_m;     // partials are indexed by the launch's own rows
+          p.part_s[split * p.part_stride + row_local] = run_s;
         }
       }
     }

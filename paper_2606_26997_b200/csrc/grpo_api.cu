@@ -206,7 +206,7 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   const int xsync = ctx->cfg.gemm_drift_epoch_kb == 0 ? 32 : ctx->cfg.gemm_drift_epoch_kb;
   if (pl.sync != nullptr && xsync > 0 && grid / CG > 1) {
     const int64_t n_pairs = grid / CG;
-    const int64_t kb_unit = static_cast<int64_t>(p.k_blocks) * (EPI == EPI_LSE ? p.tiles_per_split : 1);
+    const int64_t kb_unit = static_cast<int64_t>(p.k_blocks) * (is_lse(EPI) ? p.tiles_per_split : 1);
     const int64_t max_kb = (n_units + n_pairs - 1) / n_pairs * kb_unit;
     int64_t E = xsync;
     while ((max_kb + E - 1) / E + 1 > kSyncCap) E *= 2;
@@ -417,78 +417,114 @@ extern "C" int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, con
 }
 
 // ------------------------------------------------------------------------------------- A2 + A3
-static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
-                        const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv, const float* old_logp,
-                        const float* ref_logp, const uint8_t* mask, double loss_denom, const float* denom_dev,
-                        float* logp_out, float* lse_out, float* coeff_out, float* loss_accum, float* metrics_accum,
-                        cudaStream_t st) {
-  const grpo_config& c = ctx->cfg;
+// Per-token inputs / outputs of the forward, all indexed by the packed row of the whole call.
+struct FwdArgs {
+  const int32_t* cu_seqlens; int32_t S;
+  const float* adv; const float* old_logp; const float* ref_logp; const uint8_t* mask;
+  double loss_denom; const float* denom_dev;
+  float* logp_out; float* lse_out; float* coeff_out; float* loss_accum; float* metrics_accum;
+};
+
+static int32_t fwd_check(grpo_ctx* ctx, int32_t S, int64_t T) {
   if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
   if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
   if (S > ctx->lay.s_max) return fail(GRPO_ERR_WORKSPACE, "S=%d exceeds workspace capacity", S);
   if (T > INT32_MAX - 256) return fail(GRPO_ERR_SHAPE, "T too large");
+  return GRPO_OK;
+}
+
+// Loss-bearing token counts that define the mean (whole call, before any row is processed).
+static int32_t fwd_counts(grpo_ctx* ctx, int slot, const int32_t* targets, const FwdArgs& a, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  const SlotLayout& L = ctx->lay;
+  float* total = slot_ptr<float>(ctx, slot, L.off_total);
+  float* seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
+  const bool implicit_denom = c.loss_agg == 0 && !(a.loss_denom > 0.0) && a.denom_dev == nullptr;
+  if (c.loss_agg == 1 || implicit_denom) {
+    CU_OK(cudaMemsetAsync(total, 0, 4, st));
+    const int threads = 128;
+    const int blocks = (a.S * 32 + threads - 1) / threads;
+    {
+      LaunchScope ls(ctx, GRPO_KERNEL_TOKEN_COUNT, st);
+      token_count_kernel<<<blocks, threads, 0, st>>>(a.mask, targets, c.V, a.cu_seqlens, a.S, seq_count, total);
+    }
+    CU_OK(cudaGetLastError());
+  }
+  return GRPO_OK;
+}
+
+// A2 + A3 over packed rows [t0, t0 + rows) of a call of T tokens.  stash != nullptr: the 3-contraction
+// variant's forward, which also writes the chunk's scaled logits (fp16) to `stash`.
+static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
+                        const FwdArgs& a, int64_t T, int64_t t0, int64_t rows, __nv_bfloat16* stash, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
   const SlotLayout& L = ctx->lay;
   float* part_m = slot_ptr<float>(ctx, slot, L.off_part_m);
   float* part_s = slot_ptr<float>(ctx, slot, L.off_part_s);
   float* zy = slot_ptr<float>(ctx, slot, L.off_zy);
-  float* total = slot_ptr<float>(ctx, slot, L.off_total);
-  float* seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
-
-  const bool implicit_denom = c.loss_agg == 0 && !(loss_denom > 0.0) && denom_dev == nullptr;
-  if (c.loss_agg == 1 || implicit_denom) {
-    CU_OK(cudaMemsetAsync(total, 0, 4, st));
-    const int threads = 128;
-    const int blocks = (S * 32 + threads - 1) / threads;
-    {
-      LaunchScope ls(ctx, GRPO_KERNEL_TOKEN_COUNT, st);
-      token_count_kernel<<<blocks, threads, 0, st>>>(mask, targets, c.V, cu_seqlens, S, seq_count, total);
-    }
-    CU_OK(cudaGetLastError());
-  }
 
   CUtensorMap tmH, tmW;
-  GRPO_TRY(make_tmap(ctx, &tmH, hidden, c.d, T, static_cast<uint64_t>(c.d) * 2, BK, BM));
+  const void* Hc = static_cast<const uint8_t*>(hidden) + t0 * c.d * 2;
+  GRPO_TRY(make_tmap(ctx, &tmH, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
   const int TM = BM * ctx->cg;                      // rows of C per scheduling unit (CTA or CTA pair)
   GRPO_TRY(make_tmap(ctx, &tmW, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN / ctx->cg));
   GemmParams p;
   std::memset(&p, 0, sizeof(p));
   set_desc_defaults(p, false, false);
-  p.m_total = static_cast<int>(T);
+  p.m_total = static_cast<int>(rows);
   p.n_total = c.V;
-  p.m_tiles = static_cast<int>((T + TM - 1) / TM);
+  p.m_tiles = static_cast<int>((rows + TM - 1) / TM);
   p.n_tiles = (c.V + BN - 1) / BN;
   p.k_blocks = (c.d + BK - 1) / BK;
-  p.n_split = choose_n_split(p.m_tiles, p.n_tiles, ctx->num_sms / ctx->cg, std::max<int64_t>(1, L.part_cap / T));
+  p.n_split = choose_n_split(p.m_tiles, p.n_tiles, ctx->num_sms / ctx->cg, std::max<int64_t>(1, L.part_cap / rows));
   p.tiles_per_split = (p.n_tiles + p.n_split - 1) / p.n_split;
+  p.row_offset = t0;
   p.targets = targets;
   p.scale_log2e = c.logit_scale * kLog2e;
   p.logit_scale = c.logit_scale;
   p.part_m = part_m;
   p.part_s = part_s;
-  p.part_stride = T;
+  p.part_stride = rows;
   p.zy = zy;
+  p.dz = stash; p.dz_pitch = L.v_pad;
   p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
-  GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
+  if (stash)
+    GRPO_TRY((launch_gemm<false, false, EPI_LSE_STASH>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
+  else
+    GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
 
   LossParams lp;
   std::memset(&lp, 0, sizeof(lp));
-  lp.T = T; lp.S = S; lp.V = c.V; lp.n_split = p.n_split; lp.part_stride = T;
-  lp.part_m = part_m; lp.part_s = part_s; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = cu_seqlens;
-  lp.adv = adv; lp.old_logp = old_logp; lp.ref_logp = ref_logp; lp.mask = mask;
-  lp.seq_count = seq_count; lp.total_count = denom_dev ? denom_dev : total;
-  lp.denom_host = loss_denom > 0.0 ? static_cast<float>(loss_denom) : 0.f;
+  lp.T = rows; lp.t_begin = t0; lp.S = a.S; lp.V = c.V; lp.n_split = p.n_split; lp.part_stride = rows;
+  lp.part_m = part_m; lp.part_s = part_s; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = a.cu_seqlens;
+  lp.adv = a.adv; lp.old_logp = a.old_logp; lp.ref_logp = a.ref_logp; lp.mask = a.mask;
+  lp.seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
+  lp.total_count = a.denom_dev ? a.denom_dev : slot_ptr<float>(ctx, slot, L.off_total);
+  lp.denom_host = a.loss_denom > 0.0 ? static_cast<float>(a.loss_denom) : 0.f;
   lp.loss_agg = c.loss_agg; lp.clip_lo = c.clip_lo; lp.clip_hi = c.clip_hi; lp.kl_beta = c.kl_beta;
   lp.kl_type = c.kl_type; lp.dual_clip = c.dual_clip;
-  lp.logp = logp_out; lp.lse = lse_out; lp.coeff = coeff_out; lp.loss_accum = loss_accum;
-  lp.metrics_accum = metrics_accum; lp.err_flag = ctx->err_dev;
+  lp.logp = a.logp_out; lp.lse = a.lse_out; lp.coeff = a.coeff_out; lp.loss_accum = a.loss_accum;
+  lp.metrics_accum = a.metrics_accum; lp.err_flag = ctx->err_dev;
   const int threads = 256;
-  const int blocks = static_cast<int>((T + threads - 1) / threads);
+  const int blocks = static_cast<int>((rows + threads - 1) / threads);
   {
     LaunchScope ls(ctx, GRPO_KERNEL_LOSS, st);
     loss_epilogue_kernel<<<blocks, threads, 0, st>>>(lp);
   }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
+}
+
+static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
+                        const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv, const float* old_logp,
+                        const float* ref_logp, const uint8_t* mask, double loss_denom, const float* denom_dev,
+                        float* logp_out, float* lse_out, float* coeff_out, float* loss_accum, float* metrics_accum,
+                        cudaStream_t st) {
+  GRPO_TRY(fwd_check(ctx, S, T));
+  const FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
+                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
+  return fwd_rows(ctx, slot, hidden, W, targets, a, T, 0, T, nullptr, st);
 }
 
 extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const void* W,
@@ -506,13 +542,16 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden
 }
 
 // ------------------------------------------------------------------------------------- A4 - A6
+// fused == nullptr: the backward of north_star (A4 recomputes the logits).  fused != nullptr: the
+// 3-contraction variant: per chunk, the forward runs first and stashes the chunk's
+// logits, which are then converted to dZ in place instead of being recomputed; lse / coeff are fused's.
 static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
                         const float* lse, const float* coeff, int64_t T, float grad_scale, void* dhidden_out,
-                        float* dW_accum, cudaStream_t st) {
+                        float* dW_accum, cudaStream_t st, const FwdArgs* fused = nullptr) {
   const grpo_config& c = ctx->cfg;
   if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
   if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
-  if (!dhidden_out && !dW_accum) return GRPO_OK;
+  if (!dhidden_out && !dW_accum && !fused) return GRPO_OK;
   const SlotLayout& L = ctx->lay;
   __nv_bfloat16* dz = slot_ptr<__nv_bfloat16>(ctx, slot, L.off_dz);
   const int64_t Tc = L.chunk_rows;
@@ -535,6 +574,8 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
     GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
 
+    if (fused) GRPO_TRY(fwd_rows(ctx, slot, hidden, W, targets, *fused, T, t0, rows, dz, st));
+    if (!dhidden_out && !dW_accum) continue;
     // zero-coefficient tile skipping: scan this chunk's coefficients on the device
     const int* tile_list = nullptr;
     if (c.bwd_skip_zero_tiles >= 0) {
@@ -554,7 +595,13 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       }
       tile_list = list;
     }
-    {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
+    if (fused) {  // stashed logits -> dZ in place (HBM-bound elementwise pass instead of the A4 contraction)
+      LaunchScope ls(ctx, GRPO_KERNEL_STASH_DZ, st);
+      stash_to_dz_kernel<<<static_cast<unsigned>(rows), 256, 0, st>>>(
+          reinterpret_cast<uint16_t*>(dz), static_cast<int>(rows), c.V, L.v_pad, targets + t0, lse + t0, coeff + t0,
+          c.logit_scale * grad_scale, tile_list, TM);
+      CU_OK(cudaGetLastError());
+    } else {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
       set_desc_defaults(p, false, false);
@@ -606,6 +653,25 @@ extern "C" int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden
   if (T <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0");
   return bwd_impl(ctx, 0, hidden, W, targets, lse, coeff, T, grad_scale, dhidden_out, dW_accum,
                   static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hidden, const void* W,
+                                                   const int32_t* targets, const int32_t* cu_seqlens, int32_t S,
+                                                   int64_t T, const float* adv, const float* old_logp,
+                                                   const float* ref_logp, const uint8_t* mask, double loss_denom,
+                                                   float grad_scale, float* logp_out, float* lse_out, float* coeff_out,
+                                                   float* loss_accum, float* metrics_accum, void* dhidden_out,
+                                                   float* dW_accum, void* stream) {
+  if (!ctx || !hidden || !W || !targets || !cu_seqlens || !adv || !old_logp || !logp_out || !lse_out || !coeff_out ||
+      !loss_accum)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0 and S > 0 (got T=%lld S=%d)", (long long)T, S);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  GRPO_TRY(fwd_check(ctx, S, T));
+  const FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
+                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  GRPO_TRY(fwd_counts(ctx, 0, targets, a, st));
+  return bwd_impl(ctx, 0, hidden, W, targets, lse_out, coeff_out, T, grad_scale, dhidden_out, dW_accum, st, &a);
 }
 
 // ------------------------------------------------------------------------------------- A0 / A7: CGP FIFO
@@ -749,11 +815,19 @@ static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, cons
   float* logp = (k == 1 && groups[0].desc.logp_out) ? groups[0].desc.logp_out : slot_ptr<float>(ctx, slot, L.off_logp);
   float* lse = slot_ptr<float>(ctx, slot, L.off_lse);
   float* coeff = slot_ptr<float>(ctx, slot, L.off_coeff);
-  GRPO_TRY(fwd_impl(ctx, slot, hidden, W, targets, d_cu_seq, S, T, d_adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
-                    logp, lse, coeff, loss_accum, metrics_accum, st));
   void* dh = nullptr;
   if (any_dh) dh = (k == 1) ? groups[0].desc.dhidden_out : static_cast<void*>(slot_ptr<uint8_t>(ctx, slot, L.off_dh));
-  GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st));
+  if (c.stash_logits) {
+    GRPO_TRY(fwd_check(ctx, S, T));
+    const FwdArgs a{d_cu_seq, S, d_adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
+                    logp, lse, coeff, loss_accum, metrics_accum};
+    GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
+    GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st, &a));
+  } else {
+    GRPO_TRY(fwd_impl(ctx, slot, hidden, W, targets, d_cu_seq, S, T, d_adv, old_logp, ref_logp, mask, loss_denom,
+                      denom_dev, logp, lse, coeff, loss_accum, metrics_accum, st));
+    GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st));
+  }
   if (k > 1) {
     int64_t off = 0;
     for (int i = 0; i < k; ++i) {
@@ -893,9 +967,17 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   CU_OK(cudaMemcpyAsync(d_rw, rewards_host, S * 4, cudaMemcpyHostToDevice, st));
   CU_OK(cudaMemsetAsync(loss_dev, 0, 4, st));
   GRPO_TRY(grpo_group_advantage(ctx, d_rw, nullptr, n_groups, G, d_adv, nullptr, st));
-  GRPO_TRY(fwd_impl(ctx, 0, sh, W, stg, d_cu, S, T, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr,
-                    loss_denom, nullptr, logp, lse, coeff, loss_dev, nullptr, st));
-  GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st));
+  if (c.stash_logits) {
+    GRPO_TRY(fwd_check(ctx, S, T));
+    const FwdArgs a{d_cu, S, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr, loss_denom, nullptr,
+                    logp, lse, coeff, loss_dev, nullptr};
+    GRPO_TRY(fwd_counts(ctx, 0, stg, a, st));
+    GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, &a));
+  } else {
+    GRPO_TRY(fwd_impl(ctx, 0, sh, W, stg, d_cu, S, T, d_adv, so, ref_logp_host ? sr : nullptr,
+                      mask_host ? sm : nullptr, loss_denom, nullptr, logp, lse, coeff, loss_dev, nullptr, st));
+    GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st));
+  }
   CU_OK(cudaMemcpyAsync(loss_host, loss_dev, 4, cudaMemcpyDeviceToHost, st));
   if (logp_host) CU_OK(cudaMemcpyAsync(logp_host, logp, T * 4, cudaMemcpyDeviceToHost, st));
   if (dhidden_host) CU_OK(cudaMemcpyAsync(dhidden_host, dh, T * c.d * dh_elem, cudaMemcpyDeviceToHost, st));

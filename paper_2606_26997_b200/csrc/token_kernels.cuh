@@ -1,6 +1,8 @@
 // HBM-bound per-group / per-token kernels of the GRPO step: A1 (group advantage), the mask counts that
 // define the mean, and A3 (partial-LSE combine + clipped surrogate + k3 + coefficient for the backward).
 #pragma once
+#include <cuda_fp16.h>
+
 #include "ptx_sm100.cuh"
 
 namespace grpo {
@@ -79,7 +81,8 @@ __global__ void token_count_kernel(const uint8_t* __restrict__ mask, const int32
 }
 
 struct LossParams {
-  int64_t T;
+  int64_t T;                 // tokens handled by this launch: packed rows [t_begin, t_begin + T)
+  int64_t t_begin;
   int S, V;
   int n_split;
   int64_t part_stride;
@@ -109,15 +112,16 @@ struct LossParams {
 
 // A3.  One thread per packed token; block-level reduction, then one atomic per block and quantity.
 __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) {
-  const int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const int64_t t = p.t_begin + static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   float loss_t = 0.f, m_cnt = 0.f, m_rho = 0.f, m_k3 = 0.f, m_clip = 0.f;
-  if (t < p.T) {
+  if (t < p.t_begin + p.T) {
     // combine the per-split (max, sum 2^(z2 - max)) pairs -> natural-log lse
+    const int64_t tl = t - p.t_begin;                 // the A2 launch's own row
     float M = -INFINITY;
-    for (int i = 0; i < p.n_split; ++i) M = fmaxf(M, p.part_m[i * p.part_stride + t]);
+    for (int i = 0; i < p.n_split; ++i) M = fmaxf(M, p.part_m[i * p.part_stride + tl]);
     float sum = 0.f;
     for (int i = 0; i < p.n_split; ++i)
-      sum += p.part_s[i * p.part_stride + t] * exp2f(p.part_m[i * p.part_stride + t] - M);
+      sum += p.part_s[i * p.part_stride + tl] * exp2f(p.part_m[i * p.part_stride + tl] - M);
     const float lse = (M + log2f(sum)) * kLn2;
     const int y = p.targets[t];
     const bool valid = y >= 0 && y < p.V;
@@ -220,6 +224,46 @@ __global__ void __launch_bounds__(1024) active_tiles_kernel(const float* __restr
     list[0] = n;
     list[1] = n_tiles;
     if (stats) { atomicAdd(stats, n); atomicAdd(stats + 1, n_tiles); }
+  }
+}
+
+// 3-contraction variant: turn the stashed scaled logits z2 = z s log2(e) (fp16, written
+// by the EPI_LSE_STASH epilogue) into dZ = k_t (1[v = y_t] - 2^(z2 - lse2_t)) (bf16) in place; k_t = coeff_t *
+// coeff_mul.  HBM-bound: 2 B read + 2 B written per logit.  One block per walked row; 16-byte accesses.
+__global__ void __launch_bounds__(256) stash_to_dz_kernel(uint16_t* __restrict__ buf, int rows, int V, int64_t pitch,
+                                                          const int32_t* __restrict__ targets,
+                                                          const float* __restrict__ lse, const float* __restrict__ coeff,
+                                                          float coeff_mul, const int* __restrict__ tile_list,
+                                                          int tile_rows) {
+  int row = blockIdx.x;
+  if (tile_list != nullptr) {
+    const int w = row / tile_rows;
+    if (w >= tile_list[0]) return;
+    row = tile_list[2 + w] * tile_rows + row % tile_rows;
+  }
+  if (row >= rows) return;
+  const float lse2 = lse[row] * kLog2e;
+  const float k = coeff[row] * coeff_mul;
+  int y = targets[row];
+  if (y >= V) y = -1;
+  uint4* line = reinterpret_cast<uint4*>(buf + static_cast<int64_t>(row) * pitch);
+  const int n_vec = (V + 7) / 8;
+  for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
+    const uint4 in = line[i];
+    const uint32_t w4[4] = {in.x, in.y, in.z, in.w};
+    float dz[8];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w4[j]));
+      dz[2 * j] = -k * ex2_approx(f.x - lse2);
+      dz[2 * j + 1] = -k * ex2_approx(f.y - lse2);
+    }
+    if (static_cast<uint32_t>(y - i * 8) < 8u) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) dz[j] = (y - i * 8 == j) ? dz[j] + k : dz[j];
+    }
+    line[i] = make_uint4(pack_bf16x2(dz[0], dz[1]), pack_bf16x2(dz[2], dz[3]), pack_bf16x2(dz[4], dz[5]),
+                         pack_bf16x2(dz[6], dz[7]));
   }
 }
 

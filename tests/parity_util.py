@@ -32,15 +32,23 @@ def make_ctx(b, **kw):
     return GrpoContext(b.d, b.V, **args)
 
 
-def run_cuda(ctx, b, loss_denom=0.0, want_dw=True, want_dh=True, grad_scale=1.0):
+def run_cuda(ctx, b, loss_denom=0.0, want_dw=True, want_dh=True, grad_scale=1.0, fused=False):
+    """fused=False: grpo_fused_logprob_loss_fwd then _bwd (north_star: logits recomputed in the backward);
+    fused=True: grpo_fused_logprob_loss_fwd_bwd (3-contraction variant, logits stashed per chunk)."""
     dev = b.hidden.device
     adv, zv = ctx.grpo_group_advantage(b.rewards, G=b.G, want_zero_var=True)
     metrics = torch.zeros(4, dtype=torch.float32, device=dev)
-    f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
-                                        b.mask, loss_denom=loss_denom, metrics_accum=metrics)
     dW = torch.zeros(b.V, b.d, dtype=torch.float32, device=dev) if want_dw else None
-    dH = ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW,
-                                         grad_scale=grad_scale, want_dhidden=want_dh)
+    if fused:
+        f = ctx.grpo_fused_logprob_loss_fwd_bwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                                b.mask, loss_denom=loss_denom, grad_scale=grad_scale,
+                                                metrics_accum=metrics, dW_accum=dW, want_dhidden=want_dh)
+        dH = f.pop("dH")
+    else:
+        f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                            b.mask, loss_denom=loss_denom, metrics_accum=metrics)
+        dH = ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW,
+                                             grad_scale=grad_scale, want_dhidden=want_dh)
     torch.cuda.synchronize()
     return dict(adv=adv, zero_var=zv, metrics=metrics, dW=dW, dH=dH, **f)
 
