@@ -85,6 +85,7 @@ struct GemmParams {
   unsigned int* sync;
   int sync_epoch_kb;                 // k blocks per epoch
   int sync_epochs;                   // counters in `sync` (epochs any pair can reach)
+  int sync_lag;                      // a pair may run this many epochs ahead of the slowest pair (>= 1)
 };
 
 struct alignas(8) GemmBarriers {
@@ -228,9 +229,10 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             if (sync_on && cta_rank == 0 && --to_epoch == 0) {
               to_epoch = p.sync_epoch_kb;
               red_add_u32(p.sync + epoch, 1u);
-              if (ld_volatile_shared_i32(&bars->gate_open) < epoch) {
+              const int need = epoch - (p.sync_lag - 1);         // every pair has arrived on epoch need - 1
+              if (ld_volatile_shared_i32(&bars->gate_open) < need) {
                 const long long t0 = clock64();
-                while (ld_volatile_shared_i32(&bars->gate_open) < epoch)
+                while (ld_volatile_shared_i32(&bars->gate_open) < need)
                   if (clock64() - t0 > 2 * kGateMaxTimeouts * kGateTimeoutClk) { sync_on = false; break; }
               }
               ++epoch;

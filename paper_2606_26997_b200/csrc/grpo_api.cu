@@ -204,6 +204,7 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   GemmParams pl = p;
   // drift gate (gemm_sm100.cuh): epoch counters live in the launch's workspace slot, zeroed on the stream
   const int xsync = ctx->cfg.gemm_drift_epoch_kb == 0 ? 32 : ctx->cfg.gemm_drift_epoch_kb;
+  pl.sync_lag = 1;   // epochs a pair may lead the slowest pair by (2-8 measured: no different from 1)
   if (pl.sync != nullptr && xsync > 0 && grid / CG > 1) {
     const int64_t n_pairs = grid / CG;
     const int64_t kb_unit = static_cast<int64_t>(p.k_blocks) * (is_lse(EPI) ? p.tiles_per_split : 1);
