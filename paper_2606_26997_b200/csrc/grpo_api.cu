@@ -77,6 +77,7 @@ struct grpo_ctx {
   float* denom_ring = nullptr;   // device scalars for implicit per-update denominators
   int denom_next = 0;
   cudaEvent_t denom_event = nullptr;
+  cudaStream_t copy_stream = nullptr;   // grpo_step_host: H2D / D2H overlapped with the compute stream
   uint8_t* ws = nullptr;
   int64_t ws_max_T = 0;
   int n_slots = 0;
@@ -309,7 +310,8 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
   }
   ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
   if (cudaMalloc(&ctx->err_dev, 256) != cudaSuccess || cudaMalloc(&ctx->denom_ring, kDenomRing * 4) != cudaSuccess ||
-      cudaEventCreateWithFlags(&ctx->denom_event, cudaEventDisableTiming) != cudaSuccess) {
+      cudaEventCreateWithFlags(&ctx->denom_event, cudaEventDisableTiming) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
     delete ctx;
     return fail(GRPO_ERR_CUDA, "context allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
   }
@@ -324,6 +326,7 @@ extern "C" int32_t grpo_destroy(grpo_ctx* ctx) {
   cudaFree(ctx->denom_ring);
   prof_clear(ctx);
   if (ctx->denom_event) cudaEventDestroy(ctx->denom_event);
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   delete ctx;
   return GRPO_OK;
 }
@@ -543,22 +546,38 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden
 }
 
 // ------------------------------------------------------------------------------------- A4 - A6
+// Token rows per backward chunk: whole pair tiles, equalised so that the last chunk is not a sliver.
+static int64_t rows_per_chunk_for(const grpo_ctx* ctx, int64_t T) {
+  const int64_t Tc = ctx->lay.chunk_rows;
+  const int64_t n_chunks = (T + Tc - 1) / Tc;
+  return std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, BM * ctx->cg));
+}
+
+// grpo_step_host's copy pipeline: chunk i of the hidden states arrives on the copy stream (in[i]), and the
+// dHidden rows of chunk i leave on it as soon as A5 has written them, under the next chunk's contractions.
+struct HostPipe {
+  cudaStream_t cs;
+  std::vector<cudaEvent_t> in, out;
+  uint8_t* dh_host;
+  ~HostPipe() {
+    for (auto e : in) if (e) cudaEventDestroy(e);
+    for (auto e : out) if (e) cudaEventDestroy(e);
+  }
+};
+
 // fused == nullptr: the backward of north_star (A4 recomputes the logits).  fused != nullptr: the
 // 3-contraction variant: per chunk, the forward runs first and stashes the chunk's
 // logits, which are then converted to dZ in place instead of being recomputed; lse / coeff are fused's.
 static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
                         const float* lse, const float* coeff, int64_t T, float grad_scale, void* dhidden_out,
-                        float* dW_accum, cudaStream_t st, const FwdArgs* fused = nullptr) {
+                        float* dW_accum, cudaStream_t st, const FwdArgs* fused = nullptr, HostPipe* pipe = nullptr) {
   const grpo_config& c = ctx->cfg;
   if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
   if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
   if (!dhidden_out && !dW_accum && !fused) return GRPO_OK;
   const SlotLayout& L = ctx->lay;
   __nv_bfloat16* dz = slot_ptr<__nv_bfloat16>(ctx, slot, L.off_dz);
-  const int64_t Tc = L.chunk_rows;
-  const int n_chunks = static_cast<int>((T + Tc - 1) / Tc);
-  // equalise chunks (whole 128-row tiles) so the last one is not a sliver
-  const int64_t rows_per_chunk = std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, BM * ctx->cg));
+  const int64_t rows_per_chunk = rows_per_chunk_for(ctx, T);
   const uint8_t* Hb = static_cast<const uint8_t*>(hidden);
   const int dh_elem = c.dhidden_fp32 ? 4 : 2;
 
@@ -575,7 +594,11 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
     GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
 
-    if (fused) GRPO_TRY(fwd_rows(ctx, slot, hidden, W, targets, *fused, T, t0, rows, dz, st));
+    const size_t chunk_idx = static_cast<size_t>(t0 / rows_per_chunk);
+    if (fused) {
+      if (pipe && chunk_idx < pipe->in.size()) CU_OK(cudaStreamWaitEvent(st, pipe->in[chunk_idx], 0));
+      GRPO_TRY(fwd_rows(ctx, slot, hidden, W, targets, *fused, T, t0, rows, dz, st));
+    }
     if (!dhidden_out && !dW_accum) continue;
     // zero-coefficient tile skipping: scan this chunk's coefficients on the device
     const int* tile_list = nullptr;
@@ -627,6 +650,12 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.tile_list = tile_list;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
+      if (pipe && pipe->dh_host && chunk_idx < pipe->out.size()) {   // this chunk's dHidden rows are final
+        CU_OK(cudaEventRecord(pipe->out[chunk_idx], st));
+        CU_OK(cudaStreamWaitEvent(pipe->cs, pipe->out[chunk_idx], 0));
+        CU_OK(cudaMemcpyAsync(pipe->dh_host + t0 * c.d * dh_elem, static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem,
+                              rows * c.d * dh_elem, cudaMemcpyDeviceToHost, pipe->cs));
+      }
     }
     if (dW_accum) {  // A6: dW[V, d] += dZ^T[V, rows] H[rows, d]
       GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
@@ -958,8 +987,26 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   float* coeff = slot_ptr<float>(ctx, 0, L.off_coeff);
   uint8_t* dh = slot_ptr<uint8_t>(ctx, 0, L.off_dh);
   float* loss_dev = slot_ptr<float>(ctx, 0, L.off_total) + 8;   // scratch scalar inside the 256-byte cell
-  const int dh_elem = c.dhidden_fp32 ? 4 : 2;
-  CU_OK(cudaMemcpyAsync(sh, hidden_host, T * c.d * 2, cudaMemcpyHostToDevice, st));
+  // copy pipeline: hidden states arrive chunk by chunk on the copy stream while the compute stream works
+  const int64_t rpc = rows_per_chunk_for(ctx, T);
+  const size_t n_chunks = static_cast<size_t>((T + rpc - 1) / rpc);
+  HostPipe pipe;
+  pipe.cs = ctx->copy_stream;
+  pipe.dh_host = static_cast<uint8_t*>(dhidden_host);
+  pipe.in.resize(n_chunks, nullptr);
+  pipe.out.resize(dhidden_host ? n_chunks : 0, nullptr);
+  struct Fence { cudaEvent_t e = nullptr; ~Fence() { if (e) cudaEventDestroy(e); } } fence;
+  CU_OK(cudaEventCreateWithFlags(&fence.e, cudaEventDisableTiming));
+  for (auto& e : pipe.in) CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  for (auto& e : pipe.out) CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  CU_OK(cudaEventRecord(fence.e, st));                       // staging buffers are free once st reaches here
+  CU_OK(cudaStreamWaitEvent(pipe.cs, fence.e, 0));
+  for (size_t i = 0; i < n_chunks; ++i) {
+    const int64_t t0 = static_cast<int64_t>(i) * rpc, rows = std::min<int64_t>(rpc, T - t0);
+    CU_OK(cudaMemcpyAsync(sh + t0 * c.d * 2, static_cast<const uint8_t*>(hidden_host) + t0 * c.d * 2, rows * c.d * 2,
+                          cudaMemcpyHostToDevice, pipe.cs));
+    CU_OK(cudaEventRecord(pipe.in[i], pipe.cs));
+  }
   CU_OK(cudaMemcpyAsync(stg, targets_host, T * 4, cudaMemcpyHostToDevice, st));
   CU_OK(cudaMemcpyAsync(so, old_logp_host, T * 4, cudaMemcpyHostToDevice, st));
   if (ref_logp_host) CU_OK(cudaMemcpyAsync(sr, ref_logp_host, T * 4, cudaMemcpyHostToDevice, st));
@@ -968,20 +1015,23 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   CU_OK(cudaMemcpyAsync(d_rw, rewards_host, S * 4, cudaMemcpyHostToDevice, st));
   CU_OK(cudaMemsetAsync(loss_dev, 0, 4, st));
   GRPO_TRY(grpo_group_advantage(ctx, d_rw, nullptr, n_groups, G, d_adv, nullptr, st));
+  GRPO_TRY(fwd_check(ctx, S, T));
+  const FwdArgs a{d_cu, S, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr, loss_denom, nullptr,
+                  logp, lse, coeff, loss_dev, nullptr};
+  GRPO_TRY(fwd_counts(ctx, 0, stg, a, st));
   if (c.stash_logits) {
-    GRPO_TRY(fwd_check(ctx, S, T));
-    const FwdArgs a{d_cu, S, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr, loss_denom, nullptr,
-                    logp, lse, coeff, loss_dev, nullptr};
-    GRPO_TRY(fwd_counts(ctx, 0, stg, a, st));
-    GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, &a));
+    GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, &a, &pipe));
   } else {
-    GRPO_TRY(fwd_impl(ctx, 0, sh, W, stg, d_cu, S, T, d_adv, so, ref_logp_host ? sr : nullptr,
-                      mask_host ? sm : nullptr, loss_denom, nullptr, logp, lse, coeff, loss_dev, nullptr, st));
-    GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st));
+    for (size_t i = 0; i < n_chunks; ++i) {                  // A2 + A3 chunk by chunk, as the rows arrive
+      const int64_t t0 = static_cast<int64_t>(i) * rpc, rows = std::min<int64_t>(rpc, T - t0);
+      CU_OK(cudaStreamWaitEvent(st, pipe.in[i], 0));
+      GRPO_TRY(fwd_rows(ctx, 0, sh, W, stg, a, T, t0, rows, nullptr, st));
+    }
+    GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, nullptr, &pipe));
   }
   CU_OK(cudaMemcpyAsync(loss_host, loss_dev, 4, cudaMemcpyDeviceToHost, st));
   if (logp_host) CU_OK(cudaMemcpyAsync(logp_host, logp, T * 4, cudaMemcpyDeviceToHost, st));
-  if (dhidden_host) CU_OK(cudaMemcpyAsync(dhidden_host, dh, T * c.d * dh_elem, cudaMemcpyDeviceToHost, st));
+  CU_OK(cudaStreamSynchronize(pipe.cs));
   CU_OK(cudaStreamSynchronize(st));
   return GRPO_OK;
 }
