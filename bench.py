@@ -234,6 +234,8 @@ def run_ours(args):
 
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
     b = make_config(args.config, seed=rank_seed(rank), device=dev)
+    if args.cgp_mode != "full":
+        return run_cgp_stream(args, b, dev, world)
     T, d, V = b.T, b.d, b.V
     extra = {}
     if args.no_tile_skip:
@@ -369,6 +371,74 @@ def run_ours(args):
     return 0
 
 
+def run_cgp_stream(args, b, dev, world):
+    """configs[4] (informational): the 32 complete groups are handed to grpo_enqueue_groups one at a time in their
+    seeded arrival order, as CGP delivers them: `per_group` = U = 1, one launch per group on one
+    stream; `batch4` = U = 4, 4-group launches round-robin on 4 streams.  Gradients accumulate in fp32 across
+    launches; the denominator is the whole batch's token count (R10)."""
+    import torch
+    from paper_2606_26997_b200 import GrpoContext
+    assert world == 1 and args.config == 5, "--cgp-mode per_group|batch4 needs --config 5 on one GPU"
+    U, n_streams = (1, 1) if args.cgp_mode == "per_group" else (4, 4)
+    order = [int(g) for g in b.arrival_order]
+    gtok = [b.group_token_range(g)[1] - b.group_token_range(g)[0] for g in order]
+    max_launch = max(sum(gtok[i:i + U]) for i in range(0, len(order), U))
+    ctx = GrpoContext(b.d, b.V, max_tokens=max_launch, n_slots=n_streams, group_size=b.G, kl_beta=b.kl_beta,
+                      clip_lo=b.clip_lo, clip_hi=b.clip_hi, groups_per_update=U, groups_per_round=len(order),
+                      **({"stash_logits": 1} if args.stash else {}))
+    streams = [torch.cuda.Stream() for _ in range(n_streams)]
+    dW = torch.zeros(b.V, b.d, dtype=torch.float32, device=dev)
+    loss = torch.zeros(1, dtype=torch.float32, device=dev)
+    dH = torch.empty(b.T, b.d, dtype=torch.bfloat16, device=dev)
+    descs = []
+    for g in order:
+        t0, t1 = b.group_token_range(g)
+        descs.append(ctx.make_group_desc(g, b.seqlens[g * b.G:(g + 1) * b.G], b.hidden[t0:t1], b.targets[t0:t1],
+                                         b.old_logp[t0:t1], b.rewards[g * b.G:(g + 1) * b.G].contiguous(),
+                                         None if b.ref_logp is None else b.ref_logp[t0:t1], None, dH[t0:t1], None))
+
+    def step():
+        for d_ in descs:
+            ctx.grpo_enqueue_groups([d_], b.W, dW, loss, loss_denom=float(b.T), streams=streams)
+        if ctx.grpo_queue_state()["pending_groups"]:
+            ctx.grpo_flush(b.W, dW, loss, loss_denom=float(b.T), streams=streams)
+        ctx.grpo_reset_round()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    assert ctx.grpo_check_errors_sync() == 0
+    sampler = ClockSampler(dev.index or 0)
+    n0 = ctx.grpo_kernel_launches()
+    sampler.start()
+    cur = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(cur)
+    for s_ in streams:
+        s_.wait_event(e0)
+    for _ in range(args.steps):
+        step()
+    for s_ in streams:
+        cur.wait_stream(s_)
+    e1.record(cur)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    n1 = ctx.grpo_kernel_launches()
+    line = {"metric": METRIC, "value": b.T * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": WORKLOADS[5].replace("as ONE full-batch step", f"streamed through "
+                       f"grpo_enqueue_groups: {args.cgp_mode} (U={U}, {n_streams} stream(s))"),
+                       "tokens_per_step": b.T, "groups": len(order), "variant": "stash_logits" if args.stash else "recompute"},
+            "e2e": None, "gpu_launches": sum(n1.values()) - sum(n0.values()), "clocks": clocks,
+            "executed_tflops": (2.0 * b.T * b.V * b.d * (3 if args.stash else 4)) * args.steps / (ms * 1e-3) / 1e12,
+            "note": "dense FLOP basis (zero-coefficient tiles are skipped, so this is an upper bound on executed FLOPs)"}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+    return 0
+
+
 def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, prof, clocks, peaks, tokens_all,
                loss_val):
     T, d, V = b.T, b.d, b.V
@@ -444,6 +514,9 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5],
                     help="workload = workloads.synth.make_config index (2 = BASELINE configs[1], the headline; "
                          "3-5 are informational device-resident runs without the e2e / cpu_baseline legs)")
+    ap.add_argument("--cgp-mode", choices=["full", "per_group", "batch4"], default="full",
+                    help="--config 5 only: stream the 32 groups through grpo_enqueue_groups one launch per group "
+                         "(per_group) or in 4-group launches on 4 streams (batch4) instead of one full-batch step")
     ap.add_argument("--stash", action="store_true",
                     help="time grpo_fused_logprob_loss_fwd_bwd (3-contraction variant) as the step instead of the "
                          "north_star forward + recomputing backward")
