@@ -213,10 +213,15 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 
   if (warp == kProducerWarp) {
     // ================================================================ TMA producer
-    if (lane == 0) {
+    // Like the MMA warp, the whole warp walks the loop converged and one elected lane issues: every
+    // address and coordinate is then warp-uniform and lives in uniform registers (a lane-0-only loop costs
+    // an ELECT + four R2UR.BROADCAST per TMA instruction, which made this thread the bottleneck of A6).
+    {
+      const bool leader_lane = elect_one();
+      const uint32_t full0 = CG == 2 ? mapa_cluster(smem_u32(&bars->full[0]), 0) : smem_u32(&bars->full[0]);
       int stage = 0;
       uint32_t phase = 0;
-      bool sync_on = p.sync != nullptr;
+      bool sync_on = p.sync != nullptr && cta_rank == 0;
       int epoch = 0, to_epoch = 1;
       for (int u = unit0; u < n_units; u += unit_step) {
         int m_tile, n0, n1;
@@ -226,41 +231,45 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           const int b_row = n_tile * BN + static_cast<int>(cta_rank) * kBRows;
           for (int kbw = 0; kbw < ext.k_blocks; ++kbw) {
             const int kb = EPI == EPI_RED_F32 ? walked_k_block<CG>(p, kbw) : kbw;
-            if (sync_on && cta_rank == 0 && --to_epoch == 0) {
+            if (sync_on && --to_epoch == 0) {
               to_epoch = p.sync_epoch_kb;
-              red_add_u32(p.sync + epoch, 1u);
+              if (leader_lane) red_add_u32(p.sync + epoch, 1u);
               const int need = epoch - (p.sync_lag - 1);         // every pair has arrived on epoch need - 1
               if (ld_volatile_shared_i32(&bars->gate_open) < need) {
                 const long long t0 = clock64();
                 while (ld_volatile_shared_i32(&bars->gate_open) < need)
                   if (clock64() - t0 > 2 * kGateMaxTimeouts * kGateTimeoutClk) { sync_on = false; break; }
+                sync_on = __shfl_sync(0xffffffffu, sync_on ? 1 : 0, 0) != 0;   // one decision for the warp
               }
               ++epoch;
             }
             mbar_wait(&bars->empty[stage], phase ^ 1);
-            // the leader's barrier collects the bytes of both CTAs (one arrival: the leader's)
-            if (cta_rank == 0) mbar_arrive_expect_tx(&bars->full[stage], kStageBytes * CG);
-            const uint32_t a_dst = tiles_addr + stage * kStageBytes;
-            const uint32_t b_dst = a_dst + kABytes;
-            const uint32_t bar = CG == 2 ? mapa_cluster(smem_u32(&bars->full[stage]), 0) : smem_u32(&bars->full[stage]);
-            if constexpr (!A_MN) {
-              tma_load_2d_t<CG>(a_dst, &tmA, bar, kb * BK, a_row);
-            } else {
+            if (leader_lane) {
+              // the leader CTA's barrier collects the bytes of both CTAs (one arrival: the leader's)
+              if (cta_rank == 0) mbar_arrive_expect_tx(&bars->full[stage], kStageBytes * CG);
+              const uint32_t a_dst = tiles_addr + stage * kStageBytes;
+              const uint32_t b_dst = a_dst + kABytes;
+              const uint32_t bar = full0 + stage * 8;
+              if constexpr (!A_MN) {
+                tma_load_2d_t<CG>(a_dst, &tmA, bar, kb * BK, a_row);
+              } else {
 #pragma unroll
-              for (int i = 0; i < BM / 64; ++i) tma_load_2d_t<CG>(a_dst + i * 8192, &tmA, bar, a_row + i * 64, kb * BK);
-            }
-            if constexpr (!B_MN) {
-              tma_load_2d_t<CG>(b_dst, &tmB, bar, kb * BK, b_row);
-            } else {
+                for (int i = 0; i < BM / 64; ++i) tma_load_2d_t<CG>(a_dst + i * 8192, &tmA, bar, a_row + i * 64, kb * BK);
+              }
+              if constexpr (!B_MN) {
+                tma_load_2d_t<CG>(b_dst, &tmB, bar, kb * BK, b_row);
+              } else {
 #pragma unroll
-              for (int i = 0; i < kBRows / 64; ++i) tma_load_2d_t<CG>(b_dst + i * 8192, &tmB, bar, b_row + i * 64, kb * BK);
+                for (int i = 0; i < kBRows / 64; ++i) tma_load_2d_t<CG>(b_dst + i * 8192, &tmB, bar, b_row + i * 64, kb * BK);
+              }
             }
+            __syncwarp();
             if (++stage == kStages) { stage = 0; phase ^= 1; }
           }
         }
       }
       // pairs with fewer units must not hold the others back: arrive for every epoch not reached
-      if (p.sync != nullptr && cta_rank == 0)
+      if (p.sync != nullptr && cta_rank == 0 && leader_lane)
         for (; epoch < p.sync_epochs; ++epoch) red_add_u32(p.sync + epoch, 1u);
     }
   } else if (warp == kMmaWarp) {
