@@ -34,12 +34,14 @@ constexpr int kABytes = BM * BK * 2;        // 16 KB
 constexpr int kGemmThreads = 224;
 constexpr int kProducerWarp = 4, kMmaWarp = 5, kGateWarp = 6;
 constexpr int kTmemCols = 512;
+constexpr int kMaxTilesSmem = 1024;         // active-tile indices the A6 producer keeps in shared memory
 template <int CG> struct GemmShape {
   static constexpr int kBRows = BN / CG;                       // B rows (N index) staged by one CTA
   static constexpr int kBBytes = kBRows * BK * 2;              // 32 KB / 16 KB
   static constexpr int kStageBytes = kABytes + kBBytes;        // 48 KB / 32 KB
   static constexpr int kStages = CG == 1 ? 4 : 6;
-  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/ +
+                                    kMaxTilesSmem * 4 /*A6 tile list*/;
 };
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -95,6 +97,7 @@ struct alignas(8) GemmBarriers {
   uint64_t tmem_empty[2];
   uint32_t tmem_base;
   int gate_open;                     // highest epoch the producer may enter (written by the gate warp)
+  int klist[kMaxTilesSmem];          // A6: active token tiles of the chunk, staged by the producer warp
 };
 
 // Effective extent of a launch under tile skipping: the number of m tiles walked (A4/A5), the k blocks
@@ -115,11 +118,16 @@ __device__ __forceinline__ Extent launch_extent(const GemmParams& p, int n_units
   }
   return e;
 }
-// k block (in units of BK token rows) the kb-th walked k block of A6 maps to
+// k block (in units of BK token rows) the kb-th walked k block of A6 maps to.  `klist` is the shared-memory
+// copy of the active-tile list (a global load per k block on the producer's critical path costs more than
+// the k block's MMAs take).
 template <int CG>
-__device__ __forceinline__ int walked_k_block(const GemmParams& p, int kb) {
+__device__ __forceinline__ int walked_k_block(const GemmParams& p, const int* klist, int kb) {
   constexpr int kPerTile = BM * CG / BK;
-  return p.tile_list == nullptr ? kb : p.tile_list[2 + kb / kPerTile] * kPerTile + kb % kPerTile;
+  if (p.tile_list == nullptr) return kb;
+  const int t = kb / kPerTile;
+  const int tile = t < kMaxTilesSmem ? klist[t] : p.tile_list[2 + t];
+  return tile * kPerTile + kb % kPerTile;
 }
 
 template <int EPI>
@@ -217,6 +225,13 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     // address and coordinate is then warp-uniform and lives in uniform registers (a lane-0-only loop costs
     // an ELECT + four R2UR.BROADCAST per TMA instruction, which made this thread the bottleneck of A6).
     {
+      if constexpr (EPI == EPI_RED_F32) {
+        if (p.tile_list != nullptr) {
+          const int n_act = min(p.tile_list[0], kMaxTilesSmem);
+          for (int i = lane; i < n_act; i += 32) bars->klist[i] = p.tile_list[2 + i];
+          __syncwarp();
+        }
+      }
       const bool leader_lane = elect_one();
       const uint32_t full0 = CG == 2 ? mapa_cluster(smem_u32(&bars->full[0]), 0) : smem_u32(&bars->full[0]);
       int stage = 0;
@@ -230,7 +245,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         for (int n_tile = n0; n_tile < n1; ++n_tile) {
           const int b_row = n_tile * BN + static_cast<int>(cta_rank) * kBRows;
           for (int kbw = 0; kbw < ext.k_blocks; ++kbw) {
-            const int kb = EPI == EPI_RED_F32 ? walked_k_block<CG>(p, kbw) : kbw;
+            const int kb = EPI == EPI_RED_F32 ? walked_k_block<CG>(p, bars->klist, kbw) : kbw;
             if (sync_on && --to_epoch == 0) {
               to_epoch = p.sync_epoch_kb;
               if (leader_lane) red_add_u32(p.sync + epoch, 1u);
