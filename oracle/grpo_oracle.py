@@ -32,7 +32,7 @@ import numpy as np
 __all__ = [
     "OracleConfig", "bf16_bits_to_f64", "group_advantage", "token_advantage",
     "token_logprobs", "loss_terms", "backward", "grpo_step", "grpo_step_loops",
-    "token_rows", "dH_rows", "dW_rows",
+    "token_rows", "dH_rows", "dW_rows", "token_entropy",
 ]
 
 
@@ -119,6 +119,24 @@ def token_logprobs(H, W, y, logit_scale=1.0, chunk_tokens=1024):
         zy = z[np.arange(t1 - t0), yy]
         logp[t0:t1] = np.where(valid[t0:t1], zy - l, 0.0)
     return lse, logp
+
+
+def token_entropy(H, W, logit_scale=1.0, chunk_tokens=1024):
+    """NEXT-2 (R28): Shannon entropy of the policy at every packed row, in nats, by its definition
+    on the materialised softmax:  p_tv = exp(z_tv - lse_t),  entropy_t = - sum_v p_tv log p_tv.
+    A diagnostic output (no gradient flows through it).  Returns float64 [T]."""
+    H = np.asarray(H, dtype=np.float64)
+    W = np.asarray(W, dtype=np.float64)
+    T = H.shape[0]
+    ent = np.zeros(T)
+    for t0 in range(0, T, chunk_tokens):
+        t1 = min(T, t0 + chunk_tokens)
+        z = logit_scale * (H[t0:t1] @ W.T)
+        m = z.max(axis=1, keepdims=True)
+        logp_all = z - (m + np.log(np.exp(z - m).sum(axis=1, keepdims=True)))
+        p_all = np.exp(logp_all)
+        ent[t0:t1] = -(p_all * logp_all).sum(axis=1)
+    return ent
 
 
 # ---------------------------------------------------------------------- steps 5 - 9a

@@ -142,3 +142,28 @@ def test_variants_loops_oracle_agrees():
         for k in ("coeff", "dH", "dW"):
             np.testing.assert_allclose(a[k], b[k], rtol=1e-11, atol=1e-15, err_msg=k)
         np.testing.assert_allclose(a["loss"], b["loss"], rtol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------- entropy (R28)
+def test_entropy_pins():
+    """Uniform policy -> ln V; two classes -> binary entropy of the logistic; library routine; bounds; the
+    identity entropy = lse - sum_v p_v z_v that the kernel's online form uses."""
+    import scipy.stats
+    from oracle.grpo_oracle import token_entropy, token_logprobs
+    rng = np.random.default_rng(3)
+    H = rng.normal(size=(6, 5))
+    assert np.allclose(token_entropy(H, np.zeros((9, 5))), np.log(9.0), rtol=1e-14)
+    W2 = rng.normal(size=(2, 5))
+    q = 1.0 / (1.0 + np.exp(-(H @ (W2[0] - W2[1]))))
+    np.testing.assert_allclose(token_entropy(H, W2), -(q * np.log(q) + (1 - q) * np.log(1 - q)), rtol=1e-12)
+    W = rng.normal(size=(13, 5))
+    ent = token_entropy(H, W, logit_scale=1.7)
+    z = 1.7 * H @ W.T
+    p = np.exp(z - z.max(1, keepdims=True)); p /= p.sum(1, keepdims=True)
+    np.testing.assert_allclose(ent, scipy.stats.entropy(p, axis=1), rtol=1e-12)
+    assert np.all(ent > 0) and np.all(ent < np.log(13.0))
+    lse, _ = token_logprobs(H, W, np.zeros(6, dtype=np.int64), logit_scale=1.7)
+    np.testing.assert_allclose(ent, lse - (p * z).sum(1), rtol=1e-12)
+    # a sharply peaked policy has (almost) no entropy; chunking does not matter
+    assert token_entropy(H, W, logit_scale=200.0).max() < 1e-3
+    np.testing.assert_array_equal(token_entropy(H, W, chunk_tokens=2), token_entropy(H, W, chunk_tokens=100))
