@@ -132,14 +132,23 @@ int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden, const voi
                                     void* dhidden_out, float* dW_accum, void* stream);
 
 /* One COMPLETE group (all K responses present, rewards verified). */
+/* Optional diagnostic output of the forward (R28): while a non-NULL
+ * device pointer is set, every later grpo_fused_logprob_loss_fwd / _fwd_bwd call of this context also writes
+ * entropy_out[t] = - sum_v p_tv log p_tv (nats) for each of its T packed rows (one more running sum in the A2
+ * epilogue; no gradient flows through it).  The caller owns the buffer ([T] fp32 of the largest call) and
+ * keeps it alive until the stream reaches the call's work.  NULL turns it off (default).  Not used by
+ * grpo_enqueue_groups / grpo_step_host. */
+int32_t grpo_set_entropy_out(grpo_ctx* ctx, float* entropy_out);
+
 /* 3-contraction variant of forward + backward in ONE call.
- * Per chunk of bwd_chunk_tokens tokens: the forward contraction (A2) also writes the chunk's scaled logits as
- * fp16 into the workspace chunk buffer, A3 runs on the chunk, an HBM-bound pass turns the stashed logits into
+ * Per chunk of bwd_chunk_tokens tokens: the forward contraction (A2) also writes the chunk's softmax numerators
+ * as fp16 into the workspace chunk buffer, A3 runs on the chunk, an HBM-bound pass turns the stashed logits into
  * dZ in place, then A5 and A6 run as in the backward.  The [T, V] logits are still never materialised (one
  * [Tc, V] chunk lives in the workspace) but nothing is recomputed: 6 T V d FLOPs instead of 8 T V d.
  * Arguments and outputs are those of grpo_fused_logprob_loss_fwd followed by grpo_fused_logprob_loss_bwd
- * (dhidden_out / dW_accum may each be NULL); results agree with that pair within the parity tolerances
- * (the stashed logit is rounded to fp16, the recomputed one is not).  The denominator of the mean must be
+ * (dhidden_out / dW_accum may each be NULL); results agree with that pair within the parity tolerances (what
+ * is stashed is each logit's exponential relative to its row's running maximum, rounded to fp16: a 2^-11
+ * relative error per probability whatever the magnitude of the logits; the recomputed path has none).  The denominator of the mean must be
  * known before the first chunk: loss_denom > 0, or it is counted from mask / targets of this call first. */
 int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hidden, const void* W, const int32_t* targets,
                                         const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv,

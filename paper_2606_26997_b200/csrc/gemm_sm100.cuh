@@ -47,8 +47,11 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
 enum Epi : int { EPI_LSE = 0, EPI_DZ = 1, EPI_STORE = 2, EPI_RED_F32 = 3, EPI_LSE_STASH = 4 };
-// EPI_LSE_STASH (3-contraction variant): EPI_LSE that also writes the scaled logits
-// z s log2(e) as fp16 into the chunk buffer `dz`, which stash_to_dz_kernel later turns into dZ in place.
+// EPI_LSE_STASH (3-contraction variant): EPI_LSE that also writes, for every logit, the
+// exponential e = 2^(z2 - m) it adds to the running sum (z2 = z s log2(e), m = the row's running max after the
+// element's 256-column tile) as fp16 into the chunk buffer `dz`, and m per (row, tile) into `stash_shift`;
+// stash_to_dz_kernel later turns e into dZ = k (1[v = y] - e 2^(m - lse2)) in place.  Stashing e instead of the
+// logit keeps the relative error of every probability at fp16's 2^-11 whatever the magnitude of the logits.
 __host__ __device__ constexpr bool is_lse(int epi) { return epi == EPI_LSE || epi == EPI_LSE_STASH; }
 
 struct GemmParams {
@@ -66,6 +69,7 @@ struct GemmParams {
   // EPI_LSE outputs (log2 domain running max / sum per split) + the target logit
   float* part_m;
   float* part_s;
+  float* part_u;                     // nullable: sum 2^(z2 - max) z2 per split, for the entropy output (R28)
   int64_t part_stride;
   float* zy;
   // EPI_DZ
@@ -74,6 +78,8 @@ struct GemmParams {
   float coeff_mul;                   // logit_scale * grad_scale
   __nv_bfloat16* dz;
   int64_t dz_pitch;
+  float* stash_shift;                // EPI_LSE_STASH: running max (log2 domain) per (row, 256-column tile)
+  int64_t shift_pitch;
   // EPI_STORE (bf16 or fp32) / EPI_RED_F32
   void* c_out;
   int64_t c_pitch;                   // elements
@@ -370,7 +376,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       const int64_t row_g = p.row_offset + row_local;            // index into per-token arrays
 
       [[maybe_unused]] int y = -1;
-      [[maybe_unused]] float run_m = -INFINITY, run_s = 0.f;     // EPI_LSE running stats (log2 domain)
+      [[maybe_unused]] float run_m = -INFINITY, run_s = 0.f, run_u = 0.f;   // EPI_LSE running stats (log2 domain)
       [[maybe_unused]] float lse2 = 0.f, kcoef = 0.f;            // EPI_DZ per-row constants
       if constexpr (is_lse(EPI) || EPI == EPI_DZ) {
         if (row_ok) {
@@ -390,6 +396,27 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         tc_fence_after();
         const uint32_t t_addr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
         const int col_tile = n_tile * BN;
+        if constexpr (EPI == EPI_LSE_STASH) {
+          // first pass over the accumulator: the tile's maximum, so that one running max covers the whole tile
+          float tmax = -INFINITY;
+#pragma unroll 1
+          for (int c = 0; c < BN / 32; ++c) {
+            const int cbase = col_tile + c * 32;
+            if (cbase >= p.n_total) break;
+            float v[32];
+            tmem_ld32(t_addr + c * 32, v);
+            tmem_ld_wait();
+            const int nvalid = p.n_total - cbase;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, i < nvalid ? v[i] * p.scale_log2e : -INFINITY);
+          }
+          const float new_m = fmaxf(run_m, tmax);
+          const float rescale = ex2_approx(run_m - new_m);
+          run_s *= rescale;
+          run_u *= rescale;
+          run_m = new_m;
+          if (row_ok) p.stash_shift[static_cast<int64_t>(row_local) * p.shift_pitch + n_tile] = new_m;
+        }
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c) {
           const int cbase = col_tile + c * 32;
@@ -411,20 +438,39 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                 cmax = fmaxf(cmax, v[i]);
               }
             }
+            const float new_m = EPI == EPI_LSE_STASH ? run_m : fmaxf(run_m, cmax);   // stash: tile max already in
+            float s = 0.f;
+            const float rescale = ex2_approx(run_m - new_m);
             if constexpr (EPI == EPI_LSE_STASH) {
-              if (row_ok) {   // scaled logits (log2 domain) as fp16; padding columns hold -inf
+              float e[32], uc = 0.f;
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                e[i] = ex2_approx(v[i] - new_m);                   // padding columns: 2^-inf = 0
+                s += e[i];
+                if (p.part_u != nullptr) uc = fmaf(e[i], i < nvalid ? v[i] : 0.f, uc);
+              }
+              run_u += uc;
+              if (row_ok) {
                 __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
 #pragma unroll
                 for (int g = 0; g < 4; ++g)
-                  st_global_v4(dst + g * 8, pack_f16x2(v[g * 8 + 0], v[g * 8 + 1]), pack_f16x2(v[g * 8 + 2], v[g * 8 + 3]),
-                               pack_f16x2(v[g * 8 + 4], v[g * 8 + 5]), pack_f16x2(v[g * 8 + 6], v[g * 8 + 7]));
+                  st_global_v4(dst + g * 8, pack_f16x2(e[g * 8 + 0], e[g * 8 + 1]), pack_f16x2(e[g * 8 + 2], e[g * 8 + 3]),
+                               pack_f16x2(e[g * 8 + 4], e[g * 8 + 5]), pack_f16x2(e[g * 8 + 6], e[g * 8 + 7]));
               }
-            }
-            const float new_m = fmaxf(run_m, cmax);
-            float s = 0.f;
+            } else if (p.part_u == nullptr) {
 #pragma unroll
-            for (int i = 0; i < 32; ++i) s += ex2_approx(v[i] - new_m);
-            run_s = run_s * ex2_approx(run_m - new_m) + s;
+              for (int i = 0; i < 32; ++i) s += ex2_approx(v[i] - new_m);
+            } else {   // entropy = lse - sum_v p_v z_v: one more running sum, rescaled like the sum of exponentials
+              float uc = 0.f;
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                const float e = ex2_approx(v[i] - new_m);
+                s += e;
+                uc = fmaf(e, i < nvalid ? v[i] : 0.f, uc);        // padding columns hold -inf: 0 * -inf is NaN
+              }
+              run_u = run_u * rescale + uc;
+            }
+            run_s = run_s * rescale + s;
             run_m = new_m;
             if (static_cast<uint32_t>(y - cbase) < 32u) {          // rare: target column in this chunk
               float zy2 = 0.f;
@@ -494,6 +540,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           const int split = u / p.m_tiles;
           p.part_m[split * p.part_stride + row_local] = run_m;     // partials are indexed by the launch's own rows
           p.part_s[split * p.part_stride + row_local] = run_s;
+          if (p.part_u != nullptr) p.part_u[split * p.part_stride + row_local] = run_u;
         }
       }
     }

@@ -53,6 +53,8 @@ struct SlotLayout {
   int64_t s_max = 0;
   int64_t chunk_rows = 0;
   int64_t v_pad = 0;
+  int64_t off_part_u = 0, off_shift = 0;
+  int64_t n_vtiles = 0;   // 256-column vocab tiles (pitch of the stash shift array)
   int64_t off_part_m = 0, off_part_s = 0, off_zy = 0, off_total = 0, off_seq_count = 0, off_dz = 0;
   int64_t off_hidden = 0, off_targets = 0, off_old = 0, off_ref = 0, off_mask = 0, off_rewards = 0, off_adv = 0,
           off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0, off_sync = 0,
@@ -77,6 +79,7 @@ struct grpo_ctx {
   float* denom_ring = nullptr;   // device scalars for implicit per-update denominators
   int denom_next = 0;
   cudaEvent_t denom_event = nullptr;
+  float* entropy_out = nullptr;         // grpo_set_entropy_out: per-token entropy of the direct forward calls
   cudaStream_t copy_stream = nullptr;   // grpo_step_host: H2D / D2H overlapped with the compute stream
   uint8_t* ws = nullptr;
   int64_t ws_max_T = 0;
@@ -132,10 +135,13 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.v_pad = align_up(c.V, 64);
   L.off_part_m = take(L.part_cap * 4);
   L.off_part_s = take(L.part_cap * 4);
+  L.off_part_u = take(L.part_cap * 4);
   L.off_zy = take(max_T * 4);
   L.off_total = take(256);
   L.off_seq_count = take(L.s_max * 4);
   L.off_dz = take(L.chunk_rows * L.v_pad * 2);
+  L.n_vtiles = (c.V + BN - 1) / BN;
+  L.off_shift = take(L.chunk_rows * L.n_vtiles * 4);
   L.off_hidden = take(max_T * c.d * 2);
   L.off_targets = take(max_T * 4);
   L.off_old = take(max_T * 4);
@@ -427,6 +433,7 @@ struct FwdArgs {
   const float* adv; const float* old_logp; const float* ref_logp; const uint8_t* mask;
   double loss_denom; const float* denom_dev;
   float* logp_out; float* lse_out; float* coeff_out; float* loss_accum; float* metrics_accum;
+  float* entropy_out = nullptr;   // nullable (grpo_set_entropy_out)
 };
 
 static int32_t fwd_check(grpo_ctx* ctx, int32_t S, int64_t T) {
@@ -488,9 +495,11 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
   p.logit_scale = c.logit_scale;
   p.part_m = part_m;
   p.part_s = part_s;
+  p.part_u = a.entropy_out ? slot_ptr<float>(ctx, slot, L.off_part_u) : nullptr;
   p.part_stride = rows;
   p.zy = zy;
   p.dz = stash; p.dz_pitch = L.v_pad;
+  p.stash_shift = slot_ptr<float>(ctx, slot, L.off_shift); p.shift_pitch = L.n_vtiles;
   p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
   if (stash)
     GRPO_TRY((launch_gemm<false, false, EPI_LSE_STASH>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
@@ -500,7 +509,7 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
   LossParams lp;
   std::memset(&lp, 0, sizeof(lp));
   lp.T = rows; lp.t_begin = t0; lp.S = a.S; lp.V = c.V; lp.n_split = p.n_split; lp.part_stride = rows;
-  lp.part_m = part_m; lp.part_s = part_s; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = a.cu_seqlens;
+  lp.part_m = part_m; lp.part_s = part_s; lp.part_u = p.part_u; lp.entropy = a.entropy_out; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = a.cu_seqlens;
   lp.adv = a.adv; lp.old_logp = a.old_logp; lp.ref_logp = a.ref_logp; lp.mask = a.mask;
   lp.seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
   lp.total_count = a.denom_dev ? a.denom_dev : slot_ptr<float>(ctx, slot, L.off_total);
@@ -523,10 +532,11 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
                         const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv, const float* old_logp,
                         const float* ref_logp, const uint8_t* mask, double loss_denom, const float* denom_dev,
                         float* logp_out, float* lse_out, float* coeff_out, float* loss_accum, float* metrics_accum,
-                        cudaStream_t st) {
+                        cudaStream_t st, float* entropy_out = nullptr) {
   GRPO_TRY(fwd_check(ctx, S, T));
-  const FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
-                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
+            logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  a.entropy_out = entropy_out;
   GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
   return fwd_rows(ctx, slot, hidden, W, targets, a, T, 0, T, nullptr, st);
 }
@@ -542,7 +552,14 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden
     return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
   if (T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0 and S > 0 (got T=%lld S=%d)", (long long)T, S);
   return fwd_impl(ctx, 0, hidden, W, targets, cu_seqlens, S, T, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
-                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum, static_cast<cudaStream_t>(stream));
+                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum, static_cast<cudaStream_t>(stream),
+                  ctx->entropy_out);
+}
+
+extern "C" int32_t grpo_set_entropy_out(grpo_ctx* ctx, float* entropy_out) {
+  if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL");
+  ctx->entropy_out = entropy_out;
+  return GRPO_OK;
 }
 
 // ------------------------------------------------------------------------------------- A4 - A6
@@ -622,8 +639,8 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     if (fused) {  // stashed logits -> dZ in place (HBM-bound elementwise pass instead of the A4 contraction)
       LaunchScope ls(ctx, GRPO_KERNEL_STASH_DZ, st);
       stash_to_dz_kernel<<<static_cast<unsigned>(rows), 256, 0, st>>>(
-          reinterpret_cast<uint16_t*>(dz), static_cast<int>(rows), c.V, L.v_pad, targets + t0, lse + t0, coeff + t0,
-          c.logit_scale * grad_scale, tile_list, TM);
+          reinterpret_cast<uint16_t*>(dz), static_cast<int>(rows), c.V, L.v_pad, slot_ptr<float>(ctx, slot, L.off_shift),
+          L.n_vtiles, BN, targets + t0, lse + t0, coeff + t0, c.logit_scale * grad_scale, tile_list, TM);
       CU_OK(cudaGetLastError());
     } else {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
       GemmParams p;
@@ -698,8 +715,9 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hi
   if (T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0 and S > 0 (got T=%lld S=%d)", (long long)T, S);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   GRPO_TRY(fwd_check(ctx, S, T));
-  const FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
-                  logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
+            logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  a.entropy_out = ctx->entropy_out;
   GRPO_TRY(fwd_counts(ctx, 0, targets, a, st));
   return bwd_impl(ctx, 0, hidden, W, targets, lse_out, coeff_out, T, grad_scale, dhidden_out, dW_accum, st, &a);
 }

@@ -88,6 +88,7 @@ struct LossParams {
   int64_t part_stride;
   const float* part_m;
   const float* part_s;
+  const float* part_u;       // nullable (entropy output)
   const float* zy;
   const int32_t* targets;
   const int32_t* cu_seqlens;
@@ -105,6 +106,7 @@ struct LossParams {
   float* logp;
   float* lse;
   float* coeff;
+  float* entropy;            // nullable: per-token policy entropy in nats (R28), every row of the launch
   float* loss_accum;
   float* metrics_accum;      // nullable, [4]
   int32_t* err_flag;
@@ -123,6 +125,12 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
     for (int i = 0; i < p.n_split; ++i)
       sum += p.part_s[i * p.part_stride + tl] * exp2f(p.part_m[i * p.part_stride + tl] - M);
     const float lse = (M + log2f(sum)) * kLn2;
+    if (p.entropy != nullptr && p.part_u != nullptr) {          // entropy = lse - sum_v p_v z_v   (log2 domain, then nats)
+      float usum = 0.f;
+      for (int i = 0; i < p.n_split; ++i)
+        usum += p.part_u[i * p.part_stride + tl] * exp2f(p.part_m[i * p.part_stride + tl] - M);
+      p.entropy[t] = ((M + log2f(sum)) - usum / sum) * kLn2;
+    }
     const int y = p.targets[t];
     const bool valid = y >= 0 && y < p.V;
     if (y >= p.V) atomicOr(p.err_flag, 1);
@@ -227,11 +235,13 @@ __global__ void __launch_bounds__(1024) active_tiles_kernel(const float* __restr
   }
 }
 
-// 3-contraction variant: turn the stashed scaled logits z2 = z s log2(e) (fp16, written
-// by the EPI_LSE_STASH epilogue) into dZ = k_t (1[v = y_t] - 2^(z2 - lse2_t)) (bf16) in place; k_t = coeff_t *
-// coeff_mul.  HBM-bound: 2 B read + 2 B written per logit.  One block per walked row; 16-byte accesses.
+// 3-contraction variant: turn the stashed exponentials e = 2^(z2 - m) (fp16, written by the
+// EPI_LSE_STASH epilogue together with m per (row, 256-column tile) in `shift`) into
+// dZ = k_t (1[v = y_t] - e 2^(m - lse2_t)) (bf16) in place; k_t = coeff_t * coeff_mul.  HBM-bound: 2 B read + 2 B
+// written per logit.  One block per walked row; 16-byte accesses; one ex2 per 8 logits.
 __global__ void __launch_bounds__(256) stash_to_dz_kernel(uint16_t* __restrict__ buf, int rows, int V, int64_t pitch,
-                                                          const int32_t* __restrict__ targets,
+                                                          const float* __restrict__ shift, int64_t shift_pitch,
+                                                          int tile_cols, const int32_t* __restrict__ targets,
                                                           const float* __restrict__ lse, const float* __restrict__ coeff,
                                                           float coeff_mul, const int* __restrict__ tile_list,
                                                           int tile_rows) {
@@ -247,16 +257,18 @@ __global__ void __launch_bounds__(256) stash_to_dz_kernel(uint16_t* __restrict__
   int y = targets[row];
   if (y >= V) y = -1;
   uint4* line = reinterpret_cast<uint4*>(buf + static_cast<int64_t>(row) * pitch);
+  const float* sh = shift + static_cast<int64_t>(row) * shift_pitch;
   const int n_vec = (V + 7) / 8;
   for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
     const uint4 in = line[i];
+    const float f = -k * ex2_approx(sh[i * 8 / tile_cols] - lse2);      // - k 2^(m - lse2) <= k in magnitude
     const uint32_t w4[4] = {in.x, in.y, in.z, in.w};
     float dz[8];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-      const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w4[j]));
-      dz[2 * j] = -k * ex2_approx(f.x - lse2);
-      dz[2 * j + 1] = -k * ex2_approx(f.y - lse2);
+      const float2 e = __half22float2(*reinterpret_cast<const __half2*>(&w4[j]));
+      dz[2 * j] = f * e.x;
+      dz[2 * j + 1] = f * e.y;
     }
     if (static_cast<uint32_t>(y - i * 8) < 8u) {
 #pragma unroll

@@ -65,6 +65,13 @@ def test_temperature_sample_std_explicit_denominator_and_grad_scale():
            loss_denom=float(b.T) / 3.0)
 
 
+def test_large_logits_keep_their_precision():
+    """|z| up to ~100 (w_std = 3, d = 64, temperature 1/1.3): what is stashed is the exponential relative to the
+    row's running max, not the logit, so the relative error of every probability stays at fp16's 2^-11."""
+    b = make_config(1, device="cuda", seed=13, variant="1b", w_std=3.0)
+    _check(b, ctx_kw=dict(logit_scale=1.3, bwd_chunk_tokens=128, dhidden_fp32=1), oracle_kw=dict(logit_scale=1.3))
+
+
 def test_agrees_with_the_recompute_path():
     b = make_config(3, device="cuda", seed=5, d=128, V=3000, n_groups=3, G=4, len_div=8.0)
     outs = []

@@ -117,3 +117,45 @@ def test_all_tiles_zero_gives_zero_gradients():
     finally:
         ctx.close()
     assert torch.all(out["dH"] == 0) and torch.all(out["dW"] == 0)
+
+
+# ------------------------------------------------------------------ per-token entropy output (R28)
+@pytest.mark.parametrize("fused", [False, True])
+@pytest.mark.parametrize("w_std,scale", [(0.02, 1.0), (1.0, 0.8), (3.0, 1.3)])
+def test_entropy_output(fused, w_std, scale):
+    """V = 1000 leaves 24 padding columns in the last 32-column chunk and T ~ 320 splits the vocab over many
+    CTA pairs (partial sums combined in A3); w_std spans near-uniform to sharply peaked policies."""
+    from oracle.grpo_oracle import token_entropy
+    b = make_config(1, device="cuda", seed=13, variant="1b", w_std=w_std, bad_target_frac=0.1)
+    ctx = make_ctx(b, logit_scale=scale, bwd_chunk_tokens=128)
+    try:
+        ent = torch.full((b.T,), float("nan"), dtype=torch.float32, device="cuda")
+        ctx.grpo_set_entropy_out(ent)
+        out = run_cuda(ctx, b, fused=fused)
+        ctx.grpo_set_entropy_out(None)
+        ent2 = ent.clone()
+        run_cuda(ctx, b, fused=fused)                                      # off again: the buffer is not touched
+        assert torch.equal(ent, ent2)
+    finally:
+        ctx.close()
+    x = b.numpy_f64()
+    ref = token_entropy(x["H"], x["W"], logit_scale=scale)
+    assert np.abs(to64(ent) - ref).max() <= 2e-3, np.abs(to64(ent) - ref).max()
+    assert_gates(gates(b, out, run_oracle(b, logit_scale=scale), logit_scale=scale))   # the rest is unchanged
+
+
+def test_entropy_output_full_vocab_sampled_rows():
+    from oracle.grpo_oracle import token_entropy
+    b = make_config(2, device="cuda", seed=1, len_div=16.0)               # d = 2048, V = 151936, T ~ 1.2k
+    ctx = make_ctx(b)
+    try:
+        ent = torch.zeros(b.T, dtype=torch.float32, device="cuda")
+        ctx.grpo_set_entropy_out(ent)
+        run_cuda(ctx, b, want_dw=False, want_dh=False)
+    finally:
+        ctx.close()
+    rows = np.unique(np.concatenate([[0, 127, 128, b.T - 1], np.random.default_rng(0).choice(b.T, 24, replace=False)]))
+    x = b.numpy_f64()
+    ref = token_entropy(x["H"][rows], x["W"])
+    assert np.abs(to64(ent)[rows] - ref).max() <= 2e-3
+    assert 11.0 < ref.min() and ref.max() < np.log(151936.0)              # near-uniform synthetic softmax
