@@ -34,13 +34,14 @@ constexpr int kABytes = BM * BK * 2;        // 16 KB
 constexpr int kGemmThreads = 224;
 constexpr int kProducerWarp = 4, kMmaWarp = 5, kGateWarp = 6;
 constexpr int kTmemCols = 512;
+constexpr int kRedStageBytes = 4 * 32 * 32 * 4;   // A6 epilogue: one 32 x 32 fp32 block per epilogue warp (16 KB)
 constexpr int kMaxTilesSmem = 1024;         // active-tile indices the A6 producer keeps in shared memory
 template <int CG> struct GemmShape {
   static constexpr int kBRows = BN / CG;                       // B rows (N index) staged by one CTA
   static constexpr int kBBytes = kBRows * BK * 2;              // 32 KB / 16 KB
   static constexpr int kStageBytes = kABytes + kBBytes;        // 48 KB / 32 KB
   static constexpr int kStages = CG == 1 ? 4 : 6;
-  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/ +
+  static constexpr int kSmemBytes = kStages * kStageBytes + kRedStageBytes + 1024 /*align slack*/ + 256 /*barriers*/ +
                                     kMaxTilesSmem * 4 /*A6 tile list*/;
 };
 constexpr float kLog2e = 1.4426950408889634f;
@@ -184,7 +185,7 @@ __device__ __forceinline__ void st_volatile_shared_i32(int* p, int v) {
 template <int CG, bool A_MN, bool B_MN, int EPI>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                 const GemmParams p, const int n_units_dense) {
+                 const __grid_constant__ CUtensorMap tmC, const GemmParams p, const int n_units_dense) {
   using Shape = GemmShape<CG>;
   constexpr int kStages = Shape::kStages;
   constexpr int kStageBytes = Shape::kStageBytes;
@@ -195,7 +196,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   const uint32_t pad = (1024u - (raw_addr & 1023u)) & 1023u;
   uint8_t* smem = smem_raw + pad;
   const uint32_t tiles_addr = raw_addr + pad;
-  GemmBarriers* bars = reinterpret_cast<GemmBarriers*>(smem + kStages * kStageBytes);
+  GemmBarriers* bars = reinterpret_cast<GemmBarriers*>(smem + kStages * kStageBytes + kRedStageBytes);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -515,12 +516,22 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                                  pack_bf16x2(v[g * 8 + 6], v[g * 8 + 7]));
               }
             }
-          } else {  // EPI_RED_F32: C += acc (fp32, atomic so launches on other streams may accumulate too)
-            if (row_ok) {
-              float* dst = reinterpret_cast<float*>(p.c_out) + static_cast<int64_t>(row_local) * p.c_pitch + cbase;
+          } else {  // EPI_RED_F32: C += acc.  The warp's 32 x 32 fp32 block goes through shared memory (128B-swizzled,
+            // conflict-free 16-byte stores) and ONE TMA reduce-add: whole 128-byte lines are reduced at L2 instead
+            // of 256 scattered 16-byte red.global per block, rows / columns out of range are clipped by the TMA
+            // unit, and launches on other streams may accumulate into the same dW concurrently (atomic at L2).
+            const uint32_t red_buf = tiles_addr + kStages * kStageBytes + quad * 4096;
+            if (lane == 0) tma_store_wait_read<0>();            // the previous block has been read out of red_buf
+            __syncwarp();
 #pragma unroll
-              for (int g = 0; g < 8; ++g)
-                if (g * 4 < nvalid) red_add_v4_f32(dst + g * 4, v[g * 4], v[g * 4 + 1], v[g * 4 + 2], v[g * 4 + 3]);
+            for (int j = 0; j < 8; ++j)
+              st_shared_v4_f32(red_buf + lane * 128 + ((j ^ (lane & 7)) << 4), v[4 * j], v[4 * j + 1], v[4 * j + 2],
+                               v[4 * j + 3]);
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+              tma_reduce_add_2d(&tmC, red_buf, cbase, (m_tile * CG + static_cast<int>(cta_rank)) * BM + quad * 32);
+              tma_store_commit();
             }
           }
         }
@@ -535,6 +546,9 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         if (acc == 0) acc_phase ^= 1;
       }
 
+      if constexpr (EPI == EPI_RED_F32) {
+        if (lane == 0) tma_store_wait<0>();                     // this unit's reductions are complete
+      }
       if constexpr (is_lse(EPI)) {
         if (row_ok) {
           const int split = u / p.m_tiles;

@@ -187,6 +187,23 @@ static int32_t make_tmap(const grpo_ctx* ctx, CUtensorMap* m, const void* base, 
   return GRPO_OK;
 }
 
+// fp32 C tensor [outer, inner] for the A6 epilogue's TMA reduce-add: 32 x 32 boxes (128-byte rows), 128B swizzle.
+static int32_t make_tmap_c_f32(const grpo_ctx* ctx, CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer,
+                               uint64_t pitch_bytes) {
+  if ((reinterpret_cast<uintptr_t>(base) & 15) != 0 || (pitch_bytes & 15) != 0)
+    return fail(GRPO_ERR_SHAPE, "dW base/pitch not 16-byte aligned (base %p pitch %llu)", base,
+                (unsigned long long)pitch_bytes);
+  cuuint64_t dims[2] = {inner, outer};
+  cuuint64_t strides[1] = {pitch_bytes};
+  cuuint32_t box[2] = {32, 32};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(GRPO_ERR_CUDA, "cuTensorMapEncodeTiled (fp32 C) failed with CUresult %d", (int)r);
+  return GRPO_OK;
+}
+
 static void set_desc_defaults(GemmParams& p, bool a_mn, bool b_mn) {
   // K-major SW128: 8-row groups 1024 B apart, +32 B per 16-element k step inside the 128 B row.
   // MN-major SW128: 64-element MN groups 8192 B apart (one TMA box), 8-row k groups 1024 B apart,
@@ -197,7 +214,7 @@ static void set_desc_defaults(GemmParams& p, bool a_mn, bool b_mn) {
 
 template <int CG, bool A_MN, bool B_MN, int EPI>
 static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                              const GemmParams& p, int n_units, cudaStream_t st) {
+                              const GemmParams& p, int n_units, cudaStream_t st, const CUtensorMap* tmC) {
   static bool attr_set = false;
   auto kern = grpo_gemm_kernel<CG, A_MN, B_MN, EPI>;
   constexpr int smem = GemmShape<CG>::kSmemBytes;
@@ -239,7 +256,7 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   lc.numAttrs = 1;
   {
     LaunchScope ls(ctx, kind, st);
-    CU_OK(cudaLaunchKernelEx(&lc, kern, tmA, tmB, pl, n_units));
+    CU_OK(cudaLaunchKernelEx(&lc, kern, tmA, tmB, tmC ? *tmC : tmA, pl, n_units));
   }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
@@ -247,9 +264,10 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
 
 template <bool A_MN, bool B_MN, int EPI>
 static int32_t launch_gemm(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
-                           int n_units, cudaStream_t st) {
-  if (ctx->cg == 2) return launch_gemm_cg<2, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st);
-  return launch_gemm_cg<1, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st);
+                           int n_units, cudaStream_t st, const CUtensorMap* tmC = nullptr) {
+  if (EPI == EPI_RED_F32 && tmC == nullptr) return fail(GRPO_ERR_INVALID_ARG, "EPI_RED_F32 needs the C tensor map");
+  if (ctx->cg == 2) return launch_gemm_cg<2, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
+  return launch_gemm_cg<1, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
 }
 
 static int choose_n_split(int m_tiles, int n_tiles, int sms, int64_t max_split) {
@@ -686,7 +704,9 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.n_fastest = 1;
       p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.tile_list = tile_list;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
-      GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_GEMM_DW, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st)));
+      CUtensorMap tmDW;
+      GRPO_TRY(make_tmap_c_f32(ctx, &tmDW, dW_accum, c.d, c.V, static_cast<uint64_t>(c.d) * 4));
+      GRPO_TRY((launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_GEMM_DW, tmDZ_mn, tmH_mn, p, p.m_tiles * p.n_tiles, st, &tmDW)));
     }
   }
   return GRPO_OK;
@@ -1076,14 +1096,17 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   else GRPO_TRY(make_tmap(ctx, &tmA, A, M, K, static_cast<uint64_t>(M) * 2, 64, BK));
   if (!b_mn) GRPO_TRY(make_tmap(ctx, &tmB, B, K, N, static_cast<uint64_t>(K) * 2, BK, BN / ctx->cg));
   else GRPO_TRY(make_tmap(ctx, &tmB, B, N, K, static_cast<uint64_t>(N) * 2, 64, BK));
+  CUtensorMap tmCm;
+  if (accumulate) GRPO_TRY(make_tmap_c_f32(ctx, &tmCm, C, N, M, static_cast<uint64_t>(N) * 4));
+  const CUtensorMap* tmC = accumulate ? &tmCm : nullptr;
   if (layout == 0) {
-    if (accumulate) return launch_gemm<false, false, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
+    if (accumulate) return launch_gemm<false, false, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st, tmC);
     return launch_gemm<false, false, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   } else if (layout == 1) {
-    if (accumulate) return launch_gemm<false, true, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
+    if (accumulate) return launch_gemm<false, true, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st, tmC);
     return launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   } else if (layout == 2) {
-    if (accumulate) return launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
+    if (accumulate) return launch_gemm<true, true, EPI_RED_F32>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st, tmC);
     return launch_gemm<true, true, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   }
   return fail(GRPO_ERR_INVALID_ARG, "layout must be 0, 1 or 2");
