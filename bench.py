@@ -38,7 +38,7 @@ REF_SAMPLE_LEN_DIV = 32.0      # --impl reference arm: T ~ 580 tokens per step
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"gemm_lse": 0.726e9, "gemm_dz": 3.519e9, "gemm_dh": 5.600e9, "gemm_dw": 7.839e9}   # profiles/r01e_ncu_gemm.md
+NCU_TRAFFIC_BYTES = {"gemm_lse": 2.188e9, "gemm_dz": 3.543e9, "gemm_dh": 5.599e9, "gemm_dw": 7.855e9}   # profiles/r01f_ncu_gemm.md
 
 
 def load_peaks():
