@@ -11,7 +11,11 @@ no KL.  With N>1 (torchrun, one rank per GPU) every rank runs its own complete g
 independent groups; the path has no collective — DESIGN.md §7); the only torch.distributed traffic is
 the barrier and the max/sum of the measurements.
 
-Output: ONE JSON line on rank 0 (keys documented in DESIGN.md §6).
+Output: ONE JSON line on rank 0 (keys documented in DESIGN.md §6).  The headline `value` is always the north_star
+path (forward, then the backward that recomputes the logits chunk by chunk); `other_variant` times the
+3-contraction variant beside it.  Informational switches: `--stash` (make that variant the step),
+`--config 3|4|5` (the other BASELINE configs, device-resident), `--cgp-mode per_group|batch4` (configs[4] streamed
+through grpo_enqueue_groups), `--no-tile-skip`, `--no-drift-gate`, `--cta-group 1`, `--bwd-chunk N` (A/B runs).
 `--impl reference` times the float64 CPU oracle (oracle/) on the host cores, on a bounded sample.
 """
 from __future__ import annotations
