@@ -245,3 +245,35 @@ def test_paper_trend_cgp_gain_grows_with_R(rp):
         gains.append(1.0 - f["t_train_end"] / s["t_train_end"])
     assert gains[0] < gains[1] < gains[2]
     assert 0.2 < gains[2] < 0.5
+
+
+def test_abi_matches_oracle_on_random_small_rounds(rp):
+    """Property test: random small rounds (ties between completion times included: integer works, zero-length
+    responses, equal materialization latencies) — every output of the C++ model equals the oracle's."""
+    from hypothesis import given, settings, strategies as st
+
+    @settings(max_examples=150, deadline=None)
+    @given(st.integers(1, 9), st.integers(1, 4), st.integers(1, 4), st.integers(0, 5), st.sampled_from([0.0, 3.0]),
+           st.integers(0, 2 ** 31 - 1))
+    def check(R, K, U, F_w, cap, seed):
+        rng = np.random.default_rng(seed)
+        work = rng.integers(0, 6, size=(R, K)).astype(np.float64)
+        mat = rng.integers(0, 3, size=R).astype(np.float64)
+        train = rng.integers(1, 4, size=R).astype(np.float64)
+        rd_o, gd_o, _ = O.rollout(work, 7.0, cap, F_w)
+        rd, gd, _ = rp.rp_rollout(work, 7.0, cap, F_w)
+        np.testing.assert_allclose(rd, rd_o, rtol=1e-10, atol=1e-9)
+        np.testing.assert_allclose(gd, gd_o, rtol=1e-10, atol=1e-9)
+        for mode in (O.MODE_SLIME, O.MODE_CGP, O.MODE_CGP_FGD):
+            # feed both timelines the oracle's trainable times so that ties are broken on identical inputs
+            trainable = (O.rollout(work, 7.0, cap, F_w if mode == O.MODE_CGP_FGD else 0)[1] + mat)
+            o = O.cgp_timeline(trainable, train, U, mode)
+            c = rp.rp_cgp_timeline(trainable, train, U, mode)
+            assert c["fifo_order"] == o.fifo_order
+            np.testing.assert_allclose(c["start"], o.start, rtol=1e-12, atol=1e-12)
+            np.testing.assert_allclose(c["end"], o.end, rtol=1e-12, atol=1e-12)
+            for k in ("t_first_U", "t_complete", "dt_cgp", "t_start", "t_train_end", "compute", "wait"):
+                assert c[k] == pytest.approx(getattr(o, k), rel=1e-12, abs=1e-12), k
+            assert o.t_train_end >= o.t_complete - 1e-12 or R == 0          # training cannot end before the rollout
+
+    check()
