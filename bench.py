@@ -464,6 +464,9 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         if k in GEMM_KINDS:
             e["tflops"] = kind_flops[k] * steps / (v["ms"] * 1e-3) / 1e12
             e["frac_of_peak"] = e["tflops"] / peak
+        if k == "loss" and world == 1 and args.config == 2 and not args.stash:
+            # A3 reads / writes >= 56 B per token (one LSE split); launch-latency bound at this size
+            e["gbps_at_least"] = 56.0 * T * steps / (v["ms"] * 1e-3) / 1e9
         if k == "stash_dz":     # HBM-bound: 2 B read + 2 B written per logit of the walked rows
             e["gbps"] = 4.0 * T * V * act * steps / (v["ms"] * 1e-3) / 1e9
             e["frac_of_hbm_peak"] = e["gbps"] / float(peaks["hbm_gbs"])
