@@ -165,3 +165,18 @@ def test_step_host_matches_device_path():
     np.testing.assert_allclose(loss_h.item(), out["loss"].item(), rtol=1e-5)
     assert torch.equal(dh_h, out["dH"].cpu())
     assert rel_l2(to64(dW), to64(out["dW"])) < 1e-5
+
+
+@pytest.mark.parametrize("d,V", [(72, 1003), (8, 9), (200, 257), (136, 5001)])
+@pytest.mark.parametrize("fused", [False, True])
+def test_odd_shapes(d, V, fused):
+    """Widths that are not multiples of the 64-element K block (only d % 8 == 0 is required) and odd vocabulary
+    sizes: K tails, partial 16-byte vectors at the row ends, V smaller than one tile; both backward variants."""
+    b = make_config(1, device="cuda", seed=21, variant="1b", d=d, V=V, w_std=0.3)
+    ctx = make_ctx(b, dhidden_fp32=1, bwd_chunk_tokens=128)
+    try:
+        out = run_cuda(ctx, b, fused=fused)
+        assert ctx.grpo_check_errors_sync() == 0
+    finally:
+        ctx.close()
+    assert_gates(gates(b, out, run_oracle(b)))
