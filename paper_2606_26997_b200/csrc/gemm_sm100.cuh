@@ -3,10 +3,15 @@
 //
 //   warps 0..3  : epilogue       (tcgen05.ld 32x32b: one accumulator row per thread; warp w owns TMEM lanes 32w..)
 //   warp 4      : TMA producer   (cp.async.bulk.tensor -> 128B-swizzled smem ring, mbarrier complete_tx)
-//   warp 5      : MMA issuer     (one elected thread: tcgen05.mma kind::f16, fp32 accumulators in TMEM, 2 stages)
-//   warp 6      : drift gate     (one thread polls the launch's epoch counters, see drift_gate_*)
-// The two single-thread roles have the highest warp ids of their scheduler partitions, so the arbiter
-// (highest warp id first) never parks them behind a busy epilogue warp.
+//   warp 5      : MMA issuer     (tcgen05.mma kind::f16, fp32 accumulators in TMEM, 2 accumulator stages)
+//   warp 6      : drift gate     (one thread polls the launch's epoch counters, see "Drift bound" below)
+// Producer and MMA warps walk their loops with all 32 lanes converged and ONE elected lane issuing, so that
+// addresses, coordinates and descriptors are warp-uniform (uniform registers; a lane-0-only producer loop paid
+// an ELECT + four R2UR.BROADCAST per TMA instruction and starved the tensor pipe).  The two issuing warps have
+// the highest warp ids of their scheduler partitions, so the arbiter never parks them behind an epilogue warp.
+//
+// Shared memory: ring stages | 16 KB staging for the A6 epilogue (one 32 x 32 fp32 block per epilogue warp,
+// reduced into dW by a TMA reduce-add) | barriers + the A6 producer's copy of the active-tile list.
 //
 // CG = 1: one CTA per SM, C tile = 128 x 256, K block = 64 bf16 (one 128-byte swizzle row), 4-stage
 //         smem ring of 48 KB stages.
