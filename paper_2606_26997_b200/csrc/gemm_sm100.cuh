@@ -65,8 +65,6 @@ struct GemmParams {
   int m_tiles, n_tiles, k_blocks;
   int n_fastest;                     // unit order: 1 = n tile fastest (A5/A6), 0 = m tile fastest (A2/A4)
   int n_split, tiles_per_split;      // EPI_LSE: a unit is (m tile, contiguous range of n tiles)
-  uint32_t lbo_a, sbo_a, kadv_a;     // smem descriptor constants (bytes); see make_smem_desc
-  uint32_t lbo_b, sbo_b, kadv_b;
   // per-token arrays are indexed by (row_offset + local row)
   int64_t row_offset;
   const int32_t* targets;

@@ -204,13 +204,6 @@ static int32_t make_tmap_c_f32(const grpo_ctx* ctx, CUtensorMap* m, const void* 
   return GRPO_OK;
 }
 
-static void set_desc_defaults(GemmParams& p, bool a_mn, bool b_mn) {
-  // K-major SW128: 8-row groups 1024 B apart, +32 B per 16-element k step inside the 128 B row.
-  // MN-major SW128: 64-element MN groups 8192 B apart (one TMA box), 8-row k groups 1024 B apart,
-  // +2048 B per 16-row k step.
-  p.lbo_a = a_mn ? 8192 : 16; p.sbo_a = 1024; p.kadv_a = a_mn ? 2048 : 32;
-  p.lbo_b = b_mn ? 8192 : 16; p.sbo_b = 1024; p.kadv_b = b_mn ? 2048 : 32;
-}
 
 template <int CG, bool A_MN, bool B_MN, int EPI>
 static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB,
@@ -499,7 +492,6 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
   GRPO_TRY(make_tmap(ctx, &tmW, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN / ctx->cg));
   GemmParams p;
   std::memset(&p, 0, sizeof(p));
-  set_desc_defaults(p, false, false);
   p.m_total = static_cast<int>(rows);
   p.n_total = c.V;
   p.m_tiles = static_cast<int>((rows + TM - 1) / TM);
@@ -663,7 +655,6 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     } else {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
-      set_desc_defaults(p, false, false);
       p.m_total = static_cast<int>(rows); p.n_total = c.V;
       p.m_tiles = m_tiles; p.n_tiles = (c.V + BN - 1) / BN; p.k_blocks = (c.d + BK - 1) / BK;
       p.n_fastest = 0;
@@ -677,7 +668,6 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d]
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
-      set_desc_defaults(p, false, true);
       p.m_total = static_cast<int>(rows); p.n_total = c.d;
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
       p.n_fastest = 1;
@@ -697,7 +687,6 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       GRPO_TRY(make_tmap(ctx, &tmH_mn, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, 64, BK));
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
-      set_desc_defaults(p, true, true);
       p.m_total = c.V; p.n_total = c.d;
       p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
@@ -1091,7 +1080,6 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   if (ctx->ws) p.sync = slot_ptr<unsigned int>(ctx, 0, ctx->lay.off_sync);
   const int units = p.m_tiles * p.n_tiles;
   const bool a_mn = layout == 2, b_mn = layout >= 1;
-  set_desc_defaults(p, a_mn, b_mn);
   if (!a_mn) GRPO_TRY(make_tmap(ctx, &tmA, A, K, M, static_cast<uint64_t>(K) * 2, BK, BM));
   else GRPO_TRY(make_tmap(ctx, &tmA, A, M, K, static_cast<uint64_t>(M) * 2, 64, BK));
   if (!b_mn) GRPO_TRY(make_tmap(ctx, &tmB, B, K, N, static_cast<uint64_t>(K) * 2, BK, BN / ctx->cg));
