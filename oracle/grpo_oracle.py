@@ -17,6 +17,10 @@ Passages followed:
   * k3 KL, masked token mean, backward (softmax - onehot) * coeff ...... north_star
   * gradients only accumulated across groups of a logical update ..... PAPER.md:111
 
+NEXT-2 switches (paper silent; R26-R28): k1 / k2 KL estimators, dual clip, per-token entropy —
+pinned in tests/test_oracle_variants.py (E[k1] = E[k3] = KL, derivative checks, a hand-evaluated dual-clip
+table, finite differences, torch autograd, closed-form / library entropies); "parity unpinned" by the paper.
+
 Pins (tests/test_oracle_pins.py): P1-P14 of SURVEY.md §8(c).  The paper prints no
 worked number for the loss, so every pin is a closed form, invariant, library special
 case, finite difference or brute force.  Unpinned by the paper: everything except
