@@ -40,9 +40,40 @@ UNIT = "tokens/s"
 SAMPLE_LEN_DIV = 8.0           # cpu_baseline leg: T ~ 2.3k tokens
 REF_SAMPLE_LEN_DIV = 32.0      # --impl reference arm: T ~ 580 tokens per step
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"gemm_lse": 2.188e9, "gemm_dz": 3.543e9, "gemm_dh": 5.599e9, "gemm_dw": 7.855e9}   # profiles/r01f_ncu_gemm.md
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.txt")
+KERNEL_SOURCES = ("gemm_sm100.cuh", "ptx_sm100.cuh", "token_kernels.cuh", "grpo_api.cu")
+
+
+def kernel_source_hash():
+    """sha256 over the CUDA sources: identifies the build an ncu capture belongs to."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2606_26997_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def load_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each contraction kernel, from the committed
+    `ncu --set full` capture (profiles/r02_traffic.txt: `key value` lines, written from the capture's raw page).
+    The capture names the source hash of the build it profiled; a capture of ANOTHER build is not reported as this
+    build's traffic: the figure is dropped (null) and the mismatch is said on stderr and in the JSON line."""
+    if not os.path.exists(TRAFFIC_FILE):
+        return {}, "no ncu capture committed for this build"
+    vals = {}
+    with open(TRAFFIC_FILE) as f:
+        for line in f:
+            line = line.split("#")[0].split()
+            if len(line) == 2:
+                vals[line[0]] = line[1]
+    have = kernel_source_hash()
+    if vals.get("kernel_source_hash") != have:
+        msg = (f"profiles/r02_traffic.txt is a capture of build {vals.get('kernel_source_hash')}, this build is {have}: "
+               "roofline.traffic dropped (re-run the ncu capture)")
+        print("bench.py: " + msg, file=sys.stderr)
+        return {}, msg
+    return {k: float(v) for k, v in vals.items() if k.startswith("gemm_")}, "profiles/r02_traffic.txt"
 
 
 def load_peaks():
@@ -92,6 +123,10 @@ class ClockSampler:
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
                 try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
+                except Exception:
+                    pass
+                try:
                     self.mask |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
                 except Exception:
                     self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
@@ -99,8 +134,16 @@ class ClockSampler:
                 pass
             self._stop.wait(self.period)
 
+    def energy_mj(self):
+        """NVML total energy counter of the board in millijoules (None if unavailable)."""
+        try:
+            return int(self.nv.nvmlDeviceGetTotalEnergyConsumption(self.h))
+        except Exception:
+            return None
+
     def start(self):
         if self.h is not None:
+            self.power = []
             self._thr = threading.Thread(target=self._run, daemon=True)
             self._thr.start()
 
@@ -111,8 +154,11 @@ class ClockSampler:
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
         reasons = [name for bit, name in self.REASONS.items() if self.mask & bit]
-        return {"sm_mhz": int(statistics.median(self.samples)), "sm_max_mhz": self.max_mhz,
-                "sm_min_mhz": min(self.samples), "samples": len(self.samples), "reasons": reasons}
+        out = {"sm_mhz": int(statistics.median(self.samples)), "sm_max_mhz": self.max_mhz,
+               "sm_min_mhz": min(self.samples), "samples": len(self.samples), "reasons": reasons}
+        if getattr(self, "power", None):
+            out["power_w_median"] = round(statistics.median(self.power), 1)
+        return out
 
 
 # ----------------------------------------------------------------------------------------- oracle legs
@@ -236,6 +282,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.sweep_T:
+        assert world == 1, "--sweep-T is a one-GPU informational run"
+        return run_sweep_T(args, dev)
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
     b = make_config(args.config, seed=rank_seed(rank), device=dev)
     if args.cgp_mode != "full":
@@ -274,11 +323,10 @@ def run_ours(args):
     dW.zero_()
     loss.zero_()
 
-    # ---- timed region: K steps, CUDA events on the launch stream, per-kernel events inside the library
+    # ---- timed region (the headline): K steps, CUDA events on the launch stream; the library's per-kernel
+    # profiling events are OFF here
     sampler = ClockSampler(local)
-    ctx.grpo_bwd_tile_stats_sync()          # clear
     n0 = ctx.grpo_kernel_launches()
-    ctx.grpo_profile_enable(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     sampler.start()
@@ -290,15 +338,55 @@ def run_ours(args):
     clocks = sampler.stop()
     barrier()
     ms_total = e0.elapsed_time(e1)
-    prof = ctx.grpo_profile_read_sync()
-    ctx.grpo_profile_enable(False)
-    tiles_walked, tiles_total = ctx.grpo_bwd_tile_stats_sync()
-    args.bwd_active_frac = tiles_walked / tiles_total if tiles_total > 0 else 1.0
-    args.bwd_tiles = {"walked": tiles_walked, "total": tiles_total}
     n1 = ctx.grpo_kernel_launches()
     launches = sum(n1.values()) - sum(n0.values())
     loss_val = loss.item()
     assert loss_val == loss_val, "loss is NaN"
+
+    # ---- the same K steps once more with a CUDA event pair around every kernel launch (recorded by the library on
+    # the launch stream): per-kernel times for the roofline; the pass's own total is reported beside the headline
+    ctx.grpo_bwd_tile_stats_sync()          # clear
+    ctx.grpo_bwd_row_stats_sync()
+    ctx.grpo_profile_enable(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    p0.record()
+    for _ in range(args.steps):
+        step()
+    p1.record()
+    torch.cuda.synchronize()
+    barrier()
+    args.profiled_ms_per_step = p0.elapsed_time(p1) / args.steps
+    prof = ctx.grpo_profile_read_sync()
+    ctx.grpo_profile_enable(False)
+    rows_walked, rows_total = ctx.grpo_bwd_row_stats_sync()
+    tiles_walked, tiles_total = ctx.grpo_bwd_tile_stats_sync()
+    if args.stash:
+        args.bwd_active_frac = tiles_walked / tiles_total if tiles_total > 0 else 1.0
+    else:
+        args.bwd_active_frac = rows_walked / rows_total if rows_total > 0 else 1.0
+    args.bwd_rows = {"walked": rows_walked, "total": rows_total, "tiles_walked_stash": tiles_walked,
+                     "tiles_total_stash": tiles_total}
+
+    # ---- energy: NVML's board energy counter around a >= 2 s run of the same step (the counter is too coarse
+    # for the 0.35 s headline region); joules per step, mean power, tokens per joule
+    args.energy = None
+    if world == 1 and not args.no_energy:
+        n_e = max(args.steps, int(2000.0 / max(ms_total / args.steps, 1e-3)) + 1)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        mj0 = sampler.energy_mj() if sampler.h is not None else None
+        g0.record()
+        for _ in range(n_e):
+            step()
+        g1.record()
+        torch.cuda.synchronize()
+        mj1 = sampler.energy_mj() if sampler.h is not None else None
+        if mj0 is not None and mj1 is not None and mj1 > mj0:
+            sec = g0.elapsed_time(g1) * 1e-3
+            joules = (mj1 - mj0) * 1e-3
+            args.energy = {"joules_per_step": joules / n_e, "mean_power_w": joules / sec, "tokens_per_joule": T * n_e / joules,
+                           "steps": n_e, "tokens_per_s": T * n_e / sec, "source": "nvmlDeviceGetTotalEnergyConsumption"}
 
     # ---- the other variant of the step, timed the same way (reported beside the headline, never as it)
     args.other_variant = None
@@ -372,6 +460,66 @@ def run_ours(args):
     ctx.close()
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+SWEEP_T = (2000, 4000, 8000, 10000, 16000, 18701, 24000, 33000)
+
+
+def run_sweep_T(args, dev):
+    """Informational (one JSON line): tokens/s of ONE complete group per launch at T ~ 2k .. 33k tokens - the range
+    configs[1] draws from (8 responses of 512..4096 tokens) and the regime CGP feeds, one launch per arriving group
+    (PAPER.md:92).  Same recipe as configs[1] with the response lengths rescaled; device-resident; north_star path
+    and the 3-contraction variant."""
+    import torch
+    from paper_2606_26997_b200 import GrpoContext
+    from workloads.synth import make_config
+    rows = []
+    ctx = None
+    for T_target in SWEEP_T:
+        b = make_config(2, seed=0, device=dev, len_div=18701.0 / T_target)
+        if ctx is None:
+            ctx = GrpoContext(b.d, b.V, max_tokens=int(max(SWEEP_T) * 1.1), group_size=b.G, kl_beta=b.kl_beta,
+                              clip_lo=b.clip_lo, clip_hi=b.clip_hi)
+        dW = torch.zeros(b.V, b.d, dtype=torch.float32, device=dev)
+        loss = torch.zeros(1, dtype=torch.float32, device=dev)
+        dH = torch.empty(b.T, b.d, dtype=torch.bfloat16, device=dev)
+
+        def step_recompute():
+            adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+            f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                                b.mask, loss_accum=loss)
+            ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW, dhidden_out=dH)
+
+        def step_stash():
+            adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+            ctx.grpo_fused_logprob_loss_fwd_bwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                                b.mask, loss_accum=loss, dW_accum=dW, dhidden_out=dH)
+
+        row = {"T": b.T}
+        for name, fn in (("recompute", step_recompute), ("stash", step_stash)):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            n = max(args.steps, int(300.0 * 18701 / b.T / 35.0) + 1)      # ~0.3 s per point
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(n):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / n
+            row[name] = {"tokens_per_s": b.T / (ms * 1e-3), "ms_per_step": ms, "steps": n}
+        rows.append(row)
+        del dW, dH, b
+    ref = next(r for r in rows if abs(r["T"] - 18701) < 200)
+    for r in rows:
+        r["recompute"]["vs_T18701"] = r["recompute"]["tokens_per_s"] / ref["recompute"]["tokens_per_s"]
+        r["stash"]["vs_T18701"] = r["stash"]["tokens_per_s"] / ref["stash"]["tokens_per_s"]
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "informational": "sweep_T", "n_gpus": 1, "dtype": "bf16",
+                      "data": "synthetic", "config": {"workload": "configs[1] recipe, one complete group G=8 per launch, "
+                      "response lengths rescaled to T tokens; d=2048, V=151936"}, "sweep_T": rows}), flush=True)
+    ctx.close()
     return 0
 
 
@@ -472,18 +620,21 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
             e["frac_of_hbm_peak"] = e["gbps"] / float(peaks["hbm_gbs"])
         kernels[k] = e
     gemm_ms = sum(prof[k]["ms"] for k in GEMM_KINDS)
+    traffic, traffic_src = load_traffic()
     dom = max(GEMM_KINDS, key=lambda k: prof[k]["ms"])
     dom_tflops = kernels[dom]["tflops"]
     exec_flops = sum(kind_flops.values())
     path_tflops = exec_flops * steps / (gemm_ms * 1e-3) / 1e12
     step_tflops = exec_flops * steps / (ms_total * 1e-3) / 1e12 if world == 1 else None
+    prof_total = getattr(args, "profiled_ms_per_step", None)
+    gemm_share = gemm_ms / (prof_total * steps) if prof_total else gemm_ms / ms_total
     roofline = {
         "bound": "tensor", "kernel": dom, "achieved": dom_tflops, "peak": peak, "unit": "TFLOP/s",
-        "frac": dom_tflops / peak, "traffic": NCU_TRAFFIC_BYTES.get(dom),
+        "frac": dom_tflops / peak, "traffic": traffic.get(dom), "traffic_source": traffic_src,
         "peak_source": f"{peaks['_source']} bf16_tflops_sustained (MEASURED_PEAKS.json); burst {peak_burst:g}",
         "frac_of_burst": dom_tflops / peak_burst,
         "flops_per_launch": kind_flops[dom] / kernels[dom]["launches_per_step"],
-        "all_gemms": {"achieved": path_tflops, "frac": path_tflops / peak, "share_of_step": gemm_ms / ms_total},
+        "all_gemms": {"achieved": path_tflops, "frac": path_tflops / peak, "share_of_step": gemm_share},
         "whole_step": None if step_tflops is None else {"achieved": step_tflops, "frac": step_tflops / peak,
                                                         "flops_basis": "executed: 2*T*V*d (A2) + 2*T_walked*V*d per backward "
                                                                        "contraction (3 recompute / 2 stash); 8*T*V*d for "
@@ -503,7 +654,9 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         "e2e": None if e2e_value is None else {
             "value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "api": "grpo_step_host (C ABI, pinned host buffers; W and dW resident on the device)"},
-        "bwd_tiles": getattr(args, "bwd_tiles", None),
+        "bwd_rows": getattr(args, "bwd_rows", None),
+        "profiled_ms_per_step": getattr(args, "profiled_ms_per_step", None),
+        "energy": getattr(args, "energy", None),
         "other_variant": getattr(args, "other_variant", None),
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
         "loss_after_steps": loss_val,
@@ -532,14 +685,22 @@ def main():
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
+    ap.add_argument("--no-energy", action="store_true", help="skip the >= 2 s NVML energy leg (profiling runs)")
+    ap.add_argument("--sweep-T", action="store_true",
+                    help="informational: single-group launches (configs[1] recipe, lengths rescaled) at "
+                         "T ~ 2k .. 33k tokens, the range CGP feeds one complete group at a time (PAPER.md:92)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.gpus != world:
-        if world == 1 and args.gpus > 1:
-            raise SystemExit(f"bench.py --gpus {args.gpus}: launch with torch.distributed.run --nproc-per-node "
-                             f"{args.gpus} (one rank per GPU)")
+    if args.gpus > 1 and world == 1 and "RANK" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start one rank per GPU ourselves (the same command the
+        # driver uses) and let rank 0 print the line
+        import subprocess
+        port = 29500 + (os.getpid() % 2000)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
     return run_ours(args)
 
 

@@ -76,11 +76,13 @@ typedef struct {
                                 1 = k1 = logp - ref, 2 = k2 = (logp - ref)^2 / 2 */
   float   dual_clip;         /* 0 = off; c > 1: for A < 0 the surrogate is max(min(rho A, clip(rho) A), c A)
                                 (R27) */
-  int32_t bwd_skip_zero_tiles; /* 0 = default (on), < 0 = off.  The backward skips every token tile whose
-                                coefficients dloss/dlogp are all exactly zero (zero-variance groups at
-                                kl_beta = 0, masked spans): their dHidden rows are written as zeros and they
-                                add nothing to dW, which is what the dense computation gives (DESIGN.md
-                                section 10).  Decided on the device; no host synchronisation. */
+  int32_t bwd_skip_zero_tiles; /* 0 = default (on), < 0 = off.  The backward skips every token whose coefficient
+                                dloss/dlogp is exactly zero (masked or ignored tokens; at kl_beta = 0 also clipped
+                                tokens, and zero-variance groups): the remaining rows are compacted
+                                on the device and A4-A6 run on the compact panel; skipped dHidden rows are
+                                written as zeros and add nothing to dW, which is what the dense computation
+                                gives.  The 3-contraction variant skips per 256-row token
+                                tile instead.  Decided on the device; no host synchronisation. */
   int32_t stash_logits;      /* 0 = default: grpo_enqueue_groups / grpo_step_host run forward then backward with
                                 the logits RECOMPUTED chunk by chunk (north_star, 4 contractions); 1 = they run
                                 grpo_fused_logprob_loss_fwd_bwd instead (3 contractions) */
@@ -124,6 +126,12 @@ int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const voi
                                     double loss_denom, float* logp_out, float* lse_out, float* coeff_out,
                                     float* loss_accum, float* metrics_accum, void* stream);
 
+/* loss_agg = 1 only (per-sequence mean, then mean over sequences): the number of sequences of the WHOLE logical
+ * update that later grpo_fused_logprob_loss_fwd / _fwd_bwd calls of this context divide by, for callers that cut
+ * one update into several calls (micro-batches); 0 (default) = each call's own S.  grpo_enqueue_groups does not
+ * use it: it counts the sequences of the update's groups itself (R10). */
+int32_t grpo_set_seq_denom(grpo_ctx* ctx, int32_t n_sequences);
+
 /* A4-A6.  lse, coeff from the forward.  grad_scale multiplies both gradients (upstream dLoss).
  * dhidden_out [T, d] (bf16, or fp32 if cfg.dhidden_fp32) is OVERWRITTEN; dW_accum fp32 [V, d] is
  * ADDED to with atomics (caller zeroes it at the optimizer boundary).  Either may be NULL to skip. */
@@ -131,7 +139,6 @@ int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden, const voi
                                     const float* lse, const float* coeff, int64_t T, float grad_scale,
                                     void* dhidden_out, float* dW_accum, void* stream);
 
-/* One COMPLETE group (PAPER.md:40: all K responses present, rewards verified). */
 /* Optional diagnostic output of the forward (R28): while a non-NULL
  * device pointer is set, every later grpo_fused_logprob_loss_fwd / _fwd_bwd call of this context also writes
  * entropy_out[t] = - sum_v p_tv log p_tv (nats) for each of its T packed rows (one more running sum in the A2
@@ -157,6 +164,7 @@ int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hidden, const
                                         float* coeff_out, float* loss_accum, float* metrics_accum, void* dhidden_out,
                                         float* dW_accum, void* stream);
 
+/* One COMPLETE group (PAPER.md:40: all K responses present, rewards verified). */
 typedef struct {
   int64_t group_order;          /* submission order; informational, FIFO is by arrival */
   int32_t G;                    /* responses in the group */
@@ -182,6 +190,11 @@ typedef struct {
  * HOST outputs: groups_consumed_out (total consumed so far), update_boundary_out (1 if an update was
  * run by this call: the caller may step the optimizer and zero dW once the streams reach this work).
  * n = 0 is allowed (continue draining the FIFO). */
+/* Errors leave the accumulators consistent: everything that can be rejected without the device (workspace
+ * capacity, ref_logp given for some groups of a launch only) is checked for EVERY launch of the update before the
+ * first kernel is enqueued - nothing is accumulated and the FIFO is unchanged.  If a launch fails later
+ * (GRPO_ERR_CUDA), the groups of the launches already enqueued are consumed (groups_consumed_out counts them) and
+ * the rest of the update stays at the head of the FIFO, so a retry never adds a group twice. */
 int32_t grpo_enqueue_groups(grpo_ctx* ctx, const grpo_group_desc* groups, int32_t n, const void* W,
                             float* dW_accum, float* loss_accum, float* metrics_accum, double loss_denom,
                             void* const* streams, int32_t n_streams, int32_t* groups_consumed_out,
@@ -229,12 +242,18 @@ enum {
   GRPO_KERNEL_DEBUG = 7,       /* grpo_debug_gemm */
   GRPO_KERNEL_TILE_SCAN = 8,   /* backward: zero-coefficient tile scan + zero fill of skipped dHidden rows */
   GRPO_KERNEL_STASH_DZ = 9,    /* 3-contraction variant: stashed logits -> dZ in place */
-  GRPO_NUM_KERNEL_KINDS = 10
+  GRPO_KERNEL_COMPACT = 10,    /* backward: zero-coefficient row compaction, gather of active rows, zero fill */
+  GRPO_KERNEL_DH_REDUCE = 11,  /* A5: fixed-order sum of the split-K partials (+ scatter of compacted rows) */
+  GRPO_NUM_KERNEL_KINDS = 12
 };
 
-/* Token tiles the backward calls of workspace slot 0 walked (active) and saw (total) since the last call
- * of this function; both 0 when bwd_skip_zero_tiles is off.  Synchronises. */
+/* Token tiles the 3-contraction backward calls of workspace slot 0 walked (active) and saw (total) since the last
+ * call of this function; both 0 when bwd_skip_zero_tiles is off.  Synchronises. */
 int32_t grpo_bwd_tile_stats_sync(grpo_ctx* ctx, int64_t* active_out /*HOST*/, int64_t* total_out /*HOST*/);
+
+/* Packed rows the north_star backward calls of all workspace slots ran A4-A6 over (active: coeff != 0) and saw
+ * (total) since the last call of this function; both 0 when bwd_skip_zero_tiles is off.  Synchronises. */
+int32_t grpo_bwd_row_stats_sync(grpo_ctx* ctx, int64_t* active_out /*HOST*/, int64_t* total_out /*HOST*/);
 
 /* counts_out HOST int64 [GRPO_NUM_KERNEL_KINDS]: kernels launched by this context since creation. */
 int32_t grpo_kernel_launches(const grpo_ctx* ctx, int64_t* counts_out);

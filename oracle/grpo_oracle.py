@@ -21,11 +21,17 @@ NEXT-2 switches (paper silent; R26-R28): k1 / k2 KL estimators, dual c
 pinned in tests/test_oracle_variants.py (E[k1] = E[k3] = KL, derivative checks, a hand-evaluated dual-clip
 table, finite differences, torch autograd, closed-form / library entropies); "parity unpinned" by the paper.
 
+NEXT-4 (R29-R31): the final RMSNorm in front of the path and its backward
+(``rmsnorm_fwd`` / ``rmsnorm_bwd`` / ``grpo_step_from_prenorm``) — pinned in tests/test_oracle_rmsnorm.py by a
+hand-worked example, ``torch.nn.functional.rms_norm`` and its autograd, scale invariance / orthogonality
+identities and finite differences of the whole step w.r.t. the pre-norm activations and the norm weight;
+"parity unpinned" by the paper (it never mentions the norm).
+
 Pins (tests/test_oracle_pins.py): P1-P14 of SURVEY.md §8(c).  The paper prints no
 worked number for the loss, so every pin is a closed form, invariant, library special
 case, finite difference or brute force.  Unpinned by the paper: everything except
-Eq. 1 — pinned here by P4-P14 only.  ``metrics`` (clip fraction etc.) are checked
-against brute-force loops only: "parity unpinned" beyond that.
+Eq. 1 — pinned here by P4-P14 only.  ``metrics`` (clip fraction etc.) are pinned by a five-token
+case worked by hand (test_metrics_and_loss_hand_evaluated_five_tokens) and by brute-force loops.
 """
 from __future__ import annotations
 
@@ -37,6 +43,7 @@ __all__ = [
     "OracleConfig", "bf16_bits_to_f64", "group_advantage", "token_advantage",
     "token_logprobs", "loss_terms", "backward", "grpo_step", "grpo_step_loops",
     "token_rows", "dH_rows", "dW_rows", "token_entropy",
+    "round_to_bf16", "rmsnorm_fwd", "rmsnorm_bwd", "grpo_step_from_prenorm",
 ]
 
 
@@ -292,6 +299,54 @@ def dW_rows(H, W, y, lse, coeff, vocab_ids, logit_scale=1.0):
         z = logit_scale * (H @ W[v])                      # column v of the logits, all tokens
         dz = c * ((y == v).astype(np.float64) - np.exp(z - lse))
         out[i] = logit_scale * (dz @ H)
+    return out
+
+
+# ------------------------------------------------------------- NEXT-4: the final RMSNorm in front of the path
+def round_to_bf16(a):
+    """float64 -> nearest bfloat16 (round to nearest, ties to even), returned as float64.  bf16 is the top 16
+    bits of an fp32; the value is first rounded to fp32 (every bf16 input of interest is far inside its range)."""
+    u = np.asarray(a, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    u = ((u + 0x7FFF + ((u >> 16) & 1)) >> 16) << 16
+    return u.astype(np.uint32).view(np.float32).astype(np.float64)
+
+
+def rmsnorm_fwd(x, gamma, eps_rms=1e-6, round_bf16=True):
+    """Final RMSNorm (the step before the path; BASELINE configs: "hidden ... after
+    RMSNorm-like scaling"):  rstd_t = 1 / sqrt(mean_k x_tk^2 + eps_rms);  H_tk = gamma_k x_tk rstd_t.
+    The path's contraction consumes H as bf16, so H is rounded to bf16 once (R29); round_bf16=False
+    gives the unrounded function (used by the finite-difference pins).  Returns (H [T,d], rstd [T])."""
+    x = np.asarray(x, dtype=np.float64)
+    g = np.asarray(gamma, dtype=np.float64)
+    rstd = 1.0 / np.sqrt((x * x).mean(axis=1) + eps_rms)
+    H = g[None, :] * x * rstd[:, None]
+    return (round_to_bf16(H) if round_bf16 else H), rstd
+
+
+def rmsnorm_bwd(x, gamma, rstd, dH):
+    """Backward of H = gamma * x * rstd (the bf16 rounding of H passes the gradient through unchanged, R30):
+    with xh = x rstd and g = gamma * dH:   dx_t = rstd_t (g_t - xh_t mean_k(g_tk xh_tk));   dgamma = sum_t dH_t * xh_t.
+    (mean_k x^2 + eps is differentiated exactly: d rstd / d x_k = - rstd^3 x_k / d.)"""
+    x = np.asarray(x, dtype=np.float64)
+    gm = np.asarray(gamma, dtype=np.float64)
+    dH = np.asarray(dH, dtype=np.float64)
+    xh = x * np.asarray(rstd, dtype=np.float64)[:, None]
+    g = gm[None, :] * dH
+    dx = np.asarray(rstd)[:, None] * (g - xh * (g * xh).mean(axis=1, keepdims=True))
+    dgamma = (dH * xh).sum(axis=0)
+    return dx, dgamma
+
+
+def grpo_step_from_prenorm(x, gamma, W, y, cu_seqlens, rewards, old_logp, ref_logp=None, mask=None,
+                           cfg: OracleConfig | None = None, G=None, loss_denom=None, eps_rms=1e-6,
+                           round_bf16=True, grad_scale=1.0):
+    """RMSNorm -> steps 1-9 -> RMSNorm backward: the whole step as a function of the pre-norm activations x and
+    the norm weight gamma.  Adds H, rstd, dx, dgamma to grpo_step's outputs."""
+    H, rstd = rmsnorm_fwd(x, gamma, eps_rms, round_bf16)
+    out = grpo_step(H, W, y, cu_seqlens, rewards, old_logp, ref_logp, mask=mask, cfg=cfg, G=G,
+                    loss_denom=loss_denom, grad_scale=grad_scale)
+    out["H"], out["rstd"] = H, rstd
+    out["dx"], out["dgamma"] = rmsnorm_bwd(x, gamma, rstd, out["dH"])
     return out
 
 

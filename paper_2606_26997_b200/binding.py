@@ -20,12 +20,13 @@ STATUS_NAMES = {0: "GRPO_OK", 1: "GRPO_ERR_INVALID_ARG", 2: "GRPO_ERR_SHAPE", 3:
 EXPORTS = [
     "grpo_default_config", "grpo_create", "grpo_destroy", "grpo_last_error", "grpo_workspace_bytes",
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
-    "grpo_fused_logprob_loss_fwd_bwd", "grpo_set_entropy_out",
+    "grpo_fused_logprob_loss_fwd_bwd", "grpo_set_entropy_out", "grpo_set_seq_denom", "grpo_bwd_row_stats_sync",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
     "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
 ]
-KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan", "stash_dz"]
+KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan", "stash_dz",
+                "compact", "dh_reduce"]
 
 
 class GrpoError(RuntimeError):
@@ -93,6 +94,8 @@ def load_library() -> C.CDLL:
     lib.grpo_profile_read_sync.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
     lib.grpo_bwd_tile_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     lib.grpo_set_entropy_out.argtypes = [vp, vp]
+    lib.grpo_set_seq_denom.argtypes = [vp, i32]
+    lib.grpo_bwd_row_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     _LIB = lib
     return lib
 
@@ -364,6 +367,14 @@ class GrpoContext:
         """entropy_out: fp32 CUDA tensor [>= T of the later forward calls] or None (off)."""
         self._entropy_out = entropy_out          # keep it alive
         _check(self.lib.grpo_set_entropy_out(self.h, _dev(entropy_out, torch.float32, "entropy_out")))
+
+    def grpo_set_seq_denom(self, n_sequences: int):
+        _check(self.lib.grpo_set_seq_denom(self.h, int(n_sequences)))
+
+    def grpo_bwd_row_stats_sync(self):
+        a, t = C.c_int64(0), C.c_int64(0)
+        _check(self.lib.grpo_bwd_row_stats_sync(self.h, C.byref(a), C.byref(t)))
+        return a.value, t.value
 
     def grpo_bwd_tile_stats_sync(self):
         a, t = C.c_int64(0), C.c_int64(0)

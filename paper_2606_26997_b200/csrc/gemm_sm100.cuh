@@ -64,7 +64,23 @@ struct GemmParams {
   int m_total, n_total;              // valid rows / cols of C
   int m_tiles, n_tiles, k_blocks;
   int n_fastest;                     // unit order: 1 = n tile fastest (A5/A6), 0 = m tile fastest (A2/A4)
-  int n_split, tiles_per_split;      // EPI_LSE: a unit is (m tile, contiguous range of n tiles)
+  // EPI_LSE: a unit is (m tile, contiguous range of n tiles).  The vocab split is a function of V ALONE (never of
+  // the launch's row count), so a token's log-sum-exp is summed in the same order whatever launch it is part of
+  // (batch invariance).  Units are walked in blocks of `lse_block` m tiles (= CTA pairs of the
+  // grid): inside a block the m tile is fastest, then the split, so that the pairs running together share W tiles
+  // through L2 while the block's H rows stay L2-resident and W is streamed once per block.
+  int n_split, tiles_per_split, lse_block;
+  // split-K (A5): the reduction is cut into k_split contiguous ranges of kb_per_split k blocks, again a function
+  // of the problem's K alone; split ks stores its fp32 partial tile at c_out + ks * c_split_stride, and
+  // splitk_reduce_kernel adds the partials in a fixed order.  k_split <= 1: off.
+  int k_split, kb_per_split;
+  int64_t c_split_stride;
+  // rows (A4 / A5: m_total; A6: reduction length) of this launch read from device memory (written by
+  // compact_rows_kernel: token-granular zero-coefficient compaction).  nullptr: the static
+  // m_total / k_blocks.  m_alloc: rows the dZ buffer holds (EPI_DZ zero-fills the rows of its last walked tile
+  // beyond the dynamic row count, which A6 reads as part of its last k block).
+  const int* dyn_rows;
+  int m_alloc;
   // per-token arrays are indexed by (row_offset + local row)
   int64_t row_offset;
   const int32_t* targets;
@@ -110,20 +126,32 @@ struct alignas(8) GemmBarriers {
   int klist[kMaxTilesSmem];          // A6: active token tiles of the chunk, staged by the producer warp
 };
 
-// Effective extent of a launch under tile skipping: the number of m tiles walked (A4/A5), the k blocks
-// per unit (A6) and the unit count.  Uniform over the grid (one global load each).
-struct Extent { int m_tiles, k_blocks, n_units; };
+// Effective extent of a launch under tile skipping / row compaction: the rows of C that exist, the number of m
+// tiles walked (A4/A5), the k blocks per unit (A6) and the unit count.  Uniform over the grid (one global load).
+struct Extent { int m_total, m_tiles, k_blocks, n_units; };
 template <int CG, int EPI>
 __device__ __forceinline__ Extent launch_extent(const GemmParams& p, int n_units) {
-  Extent e{p.m_tiles, p.k_blocks, n_units};
-  if (p.tile_list != nullptr && !is_lse(EPI)) {
+  Extent e{p.m_total, p.m_tiles, p.k_blocks, n_units};
+  if constexpr (is_lse(EPI)) return e;
+  const int ks = p.k_split > 1 ? p.k_split : 1;
+  if (p.dyn_rows != nullptr) {
+    const int rows = *p.dyn_rows;
+    if constexpr (EPI == EPI_RED_F32) {
+      e.k_blocks = min(p.k_blocks, (rows + BK - 1) / BK);
+      if (e.k_blocks == 0) e.n_units = 0;              // nothing to add: no MMA, so no epilogue either
+    } else {
+      e.m_total = min(p.m_total, rows);
+      e.m_tiles = min(p.m_tiles, (e.m_total + BM * CG - 1) / (BM * CG));
+      e.n_units = e.m_tiles * p.n_tiles * ks;
+    }
+  } else if (p.tile_list != nullptr) {
     const int n_active = p.tile_list[0];
     if constexpr (EPI == EPI_RED_F32) {
       e.k_blocks = min(p.k_blocks, n_active * (BM * CG / BK));
-      if (e.k_blocks == 0) e.n_units = 0;            // nothing to add: no MMA, so no epilogue either
+      if (e.k_blocks == 0) e.n_units = 0;
     } else {
       e.m_tiles = n_active;
-      e.n_units = n_active * p.n_tiles;
+      e.n_units = n_active * p.n_tiles * ks;
     }
   }
   return e;
@@ -140,26 +168,43 @@ __device__ __forceinline__ int walked_k_block(const GemmParams& p, const int* kl
   return tile * kPerTile + kb % kPerTile;
 }
 
+// One scheduling unit: output tile(s) [m_tile] x [n0, n1) reduced over k blocks [kb0, kb1); `part` is the vocab
+// split (EPI_LSE) or the K split (split-K stores) the unit belongs to.
+struct Unit { int m_tile, n0, n1, kb0, kb1, part; };
 template <int EPI>
-__device__ __forceinline__ void unit_to_tiles(const GemmParams& p, const Extent& e, int u, int& m_tile, int& n0,
-                                              int& n1) {
+__device__ __forceinline__ Unit unit_to_tiles(const GemmParams& p, const Extent& e, int u) {
+  Unit t;
+  t.kb0 = 0;
+  t.kb1 = e.k_blocks;
+  t.part = 0;
   if constexpr (is_lse(EPI)) {
-    m_tile = u % p.m_tiles;
-    int split = u / p.m_tiles;
-    n0 = split * p.tiles_per_split;
-    n1 = min(p.n_tiles, n0 + p.tiles_per_split);
-    return;
+    const int per_block = p.lse_block * p.n_split;       // only the last block of m tiles can be short
+    const int b = u / per_block, r = u - b * per_block;
+    const int mb = min(p.lse_block, p.m_tiles - b * p.lse_block);
+    t.part = r / mb;
+    t.m_tile = b * p.lse_block + (r - t.part * mb);
+    t.n0 = t.part * p.tiles_per_split;
+    t.n1 = min(p.n_tiles, t.n0 + p.tiles_per_split);
+    return t;
+  }
+  if (p.k_split > 1) {                                    // K split slowest: a wave streams one K range
+    const int per_split = e.m_tiles * p.n_tiles;
+    t.part = u / per_split;
+    u -= t.part * per_split;
+    t.kb0 = t.part * p.kb_per_split;
+    t.kb1 = min(e.k_blocks, t.kb0 + p.kb_per_split);
   }
   int m_idx;
   if (p.n_fastest) {
-    n0 = u % p.n_tiles;
+    t.n0 = u % p.n_tiles;
     m_idx = u / p.n_tiles;
   } else {
     m_idx = u % e.m_tiles;
-    n0 = u / e.m_tiles;
+    t.n0 = u / e.m_tiles;
   }
-  n1 = n0 + 1;
-  m_tile = (EPI != EPI_RED_F32 && p.tile_list != nullptr) ? p.tile_list[2 + m_idx] : m_idx;
+  t.n1 = t.n0 + 1;
+  t.m_tile = (EPI != EPI_RED_F32 && p.tile_list != nullptr && p.dyn_rows == nullptr) ? p.tile_list[2 + m_idx] : m_idx;
+  return t;
 }
 
 // Drift bound.  The CTA pairs of a launch that share operand panels through L2 (the 8 d-tiles of one dZ
@@ -249,12 +294,11 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       bool sync_on = p.sync != nullptr && cta_rank == 0;
       int epoch = 0, to_epoch = 1;
       for (int u = unit0; u < n_units; u += unit_step) {
-        int m_tile, n0, n1;
-        unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
-        const int a_row = (m_tile * CG + static_cast<int>(cta_rank)) * BM;
-        for (int n_tile = n0; n_tile < n1; ++n_tile) {
+        const Unit un = unit_to_tiles<EPI>(p, ext, u);
+        const int a_row = (un.m_tile * CG + static_cast<int>(cta_rank)) * BM;
+        for (int n_tile = un.n0; n_tile < un.n1; ++n_tile) {
           const int b_row = n_tile * BN + static_cast<int>(cta_rank) * kBRows;
-          for (int kbw = 0; kbw < ext.k_blocks; ++kbw) {
+          for (int kbw = un.kb0; kbw < un.kb1; ++kbw) {
             const int kb = EPI == EPI_RED_F32 ? walked_k_block<CG>(p, bars->klist, kbw) : kbw;
             if (sync_on && --to_epoch == 0) {
               to_epoch = p.sync_epoch_kb;
@@ -315,13 +359,13 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       int acc = 0;
       uint32_t acc_phase = 0;
       for (int u = unit0; u < n_units; u += unit_step) {
-        int m_tile, n0, n1;
-        unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
-        for (int n_tile = n0; n_tile < n1; ++n_tile) {
+        const Unit un = unit_to_tiles<EPI>(p, ext, u);
+        const int n_kb = un.kb1 - un.kb0;
+        for (int n_tile = un.n0; n_tile < un.n1; ++n_tile) {
           mbar_wait(&bars->tmem_empty[acc], acc_phase ^ 1);
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + acc * BN;
-          for (int kb = 0; kb < ext.k_blocks; ++kb) {
+          for (int kb = 0; kb < n_kb; ++kb) {
             mbar_wait(&bars->full[stage], phase);
             tc_fence_after();
             if (leader_lane) {
@@ -349,9 +393,8 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       // epochs this pair's producer enters: ceil(k blocks it issues / epoch length)
       long long my_kb = 0;
       for (int u = unit0; u < n_units; u += unit_step) {
-        int m_tile, n0, n1;
-        unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
-        my_kb += static_cast<long long>(n1 - n0) * ext.k_blocks;
+        const Unit un = unit_to_tiles<EPI>(p, ext, u);
+        my_kb += static_cast<long long>(un.n1 - un.n0) * (un.kb1 - un.kb0);
       }
       const int my_epochs = static_cast<int>((my_kb + p.sync_epoch_kb - 1) / p.sync_epoch_kb);
       const unsigned int n_pairs = gridDim.x / CG;
@@ -373,10 +416,10 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     int acc = 0;
     uint32_t acc_phase = 0;
     for (int u = unit0; u < n_units; u += unit_step) {
-      int m_tile, n0, n1;
-      unit_to_tiles<EPI>(p, ext, u, m_tile, n0, n1);
+      const Unit un = unit_to_tiles<EPI>(p, ext, u);
+      const int m_tile = un.m_tile, n0 = un.n0, n1 = un.n1;
       const int row_local = (m_tile * CG + static_cast<int>(cta_rank)) * BM + row_in_tile;   // row within this launch's C
-      const bool row_ok = row_local < p.m_total;
+      const bool row_ok = row_local < ext.m_total;
       const int64_t row_g = p.row_offset + row_local;            // index into per-token arrays
 
       [[maybe_unused]] int y = -1;
@@ -498,11 +541,18 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
 #pragma unroll
               for (int g = 0; g < 4; ++g) st_global_v4(dst + g * 8, pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+            } else if (row_local < p.m_alloc) {
+              // rows of the last walked tile beyond the (dynamic) row count: A6 reads them as the tail of its last
+              // k block, so they must hold zeros, not what an earlier chunk left there
+              __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
+#pragma unroll
+              for (int g = 0; g < 4; ++g) st_global_v4(dst + g * 8, 0u, 0u, 0u, 0u);
             }
           } else if constexpr (EPI == EPI_STORE) {
             if (row_ok) {
               if (p.c_fp32) {
-                float* dst = reinterpret_cast<float*>(p.c_out) + static_cast<int64_t>(row_local) * p.c_pitch + cbase;
+                float* dst = reinterpret_cast<float*>(p.c_out) + un.part * p.c_split_stride +
+                             static_cast<int64_t>(row_local) * p.c_pitch + cbase;
 #pragma unroll
                 for (int g = 0; g < 8; ++g)
                   if (g * 4 < nvalid)
@@ -554,7 +604,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       }
       if constexpr (is_lse(EPI)) {
         if (row_ok) {
-          const int split = u / p.m_tiles;
+          const int split = un.part;
           p.part_m[split * p.part_stride + row_local] = run_m;     // partials are indexed by the launch's own rows
           p.part_s[split * p.part_stride + row_local] = run_s;
           if (p.part_u != nullptr) p.part_u[split * p.part_stride + row_local] = run_u;

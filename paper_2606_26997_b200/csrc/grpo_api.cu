@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -60,6 +61,11 @@ struct SlotLayout {
           off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0, off_sync = 0,
           off_tiles = 0, off_tile_stats = 0;
   int64_t tile_cap = 0;   // token tiles per backward chunk
+  // token-granular compaction + split-K of A5
+  int64_t off_row_idx = 0, off_meta = 0, off_hc = 0, off_yc = 0, off_lsec = 0, off_coeffc = 0, off_dh_part = 0,
+          off_row_stats = 0;
+  int64_t n_chunks_max = 0;
+  int64_t fwd_block_rows = 0;   // rows per A2 launch (bounds the LSE partials)
   int64_t bytes = 0;
 };
 
@@ -80,7 +86,16 @@ struct grpo_ctx {
   int denom_next = 0;
   cudaEvent_t denom_event = nullptr;
   float* entropy_out = nullptr;         // grpo_set_entropy_out: per-token entropy of the direct forward calls
+  int32_t seq_denom = 0;                // grpo_set_seq_denom: sequences of the whole logical update (loss_agg 1)
   cudaStream_t copy_stream = nullptr;   // grpo_step_host: H2D / D2H overlapped with the compute stream
+  std::vector<cudaEvent_t> pipe_events; // grpo_step_host: fence + per-chunk in / out events, created once
+  // pinned staging ring for the small host-built index arrays of run_launch (cu_seqlens, cu_groups)
+  static const int kStageRing = 8;
+  int32_t* stage_host = nullptr;
+  int64_t stage_ints = 0;               // ints per ring entry
+  cudaEvent_t stage_ev[kStageRing] = {nullptr};
+  int stage_next = 0;
+  std::vector<cudaEvent_t> event_pool;  // timing events of the profiler, reused across launches
   uint8_t* ws = nullptr;
   int64_t ws_max_T = 0;
   int n_slots = 0;
@@ -101,8 +116,8 @@ struct LaunchScope {
   LaunchScope(grpo_ctx* c, int kind, cudaStream_t s) : ctx(c), st(s) {
     ctx->kernel_count[kind]++;
     if (ctx->profiling) {
-      grpo_ctx::ProfRec r{kind, nullptr, nullptr};
-      if (cudaEventCreate(&r.beg) == cudaSuccess && cudaEventCreate(&r.end) == cudaSuccess) {
+      grpo_ctx::ProfRec r{kind, take_event(c), take_event(c)};
+      if (r.beg && r.end) {
         cudaEventRecord(r.beg, st);
         end = r.end;
         ctx->prof.push_back(r);
@@ -110,16 +125,41 @@ struct LaunchScope {
     }
   }
   ~LaunchScope() { if (end) cudaEventRecord(end, st); }
+  static cudaEvent_t take_event(grpo_ctx* c) {     // from the context's pool; created only when the pool is empty
+    cudaEvent_t e = nullptr;
+    if (!c->event_pool.empty()) { e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+    return cudaEventCreate(&e) == cudaSuccess ? e : nullptr;
+  }
 };
 static const int kDenomRing = 64;
-static void prof_clear(grpo_ctx* ctx) {
-  for (auto& r : ctx->prof) { cudaEventDestroy(r.beg); cudaEventDestroy(r.end); }
+static void prof_clear(grpo_ctx* ctx) {             // records go back to the pool
+  for (auto& r : ctx->prof) { ctx->event_pool.push_back(r.beg); ctx->event_pool.push_back(r.end); }
   ctx->prof.clear();
 }
 
 
 static const int kSyncCap = 1 << 15;   // drift-gate epoch counters per workspace slot
 static int64_t chunk_tokens(const grpo_config& c) { return c.bwd_chunk_tokens > 0 ? c.bwd_chunk_tokens : 9472; }
+
+// The vocab split of the A2 units and the K split of A5 are functions of V (and the tile shape) ALONE: a token's
+// log-sum-exp and dHidden row are then summed in one fixed order whatever launch, chunk or batch the token is part
+// of (batch invariance: CGP changes "only group dispatch timing and order - not samples, advantages, or gradient
+// computation").  Load balance comes from the ORDER the units are walked in, never from re-cutting
+// a reduction.
+static const int kLseTilesPerSplit = 8;      // 256-column vocab tiles per A2 unit (2048 logits)
+static const int kDhKSplit = 4;              // K ranges of A5 (K = V)
+static void lse_split(int V, int* n_split, int* tiles_per_split) {
+  const int n_tiles = (V + BN - 1) / BN;
+  *n_split = (n_tiles + kLseTilesPerSplit - 1) / kLseTilesPerSplit;
+  *tiles_per_split = (n_tiles + *n_split - 1) / *n_split;
+  *n_split = (n_tiles + *tiles_per_split - 1) / *tiles_per_split;
+}
+static void dh_ksplit(int V, int* k_split, int* kb_per_split) {
+  const int k_blocks = (V + BK - 1) / BK;
+  const int want = std::min(kDhKSplit, k_blocks);
+  *kb_per_split = (k_blocks + want - 1) / want;
+  *k_split = (k_blocks + *kb_per_split - 1) / *kb_per_split;
+}
 
 static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   SlotLayout L;
@@ -129,9 +169,13 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
     off = align_up(off + bytes, 256);
     return o;
   };
-  L.part_cap = max_T + 148LL * 128 * 4;
+  int n_split, tps, k_split, kbps;
+  lse_split(c.V, &n_split, &tps);
+  dh_ksplit(c.V, &k_split, &kbps);
   L.s_max = std::min<int64_t>(max_T, 1 << 20);
-  L.chunk_rows = std::min<int64_t>(align_up(chunk_tokens(c), 128), align_up(max_T, 128));
+  L.chunk_rows = std::min<int64_t>(align_up(chunk_tokens(c), 256), align_up(max_T, 256));
+  L.fwd_block_rows = std::min<int64_t>(align_up(max_T, 256), 4 * 74 * 256);
+  L.part_cap = n_split * L.fwd_block_rows;
   L.v_pad = align_up(c.V, 64);
   L.off_part_m = take(L.part_cap * 4);
   L.off_part_s = take(L.part_cap * 4);
@@ -159,6 +203,15 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.tile_cap = L.chunk_rows / BM + 1;
   L.off_tiles = take((2 + 2 * L.tile_cap) * 4);
   L.off_tile_stats = take(16);
+  L.n_chunks_max = (max_T + L.chunk_rows - 1) / L.chunk_rows + 1;
+  L.off_row_idx = take(max_T * 4);
+  L.off_meta = take((2 + L.n_chunks_max) * 4);
+  L.off_hc = take(L.chunk_rows * c.d * 2);
+  L.off_yc = take(L.chunk_rows * 4);
+  L.off_lsec = take(L.chunk_rows * 4);
+  L.off_coeffc = take(L.chunk_rows * 4);
+  L.off_dh_part = take(static_cast<int64_t>(k_split) * L.chunk_rows * c.d * 4);
+  L.off_row_stats = take(16);
   L.bytes = off;
   return L;
 }
@@ -208,23 +261,28 @@ static int32_t make_tmap_c_f32(const grpo_ctx* ctx, CUtensorMap* m, const void* 
 template <int CG, bool A_MN, bool B_MN, int EPI>
 static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB,
                               const GemmParams& p, int n_units, cudaStream_t st, const CUtensorMap* tmC) {
-  static bool attr_set = false;
+  // the dynamic shared memory limit is a per-device attribute of the function: one flag bit per device and
+  // template instantiation (setting it twice is harmless, so a relaxed atomic is enough)
+  static std::atomic<uint64_t> attr_set{0};
   auto kern = grpo_gemm_kernel<CG, A_MN, B_MN, EPI>;
   constexpr int smem = GemmShape<CG>::kSmemBytes;
-  if (!attr_set) {
+  const uint64_t dev_bit = 1ull << (ctx->device & 63);
+  if (ctx->device >= 64 || !(attr_set.load(std::memory_order_relaxed) & dev_bit)) {
     CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    attr_set = true;
+    if (ctx->device < 64) attr_set.fetch_or(dev_bit, std::memory_order_relaxed);
   }
   if (n_units <= 0) return GRPO_OK;
   // persistent: one CTA (CG = 1) or one CTA pair (CG = 2, a 2-CTA cluster) per SM / SM pair
   const int grid = CG * std::min(n_units, ctx->num_sms / CG);
   GemmParams pl = p;
+  pl.lse_block = grid / CG;
   // drift gate (gemm_sm100.cuh): epoch counters live in the launch's workspace slot, zeroed on the stream
   const int xsync = ctx->cfg.gemm_drift_epoch_kb == 0 ? 32 : ctx->cfg.gemm_drift_epoch_kb;
   pl.sync_lag = 1;   // epochs a pair may lead the slowest pair by (2-8 measured: no different from 1)
   if (pl.sync != nullptr && xsync > 0 && grid / CG > 1) {
     const int64_t n_pairs = grid / CG;
-    const int64_t kb_unit = static_cast<int64_t>(p.k_blocks) * (is_lse(EPI) ? p.tiles_per_split : 1);
+    const int64_t kb_unit = is_lse(EPI) ? static_cast<int64_t>(p.k_blocks) * p.tiles_per_split
+                                        : (p.k_split > 1 ? p.kb_per_split : p.k_blocks);
     const int64_t max_kb = (n_units + n_pairs - 1) / n_pairs * kb_unit;
     int64_t E = xsync;
     while ((max_kb + E - 1) / E + 1 > kSyncCap) E *= 2;
@@ -261,21 +319,6 @@ static int32_t launch_gemm(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, cons
   if (EPI == EPI_RED_F32 && tmC == nullptr) return fail(GRPO_ERR_INVALID_ARG, "EPI_RED_F32 needs the C tensor map");
   if (ctx->cg == 2) return launch_gemm_cg<2, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
   return launch_gemm_cg<1, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
-}
-
-static int choose_n_split(int m_tiles, int n_tiles, int sms, int64_t max_split) {
-  int best = 1;
-  int64_t best_cost = INT64_MAX;
-  const int lim = static_cast<int>(std::min<int64_t>(std::min<int64_t>(max_split, n_tiles), 4 * sms));
-  for (int s = 1; s <= std::max(lim, 1); ++s) {
-    const int tps = (n_tiles + s - 1) / s;
-    const int s_eff = (n_tiles + tps - 1) / tps;
-    if (s_eff != s) continue;
-    const int64_t waves = (static_cast<int64_t>(m_tiles) * s + sms - 1) / sms;
-    const int64_t cost = waves * tps;
-    if (cost < best_cost) { best_cost = cost; best = s; }
-  }
-  return best;
 }
 
 // ------------------------------------------------------------------------------------- API: misc
@@ -342,6 +385,10 @@ extern "C" int32_t grpo_destroy(grpo_ctx* ctx) {
   cudaFree(ctx->err_dev);
   cudaFree(ctx->denom_ring);
   prof_clear(ctx);
+  for (auto e : ctx->event_pool) cudaEventDestroy(e);
+  for (auto e : ctx->pipe_events) cudaEventDestroy(e);
+  for (auto e : ctx->stage_ev) if (e) cudaEventDestroy(e);
+  if (ctx->stage_host) cudaFreeHost(ctx->stage_host);
   if (ctx->denom_event) cudaEventDestroy(ctx->denom_event);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   delete ctx;
@@ -365,7 +412,21 @@ extern "C" int32_t grpo_set_workspace(grpo_ctx* ctx, void* dev_ptr, int64_t byte
   ctx->ws_max_T = max_T;
   ctx->n_slots = n_slots;
   ctx->lay = L;
-  for (int i = 0; i < n_slots; ++i) CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_tile_stats), 0, 16));
+  for (int i = 0; i < n_slots; ++i) {
+    CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_tile_stats), 0, 16));
+    CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_row_stats), 0, 16));
+  }
+  // pinned ring for run_launch's index arrays: cu_seqlens [S+1] + cu_groups [S+1] per entry
+  const int64_t need = 2 * (L.s_max + 1);
+  if (need > ctx->stage_ints) {
+    CU_OK(cudaDeviceSynchronize());
+    if (ctx->stage_host) cudaFreeHost(ctx->stage_host);
+    ctx->stage_host = nullptr;
+    CU_OK(cudaMallocHost(&ctx->stage_host, static_cast<size_t>(need) * grpo_ctx::kStageRing * 4));
+    ctx->stage_ints = need;
+    for (auto& e : ctx->stage_ev)
+      if (!e) CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
   return GRPO_OK;
 }
 
@@ -419,6 +480,22 @@ extern "C" int32_t grpo_bwd_tile_stats_sync(grpo_ctx* ctx, int64_t* active_out, 
   return GRPO_OK;
 }
 
+extern "C" int32_t grpo_bwd_row_stats_sync(grpo_ctx* ctx, int64_t* active_out, int64_t* total_out) {
+  if (!ctx || !active_out || !total_out) return fail(GRPO_ERR_INVALID_ARG, "NULL pointer");
+  *active_out = *total_out = 0;
+  if (!ctx->ws) return GRPO_OK;
+  CU_OK(cudaDeviceSynchronize());
+  for (int i = 0; i < ctx->n_slots; ++i) {
+    long long h[2] = {0, 0};
+    long long* stats = slot_ptr<long long>(ctx, i, ctx->lay.off_row_stats);
+    CU_OK(cudaMemcpy(h, stats, 16, cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemset(stats, 0, 16));
+    *active_out += h[0];
+    *total_out += h[1];
+  }
+  return GRPO_OK;
+}
+
 // ------------------------------------------------------------------------------------- A1
 extern "C" int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, const int32_t* cu_groups,
                                         int32_t n_groups, int32_t G, float* adv_out, uint8_t* zero_var_out,
@@ -445,6 +522,7 @@ struct FwdArgs {
   double loss_denom; const float* denom_dev;
   float* logp_out; float* lse_out; float* coeff_out; float* loss_accum; float* metrics_accum;
   float* entropy_out = nullptr;   // nullable (grpo_set_entropy_out)
+  int32_t S_norm = 0;             // loss_agg 1: sequences of the WHOLE logical update (0: this call's S)
 };
 
 static int32_t fwd_check(grpo_ctx* ctx, int32_t S, int64_t T) {
@@ -497,8 +575,9 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
   p.m_tiles = static_cast<int>((rows + TM - 1) / TM);
   p.n_tiles = (c.V + BN - 1) / BN;
   p.k_blocks = (c.d + BK - 1) / BK;
-  p.n_split = choose_n_split(p.m_tiles, p.n_tiles, ctx->num_sms / ctx->cg, std::max<int64_t>(1, L.part_cap / rows));
-  p.tiles_per_split = (p.n_tiles + p.n_split - 1) / p.n_split;
+  lse_split(c.V, &p.n_split, &p.tiles_per_split);          // a function of V alone (batch invariance)
+  if (static_cast<int64_t>(p.n_split) * rows > L.part_cap)
+    return fail(GRPO_ERR_WORKSPACE, "forward launch of %lld rows exceeds the LSE partial buffers", (long long)rows);
   p.row_offset = t0;
   p.targets = targets;
   p.scale_log2e = c.logit_scale * kLog2e;
@@ -518,7 +597,8 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
 
   LossParams lp;
   std::memset(&lp, 0, sizeof(lp));
-  lp.T = rows; lp.t_begin = t0; lp.S = a.S; lp.V = c.V; lp.n_split = p.n_split; lp.part_stride = rows;
+  lp.T = rows; lp.t_begin = t0; lp.S = a.S; lp.S_norm = a.S_norm > 0 ? a.S_norm : a.S; lp.V = c.V;
+  lp.n_split = p.n_split; lp.part_stride = rows;
   lp.part_m = part_m; lp.part_s = part_s; lp.part_u = p.part_u; lp.entropy = a.entropy_out; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = a.cu_seqlens;
   lp.adv = a.adv; lp.old_logp = a.old_logp; lp.ref_logp = a.ref_logp; lp.mask = a.mask;
   lp.seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
@@ -542,13 +622,19 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
                         const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv, const float* old_logp,
                         const float* ref_logp, const uint8_t* mask, double loss_denom, const float* denom_dev,
                         float* logp_out, float* lse_out, float* coeff_out, float* loss_accum, float* metrics_accum,
-                        cudaStream_t st, float* entropy_out = nullptr) {
+                        cudaStream_t st, float* entropy_out = nullptr, int32_t S_norm = 0) {
   GRPO_TRY(fwd_check(ctx, S, T));
   FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
             logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
   a.entropy_out = entropy_out;
+  a.S_norm = S_norm;
   GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
-  return fwd_rows(ctx, slot, hidden, W, targets, a, T, 0, T, nullptr, st);
+  // A2 + A3 in launches of at most fwd_block_rows rows: bounds the LSE partial buffers; a row's result does not
+  // depend on how the call is cut (fixed vocab split)
+  for (int64_t t0 = 0; t0 < T; t0 += ctx->lay.fwd_block_rows)
+    GRPO_TRY(fwd_rows(ctx, slot, hidden, W, targets, a, T, t0, std::min<int64_t>(ctx->lay.fwd_block_rows, T - t0),
+                      nullptr, st));
+  return GRPO_OK;
 }
 
 extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const void* W,
@@ -563,7 +649,13 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden
   if (T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0 and S > 0 (got T=%lld S=%d)", (long long)T, S);
   return fwd_impl(ctx, 0, hidden, W, targets, cu_seqlens, S, T, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
                   logp_out, lse_out, coeff_out, loss_accum, metrics_accum, static_cast<cudaStream_t>(stream),
-                  ctx->entropy_out);
+                  ctx->entropy_out, ctx->seq_denom);
+}
+
+extern "C" int32_t grpo_set_seq_denom(grpo_ctx* ctx, int32_t n_sequences) {
+  if (!ctx || n_sequences < 0) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL or n_sequences < 0");
+  ctx->seq_denom = n_sequences;
+  return GRPO_OK;
 }
 
 extern "C" int32_t grpo_set_entropy_out(grpo_ctx* ctx, float* entropy_out) {
@@ -577,24 +669,27 @@ extern "C" int32_t grpo_set_entropy_out(grpo_ctx* ctx, float* entropy_out) {
 static int64_t rows_per_chunk_for(const grpo_ctx* ctx, int64_t T) {
   const int64_t Tc = ctx->lay.chunk_rows;
   const int64_t n_chunks = (T + Tc - 1) / Tc;
-  return std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, BM * ctx->cg));
+  return std::min<int64_t>(Tc, align_up((T + n_chunks - 1) / n_chunks, 256));
 }
 
 // grpo_step_host's copy pipeline: chunk i of the hidden states arrives on the copy stream (in[i]), and the
 // dHidden rows of chunk i leave on it as soon as A5 has written them, under the next chunk's contractions.
 struct HostPipe {
   cudaStream_t cs;
-  std::vector<cudaEvent_t> in, out;
+  std::vector<cudaEvent_t> in, out;   // owned by the context (grpo_ctx::pipe_events)
   uint8_t* dh_host;
-  ~HostPipe() {
-    for (auto e : in) if (e) cudaEventDestroy(e);
-    for (auto e : out) if (e) cudaEventDestroy(e);
-  }
 };
 
 // fused == nullptr: the backward of north_star (A4 recomputes the logits).  fused != nullptr: the
 // 3-contraction variant: per chunk, the forward runs first and stashes the chunk's
 // logits, which are then converted to dZ in place instead of being recomputed; lse / coeff are fused's.
+//
+// Zero-coefficient work is skipped (cfg.bwd_skip_zero_tiles >= 0):
+//   north_star path: token-granular.  The call's rows with coeff != 0 are compacted on the device
+//     (compact_rows_kernel), each backward chunk gathers its active hidden rows into a dense panel, A4 - A6 run
+//     on that panel with the row count read from device memory, and the split-K reduction of A5 scatters the
+//     dHidden rows back; rows with coeff == 0 are written as zeros.  Nothing is decided on the host.
+//   3-contraction variant: per 256-row token tile (the chunk's logits are stashed before its coefficients exist).
 static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
                         const float* lse, const float* coeff, int64_t T, float grad_scale, void* dhidden_out,
                         float* dW_accum, cudaStream_t st, const FwdArgs* fused = nullptr, HostPipe* pipe = nullptr) {
@@ -605,31 +700,69 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   const SlotLayout& L = ctx->lay;
   __nv_bfloat16* dz = slot_ptr<__nv_bfloat16>(ctx, slot, L.off_dz);
   const int64_t rows_per_chunk = rows_per_chunk_for(ctx, T);
+  const int n_chunks = static_cast<int>((T + rows_per_chunk - 1) / rows_per_chunk);
   const uint8_t* Hb = static_cast<const uint8_t*>(hidden);
   const int dh_elem = c.dhidden_fp32 ? 4 : 2;
+  const bool skip = c.bwd_skip_zero_tiles >= 0;
+  const bool compact = skip && !fused;
+  const int TM = BM * ctx->cg;
+  int k_split, kb_per_split;
+  dh_ksplit(c.V, &k_split, &kb_per_split);
+  float* dh_part = slot_ptr<float>(ctx, slot, L.off_dh_part);
 
   CUtensorMap tmW_k, tmW_mn;
-  const int TM = BM * ctx->cg;
   GRPO_TRY(make_tmap(ctx, &tmW_k, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, BK, BN / ctx->cg));
   GRPO_TRY(make_tmap(ctx, &tmW_mn, W, c.d, c.V, static_cast<uint64_t>(c.d) * 2, 64, BK));
 
-  for (int64_t t0 = 0; t0 < T; t0 += rows_per_chunk) {
-    const int64_t rows = std::min<int64_t>(rows_per_chunk, T - t0);
-    const void* Hc = Hb + t0 * c.d * 2;
-    const int m_tiles = static_cast<int>((rows + TM - 1) / TM);
-    CUtensorMap tmH_k, tmH_mn, tmDZ_k, tmDZ_mn;
-    GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
-    GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
+  int* row_idx = slot_ptr<int>(ctx, slot, L.off_row_idx);
+  int* meta = slot_ptr<int>(ctx, slot, L.off_meta);
+  if (compact) {
+    if (n_chunks > L.n_chunks_max) return fail(GRPO_ERR_WORKSPACE, "too many backward chunks for the workspace");
+    {
+      LaunchScope ls(ctx, GRPO_KERNEL_COMPACT, st);
+      compact_rows_kernel<<<1, 1024, 0, st>>>(coeff, static_cast<int>(T), static_cast<int>(rows_per_chunk), n_chunks,
+                                              row_idx, meta, slot_ptr<long long>(ctx, slot, L.off_row_stats));
+    }
+    CU_OK(cudaGetLastError());
+    if (dhidden_out) {
+      LaunchScope ls(ctx, GRPO_KERNEL_COMPACT, st);
+      zero_coeff_rows_kernel<<<static_cast<unsigned>(T), 128, 0, st>>>(coeff, static_cast<int>(T),
+                                                                      static_cast<uint8_t*>(dhidden_out),
+                                                                      static_cast<int64_t>(c.d) * dh_elem);
+      CU_OK(cudaGetLastError());
+    }
+  }
 
+  for (int64_t t0 = 0; t0 < T; t0 += rows_per_chunk) {
+    const int64_t rows = std::min<int64_t>(rows_per_chunk, T - t0);       // static upper bound of the chunk's rows
     const size_t chunk_idx = static_cast<size_t>(t0 / rows_per_chunk);
+    const int m_tiles = static_cast<int>((rows + TM - 1) / TM);
+    // compact: the chunk's operands live in dense panels of the workspace whose tails are zero-filled explicitly
+    // (the row count is only known on the device); otherwise the tensor maps end at `rows` and TMA zero-fills.
+    const int64_t map_rows = compact ? align_up(rows, 256) : rows;
+    const int* dyn_rows = compact ? meta + 2 + chunk_idx : nullptr;
+    const void* Hc = compact ? static_cast<const void*>(slot_ptr<uint8_t>(ctx, slot, L.off_hc))
+                             : static_cast<const void*>(Hb + t0 * c.d * 2);
+    const int32_t* y_c = compact ? slot_ptr<int32_t>(ctx, slot, L.off_yc) : targets;
+    const float* lse_c = compact ? slot_ptr<float>(ctx, slot, L.off_lsec) : lse;
+    const float* coeff_c = compact ? slot_ptr<float>(ctx, slot, L.off_coeffc) : coeff;
+    const int64_t row_off = compact ? 0 : t0;
+
     if (fused) {
       if (pipe && chunk_idx < pipe->in.size()) CU_OK(cudaStreamWaitEvent(st, pipe->in[chunk_idx], 0));
       GRPO_TRY(fwd_rows(ctx, slot, hidden, W, targets, *fused, T, t0, rows, dz, st));
     }
     if (!dhidden_out && !dW_accum) continue;
-    // zero-coefficient tile skipping: scan this chunk's coefficients on the device
+
     const int* tile_list = nullptr;
-    if (c.bwd_skip_zero_tiles >= 0) {
+    if (compact) {
+      LaunchScope ls(ctx, GRPO_KERNEL_COMPACT, st);
+      gather_rows_kernel<<<static_cast<unsigned>(map_rows), 128, 0, st>>>(
+          reinterpret_cast<const uint4*>(hidden), c.d / 8, row_idx + t0, dyn_rows, 256, static_cast<int>(L.chunk_rows),
+          targets, lse, coeff, slot_ptr<uint4>(ctx, slot, L.off_hc), slot_ptr<int32_t>(ctx, slot, L.off_yc),
+          slot_ptr<float>(ctx, slot, L.off_lsec), slot_ptr<float>(ctx, slot, L.off_coeffc));
+      CU_OK(cudaGetLastError());
+    } else if (skip) {   // 3-contraction variant: scan this chunk's coefficients per token tile
       int* list = slot_ptr<int>(ctx, slot, L.off_tiles);
       {
         LaunchScope ls(ctx, GRPO_KERNEL_TILE_SCAN, st);
@@ -646,6 +779,9 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       }
       tile_list = list;
     }
+
+    CUtensorMap tmH_k, tmH_mn, tmDZ_k, tmDZ_mn;
+    GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, map_rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
     if (fused) {  // stashed logits -> dZ in place (HBM-bound elementwise pass instead of the A4 contraction)
       LaunchScope ls(ctx, GRPO_KERNEL_STASH_DZ, st);
       stash_to_dz_kernel<<<static_cast<unsigned>(rows), 256, 0, st>>>(
@@ -653,29 +789,44 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
           L.n_vtiles, BN, targets + t0, lse + t0, coeff + t0, c.logit_scale * grad_scale, tile_list, TM);
       CU_OK(cudaGetLastError());
     } else {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
+      GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, map_rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
       p.m_total = static_cast<int>(rows); p.n_total = c.V;
       p.m_tiles = m_tiles; p.n_tiles = (c.V + BN - 1) / BN; p.k_blocks = (c.d + BK - 1) / BK;
       p.n_fastest = 0;
-      p.row_offset = t0; p.targets = targets;
+      p.row_offset = row_off; p.targets = y_c;
       p.scale_log2e = c.logit_scale * kLog2e; p.logit_scale = c.logit_scale;
-      p.lse = lse; p.coeff = coeff; p.coeff_mul = c.logit_scale * grad_scale;
-      p.dz = dz; p.dz_pitch = L.v_pad; p.tile_list = tile_list;
+      p.lse = lse_c; p.coeff = coeff_c; p.coeff_mul = c.logit_scale * grad_scale;
+      p.dz = dz; p.dz_pitch = L.v_pad; p.dyn_rows = dyn_rows;
+      p.m_alloc = compact ? static_cast<int>(L.chunk_rows) : 0;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, GRPO_KERNEL_GEMM_DZ, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
     }
-    if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d]
+    if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d], K cut into k_split fixed ranges, fp32 partials
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
       p.m_total = static_cast<int>(rows); p.n_total = c.d;
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
       p.n_fastest = 1;
-      p.c_out = static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem; p.c_pitch = c.d; p.c_fp32 = c.dhidden_fp32;
-      p.tile_list = tile_list;
+      p.k_split = k_split; p.kb_per_split = kb_per_split; p.c_split_stride = L.chunk_rows * c.d;
+      p.c_out = dh_part; p.c_pitch = c.d; p.c_fp32 = 1;
+      p.tile_list = tile_list; p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
-      GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p, p.m_tiles * p.n_tiles, st)));
-      if (pipe && pipe->dh_host && chunk_idx < pipe->out.size()) {   // this chunk's dHidden rows are final
+      GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p,
+                                                    p.m_tiles * p.n_tiles * k_split, st)));
+      {  // fixed-order sum of the partials (+ scatter of compacted rows) -> dHidden
+        LaunchScope ls(ctx, GRPO_KERNEL_DH_REDUCE, st);
+        splitk_reduce_kernel<<<static_cast<unsigned>(rows), 128, 0, st>>>(
+            reinterpret_cast<const float4*>(dh_part), k_split, L.chunk_rows * c.d / 4, c.d / 4, static_cast<int>(rows),
+            dyn_rows, compact ? row_idx + t0 : nullptr, tile_list ? tile_list + 2 + L.tile_cap : nullptr, TM,
+            compact ? dhidden_out : static_cast<void*>(static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem),
+            c.dhidden_fp32);
+      }
+      CU_OK(cudaGetLastError());
+      if (pipe && pipe->dh_host && chunk_idx < pipe->out.size()) {
+        // packed rows [t0, t0 + rows) are final: compaction preserves order, so every active packed row below
+        // t0 + rows has a compact index below it as well, and rows with a zero coefficient were written first
         CU_OK(cudaEventRecord(pipe->out[chunk_idx], st));
         CU_OK(cudaStreamWaitEvent(pipe->cs, pipe->out[chunk_idx], 0));
         CU_OK(cudaMemcpyAsync(pipe->dh_host + t0 * c.d * dh_elem, static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem,
@@ -683,15 +834,15 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       }
     }
     if (dW_accum) {  // A6: dW[V, d] += dZ^T[V, rows] H[rows, d]
-      GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz, c.V, rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
-      GRPO_TRY(make_tmap(ctx, &tmH_mn, Hc, c.d, rows, static_cast<uint64_t>(c.d) * 2, 64, BK));
+      GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz, c.V, map_rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
+      GRPO_TRY(make_tmap(ctx, &tmH_mn, Hc, c.d, map_rows, static_cast<uint64_t>(c.d) * 2, 64, BK));
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
       p.m_total = c.V; p.n_total = c.d;
       p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
-      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.tile_list = tile_list;
+      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.tile_list = tile_list; p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       CUtensorMap tmDW;
       GRPO_TRY(make_tmap_c_f32(ctx, &tmDW, dW_accum, c.d, c.V, static_cast<uint64_t>(c.d) * 4));
@@ -727,6 +878,7 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hi
   FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
             logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
   a.entropy_out = ctx->entropy_out;
+  a.S_norm = ctx->seq_denom;
   GRPO_TRY(fwd_counts(ctx, 0, targets, a, st));
   return bwd_impl(ctx, 0, hidden, W, targets, lse_out, coeff_out, T, grad_scale, dhidden_out, dW_accum, st, &a);
 }
@@ -795,29 +947,54 @@ static int32_t validate_group(const grpo_ctx* ctx, const grpo_group_desc& g) {
   return GRPO_OK;
 }
 
-// One launch = A1 -> A2/A3 -> A4-A6 over `k` whole groups packed into one token stream.
-static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, const void* W, float* dW_accum,
-                          float* loss_accum, float* metrics_accum, double loss_denom, const float* denom_dev, int slot,
-                          cudaStream_t st) {
-  const grpo_config& c = ctx->cfg;
-  const SlotLayout& L = ctx->lay;
+// Everything about a launch of `k` whole groups that can be rejected WITHOUT touching the device: checked for
+// every launch of a logical update before its first kernel is enqueued, so that a bad update leaves the
+// accumulators and the FIFO untouched (drain_one_update).
+static int32_t validate_launch(const grpo_ctx* ctx, const PendingGroup* groups, int k) {
   int64_t T = 0;
-  int S = 0;
-  bool any_ref = false, all_ref = true, any_mask = false, any_dh = false;
+  int64_t S = 0;
+  bool any_ref = false, all_ref = true;
   for (int i = 0; i < k; ++i) {
     T += groups[i].tokens;
     S += groups[i].desc.G;
     any_ref |= groups[i].desc.ref_logp != nullptr;
     all_ref &= groups[i].desc.ref_logp != nullptr;
+  }
+  if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
+  if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "launch of %lld tokens exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
+  if (S > ctx->lay.s_max) return fail(GRPO_ERR_WORKSPACE, "too many sequences in one launch");
+  if (T > INT32_MAX - 256) return fail(GRPO_ERR_SHAPE, "T too large");
+  if (any_ref && !all_ref) return fail(GRPO_ERR_INVALID_ARG, "ref_logp must be given for all groups of a launch or none");
+  return GRPO_OK;
+}
+
+// One launch = A1 -> A2/A3 -> A4-A6 over `k` whole groups packed into one token stream.  S_update: sequences
+// of the whole logical update (the per-sequence mean of loss_agg 1 averages over all of them, R10).
+static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, const void* W, float* dW_accum,
+                          float* loss_accum, float* metrics_accum, double loss_denom, const float* denom_dev,
+                          int32_t S_update, int slot, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  const SlotLayout& L = ctx->lay;
+  GRPO_TRY(validate_launch(ctx, groups, k));
+  int64_t T = 0;
+  int S = 0;
+  bool any_ref = false, any_mask = false, any_dh = false;
+  for (int i = 0; i < k; ++i) {
+    T += groups[i].tokens;
+    S += groups[i].desc.G;
+    any_ref |= groups[i].desc.ref_logp != nullptr;
     any_mask |= groups[i].desc.mask != nullptr;
     any_dh |= groups[i].desc.dhidden_out != nullptr;
   }
-  if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "launch of %lld tokens exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
-  if (S > L.s_max) return fail(GRPO_ERR_WORKSPACE, "too many sequences in one launch");
-  if (any_ref && !all_ref) return fail(GRPO_ERR_INVALID_ARG, "ref_logp must be given for all groups of a launch or none");
 
-  // small host-built index arrays
-  std::vector<int32_t> cu_seq(S + 1, 0), cu_grp(k + 1, 0);
+  // small host-built index arrays, staged in the context's pinned ring (a pageable source would make the copy
+  // synchronise the stream with the host and serialise multi-stream dispatch)
+  const int ring = ctx->stage_next++ % grpo_ctx::kStageRing;
+  CU_OK(cudaEventSynchronize(ctx->stage_ev[ring]));          // the copies that last used this entry have run
+  int32_t* cu_seq = ctx->stage_host + static_cast<int64_t>(ring) * ctx->stage_ints;
+  int32_t* cu_grp = cu_seq + (L.s_max + 1);
+  cu_seq[0] = 0;
+  cu_grp[0] = 0;
   int s = 0;
   for (int i = 0; i < k; ++i) {
     for (int j = 0; j < groups[i].desc.G; ++j, ++s) cu_seq[s + 1] = cu_seq[s] + groups[i].seqlens[j];
@@ -827,8 +1004,9 @@ static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, cons
   int32_t* d_cu_grp = slot_ptr<int32_t>(ctx, slot, L.off_cu_grp);
   float* d_rewards = slot_ptr<float>(ctx, slot, L.off_rewards);
   float* d_adv = slot_ptr<float>(ctx, slot, L.off_adv);
-  CU_OK(cudaMemcpyAsync(d_cu_seq, cu_seq.data(), (S + 1) * 4, cudaMemcpyHostToDevice, st));
-  CU_OK(cudaMemcpyAsync(d_cu_grp, cu_grp.data(), (k + 1) * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(d_cu_seq, cu_seq, (S + 1) * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(d_cu_grp, cu_grp, (k + 1) * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaEventRecord(ctx->stage_ev[ring], st));
   for (int i = 0; i < k; ++i)
     CU_OK(cudaMemcpyAsync(d_rewards + cu_grp[i], groups[i].desc.rewards, groups[i].desc.G * 4, cudaMemcpyDeviceToDevice, st));
 
@@ -876,13 +1054,14 @@ static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, cons
   if (any_dh) dh = (k == 1) ? groups[0].desc.dhidden_out : static_cast<void*>(slot_ptr<uint8_t>(ctx, slot, L.off_dh));
   if (c.stash_logits) {
     GRPO_TRY(fwd_check(ctx, S, T));
-    const FwdArgs a{d_cu_seq, S, d_adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
-                    logp, lse, coeff, loss_accum, metrics_accum};
+    FwdArgs a{d_cu_seq, S, d_adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
+              logp, lse, coeff, loss_accum, metrics_accum};
+    a.S_norm = S_update;
     GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
     GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st, &a));
   } else {
     GRPO_TRY(fwd_impl(ctx, slot, hidden, W, targets, d_cu_seq, S, T, d_adv, old_logp, ref_logp, mask, loss_denom,
-                      denom_dev, logp, lse, coeff, loss_accum, metrics_accum, st));
+                      denom_dev, logp, lse, coeff, loss_accum, metrics_accum, st, nullptr, S_update));
     GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st));
   }
   if (k > 1) {
@@ -916,6 +1095,16 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
   if (n_streams < 1 || n_streams > ctx->n_slots)
     return fail(GRPO_ERR_WORKSPACE, "n_streams=%d but workspace has %d slots", n_streams, ctx->n_slots);
   std::vector<PendingGroup> upd(ctx->fifo.begin(), ctx->fifo.begin() + take);
+  // reject the whole update before anything is accumulated: every launch is checked first
+  int32_t S_update = 0;
+  {
+    int pos = 0;
+    for (int k : sizes) {
+      GRPO_TRY(validate_launch(ctx, upd.data() + pos, k));
+      pos += k;
+    }
+    for (const auto& g : upd) S_update += g.desc.G;
+  }
 
   // implicit denominator of the whole update: count loss-bearing tokens of all its groups first
   const float* denom_dev = nullptr;
@@ -939,7 +1128,16 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
   for (int k : sizes) {
     const int slot = static_cast<int>(ctx->launches % n_streams);
     cudaStream_t st = static_cast<cudaStream_t>(streams ? streams[slot] : nullptr);
-    GRPO_TRY(run_launch(ctx, upd.data() + pos, k, W, dW_accum, loss_accum, metrics_accum, loss_denom, denom_dev, slot, st));
+    const int32_t rc = run_launch(ctx, upd.data() + pos, k, W, dW_accum, loss_accum, metrics_accum, loss_denom,
+                                  denom_dev, S_update, slot, st);
+    if (rc != GRPO_OK) {
+      // a device-side failure in the middle of an update (everything checkable was checked above): the groups
+      // of the launches that did run are consumed - their gradients are in the accumulators - so that a retry
+      // cannot add them twice; the failed launch and the rest of the update stay at the head of the FIFO
+      ctx->fifo.erase(ctx->fifo.begin(), ctx->fifo.begin() + pos);
+      ctx->consumed += pos;
+      return rc;
+    }
     ctx->launches++;
     pos += k;
   }
@@ -1020,14 +1218,17 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   HostPipe pipe;
   pipe.cs = ctx->copy_stream;
   pipe.dh_host = static_cast<uint8_t*>(dhidden_host);
-  pipe.in.resize(n_chunks, nullptr);
-  pipe.out.resize(dhidden_host ? n_chunks : 0, nullptr);
-  struct Fence { cudaEvent_t e = nullptr; ~Fence() { if (e) cudaEventDestroy(e); } } fence;
-  CU_OK(cudaEventCreateWithFlags(&fence.e, cudaEventDisableTiming));
-  for (auto& e : pipe.in) CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-  for (auto& e : pipe.out) CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-  CU_OK(cudaEventRecord(fence.e, st));                       // staging buffers are free once st reaches here
-  CU_OK(cudaStreamWaitEvent(pipe.cs, fence.e, 0));
+  // events live in the context and are created once (1 fence + n_chunks in + n_chunks out)
+  while (ctx->pipe_events.size() < 1 + 2 * n_chunks) {
+    cudaEvent_t e = nullptr;
+    CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    ctx->pipe_events.push_back(e);
+  }
+  const cudaEvent_t fence = ctx->pipe_events[0];
+  pipe.in.assign(ctx->pipe_events.begin() + 1, ctx->pipe_events.begin() + 1 + n_chunks);
+  if (dhidden_host) pipe.out.assign(ctx->pipe_events.begin() + 1 + n_chunks, ctx->pipe_events.begin() + 1 + 2 * n_chunks);
+  CU_OK(cudaEventRecord(fence, st));                         // staging buffers are free once st reaches here
+  CU_OK(cudaStreamWaitEvent(pipe.cs, fence, 0));
   for (size_t i = 0; i < n_chunks; ++i) {
     const int64_t t0 = static_cast<int64_t>(i) * rpc, rows = std::min<int64_t>(rpc, T - t0);
     CU_OK(cudaMemcpyAsync(sh + t0 * c.d * 2, static_cast<const uint8_t*>(hidden_host) + t0 * c.d * 2, rows * c.d * 2,

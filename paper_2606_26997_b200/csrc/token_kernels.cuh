@@ -84,6 +84,7 @@ struct LossParams {
   int64_t T;                 // tokens handled by this launch: packed rows [t_begin, t_begin + T)
   int64_t t_begin;
   int S, V;
+  int S_norm;                 // loss_agg 1: sequences of the whole logical update (>= S)
   int n_split;
   int64_t part_stride;
   const float* part_m;
@@ -148,7 +149,7 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
       const float denom = p.denom_host > 0.f ? p.denom_host : fmaxf(*p.total_count, 1.f);
       w = m / denom;
     } else {
-      w = m / (fmaxf(p.seq_count[lo], 1.f) * static_cast<float>(p.S));
+      w = m / (fmaxf(p.seq_count[lo], 1.f) * static_cast<float>(p.S_norm));
     }
     float coeff = 0.f;
     if (m != 0.f) {
@@ -233,6 +234,118 @@ __global__ void __launch_bounds__(1024) active_tiles_kernel(const float* __restr
     list[1] = n_tiles;
     if (stats) { atomicAdd(stats, n); atomicAdd(stats + 1, n_tiles); }
   }
+}
+
+// Token-granular zero-coefficient compaction.  coeff_t = dloss/dlogp_t is exactly zero for
+// masked / ignored tokens, for clipped tokens at kl_beta = 0 (the clipped surrogate has no gradient
+// there) and for every token of a zero-variance group at kl_beta = 0; their dZ rows are zero, so the backward
+// contractions run only over the other rows.  One block: an order-preserving stream compaction of the call's T
+// rows.  row_idx[0 .. n_active) = packed rows with coeff != 0, ascending.  meta[0] = n_active, meta[1] = T,
+// meta[2 + c] = rows of backward chunk c = clamp(n_active - c * chunk_rows, 0, chunk_rows) for c < n_chunks.
+// stats (nullable): [0] += n_active, [1] += T.
+__global__ void __launch_bounds__(1024) compact_rows_kernel(const float* __restrict__ coeff, int T, int chunk_rows,
+                                                            int n_chunks, int* __restrict__ row_idx,
+                                                            int* __restrict__ meta, long long* __restrict__ stats) {
+  __shared__ int warp_cnt[32];
+  __shared__ int base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) base_s = 0;
+  __syncthreads();
+  for (int t0 = 0; t0 < T; t0 += 1024) {
+    const int t = t0 + threadIdx.x;
+    const bool act = t < T && coeff[t] != 0.f;
+    const unsigned bal = __ballot_sync(0xffffffffu, act);
+    if (lane == 0) warp_cnt[warp] = __popc(bal);
+    __syncthreads();
+    int before = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < 32; ++w) {
+      const int c = warp_cnt[w];
+      before += w < warp ? c : 0;
+      total += c;
+    }
+    const int base = base_s;
+    if (act) row_idx[base + before + __popc(bal & ((1u << lane) - 1u))] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) base_s = base + total;
+  }
+  __syncthreads();
+  const int n_active = base_s;
+  if (threadIdx.x == 0) {
+    meta[0] = n_active;
+    meta[1] = T;
+    if (stats) { atomicAdd(reinterpret_cast<unsigned long long*>(stats), static_cast<unsigned long long>(n_active));
+                 atomicAdd(reinterpret_cast<unsigned long long*>(stats + 1), static_cast<unsigned long long>(T)); }
+  }
+  for (int c = threadIdx.x; c < n_chunks; c += blockDim.x)
+    meta[2 + c] = max(0, min(chunk_rows, n_active - c * chunk_rows));
+}
+
+// Gather one backward chunk of active rows: Hc[r,:] = H[row_idx[r],:] and the per-row inputs of the dZ epilogue
+// (target, lse, coeff) for r < rows = *dyn_rows; rows [rows, round_up(rows, tile_rows)) are zero-filled (zero
+// hidden state, coeff 0, target -1): they are the tail of the last token tile A4 walks and of the last k block
+// A6 reduces over.  One block per destination row; 16-byte accesses (d % 8 == 0).
+__global__ void __launch_bounds__(128) gather_rows_kernel(const uint4* __restrict__ H, int64_t row_vec /* d / 8 */,
+                                                          const int* __restrict__ row_idx,
+                                                          const int* __restrict__ dyn_rows, int tile_rows,
+                                                          int rows_alloc, const int32_t* __restrict__ targets,
+                                                          const float* __restrict__ lse, const float* __restrict__ coeff,
+                                                          uint4* __restrict__ Hc, int32_t* __restrict__ yc,
+                                                          float* __restrict__ lsec, float* __restrict__ coeffc) {
+  const int r = blockIdx.x;
+  const int rows = *dyn_rows;
+  const int rows_pad = min(rows_alloc, (rows + tile_rows - 1) / tile_rows * tile_rows);
+  if (r >= rows_pad) return;
+  uint4* dst = Hc + static_cast<int64_t>(r) * row_vec;
+  if (r < rows) {
+    const int t = row_idx[r];
+    const uint4* src = H + static_cast<int64_t>(t) * row_vec;
+    for (int64_t i = threadIdx.x; i < row_vec; i += blockDim.x) dst[i] = src[i];
+    if (threadIdx.x == 0) { yc[r] = targets[t]; lsec[r] = lse[t]; coeffc[r] = coeff[t]; }
+  } else {
+    for (int64_t i = threadIdx.x; i < row_vec; i += blockDim.x) dst[i] = make_uint4(0u, 0u, 0u, 0u);
+    if (threadIdx.x == 0) { yc[r] = -1; lsec[r] = 0.f; coeffc[r] = 0.f; }
+  }
+}
+
+// Split-K reduction of A5 (and the scatter of compacted rows back to their packed positions):
+// out[dst(r), :] = ((part_0[r,:] + part_1[r,:]) + part_2[r,:]) + ...   in that fixed order, r < rows.
+// dst(r) = row_idx[r] if row_idx != nullptr, else r.  tile_flags (nullable): rows of token tiles with flag 0 were
+// never computed (tile skipping of the stash variant) and are left alone.  One block per row; 16-byte accesses.
+__global__ void __launch_bounds__(128) splitk_reduce_kernel(const float4* __restrict__ parts, int k_split,
+                                                            int64_t split_stride_vec, int64_t row_vec /* d / 4 */,
+                                                            int rows_static, const int* __restrict__ dyn_rows,
+                                                            const int* __restrict__ row_idx,
+                                                            const int* __restrict__ tile_flags, int tile_rows,
+                                                            void* __restrict__ out, int out_fp32) {
+  const int r = blockIdx.x;
+  const int rows = dyn_rows ? min(rows_static, *dyn_rows) : rows_static;
+  if (r >= rows) return;
+  if (tile_flags != nullptr && tile_flags[r / tile_rows] == 0) return;
+  const int64_t dst_row = row_idx ? row_idx[r] : r;
+  const float4* src = parts + static_cast<int64_t>(r) * row_vec;
+  for (int64_t i = threadIdx.x; i < row_vec; i += blockDim.x) {
+    float4 a = src[i];
+    for (int k = 1; k < k_split; ++k) {
+      const float4 b = src[k * split_stride_vec + i];
+      a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+    }
+    if (out_fp32) {
+      reinterpret_cast<float4*>(out)[dst_row * row_vec + i] = a;
+    } else {
+      reinterpret_cast<uint2*>(out)[dst_row * row_vec + i] = make_uint2(pack_bf16x2(a.x, a.y), pack_bf16x2(a.z, a.w));
+    }
+  }
+}
+
+// dHidden rows of tokens with a zero coefficient are zeros (what the dense A5 gives for an all-zero dZ row).
+// One block per packed row; 16-byte stores (row_bytes % 16 == 0).
+__global__ void __launch_bounds__(128) zero_coeff_rows_kernel(const float* __restrict__ coeff, int T,
+                                                              uint8_t* __restrict__ out, int64_t row_bytes) {
+  const int t = blockIdx.x;
+  if (t >= T || coeff[t] != 0.f) return;
+  uint4* dst = reinterpret_cast<uint4*>(out + static_cast<int64_t>(t) * row_bytes);
+  for (int64_t i = threadIdx.x; i < row_bytes / 16; i += blockDim.x) dst[i] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 // 3-contraction variant: turn the stashed exponentials e = 2^(z2 - m) (fp16, written by the

@@ -33,7 +33,8 @@ def _tiny(seed=0, T_per=(3, 4, 2, 3), d=5, V=7, G=2, spread=0.15, scale=1.0):
 
 # ------------------------------------------------------------------ P1-P3: advantage
 def test_golden_eq1_closed_forms():
-    """tests/golden/advantage_closed_form.txt: values derived by hand from Eq. 1."""
+    """tests/golden/advantage_closed_form.txt: closed forms of Eq. 1 in 40-digit decimal arithmetic, written by
+    tests/golden/make_advantage_closed_form.py (standard library only)."""
     import os
     path = os.path.join(os.path.dirname(__file__), "golden", "advantage_closed_form.txt")
     n = 0
@@ -384,6 +385,46 @@ def test_step10_blas_path_equals_loops_path():
     assert a["metrics"][0] == mm.sum()
     np.testing.assert_allclose(a["metrics"][1], a["rho"][mm].sum(), rtol=1e-13)
     np.testing.assert_allclose(a["metrics"][3], (a["u"][mm] == 0).sum())
+
+
+def test_metrics_and_loss_hand_evaluated_five_tokens():
+    """Pins loss_terms()["metrics"] (all four entries) and the loss on five tokens worked by hand from SURVEY.md
+    §8(c) steps 5-8, clip range [0.8, 1.28], beta = 0.5, token mean (denominator = 4 loss-bearing tokens):
+
+      t  A   rho  ref-logp  mask   surrogate s = min(rho A, clip(rho) A)   clipped (step 9)   k3 = e^d - d - 1
+      0  +1  1.5   ln 2      1     min(1.5, 1.28)   =  1.28                 yes (A>0, rho>hi)  2 - ln2 - 1 = 1 - ln2
+      1  +1  0.5   0         1     min(0.5, 0.8)    =  0.5                  no                 0
+      2  -1  0.5  -ln 2      1     min(-0.5, -0.8)  = -0.8                  yes (A<0, rho<lo)  1/2 + ln2 - 1 = ln2 - 1/2
+      3  -1  1.5   0         0     (masked: contributes to nothing)
+      4  -1  1.1   ln 2      1     min(-1.1, -1.1)  = -1.1                  no                 1 - ln2
+
+    metrics = {tokens, sum rho, sum k3, clipped tokens} = {4, 1.5+0.5+0.5+1.1 = 3.6, 3/2 - ln 2, 2};
+    loss = [(-1.28 - 0.5 + 0.8 + 1.1) + 0.5 (3/2 - ln 2)] / 4 = (0.12 + 0.75 - 0.5 ln 2) / 4."""
+    ln2 = 0.6931471805599453
+    rho = np.array([1.5, 0.5, 0.5, 1.5, 1.1])
+    logp = np.array([-1.0, -2.0, -0.5, -3.0, -1.5])
+    old = logp - np.log(rho)
+    ref = logp + np.array([ln2, 0.0, -ln2, 0.0, ln2])
+    A_tok = np.array([1.0, 1.0, -1.0, -1.0, -1.0])
+    mask = np.array([1, 1, 1, 0, 1], dtype=np.uint8)
+    cfg = OracleConfig(clip_lo=0.2, clip_hi=0.28, kl_beta=0.5)
+    lt = loss_terms(logp, old, ref, mask, A_tok, np.array([0, 2, 5]), cfg)
+    np.testing.assert_allclose(lt["metrics"], [4.0, 3.6, 0.8068528194400547, 2.0], rtol=1e-13)
+    np.testing.assert_allclose(lt["loss"], 0.13085660243000684, rtol=1e-13)
+    np.testing.assert_allclose(lt["surr"][mask != 0], [1.28, 0.5, -0.8, -1.1], rtol=1e-13)
+    # coefficient c_t = w_t [-A rho u + beta (1 - e^d)]: t0 clipped -> 0.5 (1 - 2) / 4; t1 -> (-0.5 + 0) / 4;
+    # t2 clipped -> 0.5 (1 - 1/2) / 4; t3 masked -> 0; t4 -> (1.1 + 0.5 (1 - 2)) / 4
+    np.testing.assert_allclose(lt["coeff"], [-0.125, -0.125, 0.0625, 0.0, 0.15], rtol=1e-12, atol=1e-16)
+    # per-sequence mean (mode 1): weights 1/(2*2) for sequence 0, 1/(2*2) for the 2 loss-bearing tokens of sequence 1
+    cfg1 = OracleConfig(clip_lo=0.2, clip_hi=0.28, kl_beta=0.5, loss_agg=1)
+    lt1 = loss_terms(logp, old, ref, mask, A_tok, np.array([0, 2, 5]), cfg1)
+    np.testing.assert_allclose(lt1["metrics"], [4.0, 3.6, 0.8068528194400547, 2.0], rtol=1e-13)
+    np.testing.assert_allclose(lt1["loss"], 0.13085660243000684, rtol=1e-13)   # both sequences have 2 such tokens
+    # the k1 / k2 estimators put their own values into metrics[2]: k1 = -d, k2 = d^2 / 2 (DESIGN.md R26)
+    lt_k1 = loss_terms(logp, old, ref, mask, A_tok, np.array([0, 2, 5]), OracleConfig(kl_beta=0.5, kl_type=1))
+    np.testing.assert_allclose(lt_k1["metrics"][2], -(ln2 + 0.0 - ln2 + ln2), rtol=1e-13)
+    lt_k2 = loss_terms(logp, old, ref, mask, A_tok, np.array([0, 2, 5]), OracleConfig(kl_beta=0.5, kl_type=2))
+    np.testing.assert_allclose(lt_k2["metrics"][2], 1.5 * ln2 * ln2, rtol=1e-13)
 
 
 def test_bf16_widening_is_exact():

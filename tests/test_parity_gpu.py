@@ -30,7 +30,7 @@ def _check(b, ctx_kw=None, oracle_kw=None, loss_denom=0.0, grad_scale=1.0):
     if grad_scale != 1.0:
         ref["dH"] *= grad_scale
         ref["dW"] *= grad_scale
-    e = gates(b, out, ref, logit_scale=okw.get("logit_scale", 1.0))
+    e = gates(b, out, ref, logit_scale=okw.get("logit_scale", 1.0), grad_scale=grad_scale)
     assert_gates(e)
     return out, ref, e
 

@@ -57,19 +57,19 @@ def _skippable_batch(beta=0.0):
 
 
 @pytest.mark.parametrize("cg", [2, 1])
-def test_zero_tiles_are_skipped_and_results_match_the_oracle(cg):
+def test_zero_coefficient_rows_are_skipped_and_results_match_the_oracle(cg):
     b = _skippable_batch()
     ctx = make_ctx(b, gemm_cta_group=cg, bwd_chunk_tokens=2048, dhidden_fp32=1)
     try:
         ctx.ensure_workspace(b.T)
-        ctx.grpo_bwd_tile_stats_sync()
+        ctx.grpo_bwd_row_stats_sync()
         out = run_cuda(ctx, b)
-        active, total = ctx.grpo_bwd_tile_stats_sync()
+        active, total = ctx.grpo_bwd_row_stats_sync()
     finally:
         ctx.close()
     ref = run_oracle(b)
     assert_gates(gates(b, out, ref))
-    assert 0 < active < total and active <= 0.75 * total, (active, total)
+    assert total == b.T and active == int((ref["coeff"] != 0.0).sum()) and active <= 0.75 * total, (active, total)
     # rows of zero-coefficient tokens are exact zeros, as in the dense computation
     zero_rows = ref["coeff"] == 0.0
     assert zero_rows.sum() > 1000
@@ -83,14 +83,14 @@ def test_skipping_on_and_off_agree():
         ctx = make_ctx(b, bwd_skip_zero_tiles=skip, bwd_chunk_tokens=2048)
         try:
             ctx.ensure_workspace(b.T)
-            ctx.grpo_bwd_tile_stats_sync()
+            ctx.grpo_bwd_row_stats_sync()
             outs.append(run_cuda(ctx, b))
-            st = ctx.grpo_bwd_tile_stats_sync()
+            st = ctx.grpo_bwd_row_stats_sync()
             assert (st[1] > 0) == (skip == 0)
         finally:
             ctx.close()
-    assert torch.equal(outs[0]["dH"], outs[1]["dH"])                     # every active tile is computed identically
-    assert rel_l2(to64(outs[0]["dW"]), to64(outs[1]["dW"])) < 1e-6       # fp32 atomics: order only
+    assert torch.equal(outs[0]["dH"], outs[1]["dH"])                     # every active row is computed identically
+    assert rel_l2(to64(outs[0]["dW"]), to64(outs[1]["dW"])) < 1e-5       # other rows share a k block: summation order only
 
 
 def test_nothing_is_skipped_when_the_kl_term_gives_every_token_a_gradient():
@@ -99,9 +99,9 @@ def test_nothing_is_skipped_when_the_kl_term_gives_every_token_a_gradient():
     ctx = make_ctx(b, bwd_chunk_tokens=2048)
     try:
         ctx.ensure_workspace(b.T)
-        ctx.grpo_bwd_tile_stats_sync()
+        ctx.grpo_bwd_row_stats_sync()
         out = run_cuda(ctx, b)
-        active, total = ctx.grpo_bwd_tile_stats_sync()
+        active, total = ctx.grpo_bwd_row_stats_sync()
     finally:
         ctx.close()
     assert active == total > 0
