@@ -286,7 +286,7 @@ def run_ours(args):
         assert world == 1, "--sweep-T is a one-GPU informational run"
         return run_sweep_T(args, dev)
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
-    b = make_config(args.config, seed=rank_seed(rank), device=dev)
+    b = make_config(args.config, seed=rank_seed(rank), device=dev, prenorm=args.prenorm)
     if args.cgp_mode != "full":
         return run_cgp_stream(args, b, dev, world)
     T, d, V = b.T, b.d, b.V
@@ -309,12 +309,22 @@ def run_ours(args):
                                             b.mask, loss_accum=loss)
         ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW, dhidden_out=dH)
 
+    dgamma = torch.zeros(d, dtype=torch.float32, device=dev)
+
+    def step_prenorm():         # NEXT-4 (informational): final RMSNorm -> north_star path -> dx, dgamma, dW
+        Hn, rstd = ctx.grpo_rmsnorm_fwd(b.x_prenorm, b.gamma, b.eps_rms)
+        adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+        f = ctx.grpo_fused_logprob_loss_fwd(Hn, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp, b.mask,
+                                            loss_accum=loss)
+        ctx.grpo_fused_logprob_loss_bwd_prenorm(b.x_prenorm, b.gamma, rstd, Hn, b.W, b.targets, f["lse"], f["coeff"],
+                                                dgamma, dW_accum=dW)
+
     def step_stash():           # 3-contraction variant: logits stashed per chunk
         adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
         ctx.grpo_fused_logprob_loss_fwd_bwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
                                             b.mask, loss_accum=loss, dW_accum=dW, dhidden_out=dH)
 
-    step = step_stash if args.stash else step_recompute
+    step = step_prenorm if args.prenorm else (step_stash if args.stash else step_recompute)
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -342,6 +352,34 @@ def run_ours(args):
     launches = sum(n1.values()) - sum(n0.values())
     loss_val = loss.item()
     assert loss_val == loss_val, "loss is NaN"
+
+    # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step.  Timed
+    # right after the headline region so that both see the same thermal / power state of the board.
+    e2e_s, h2d, d2h = 0.0, 0, 0
+    if args.config == 2 and not args.prenorm:
+        pin = lambda t: None if t is None else t.cpu().pin_memory()
+        h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
+                                                       pin(b.old_logp))
+        h_logp = torch.empty(T, dtype=torch.float32).pin_memory()
+        h_dh = torch.empty(T, d, dtype=torch.bfloat16).pin_memory()
+        h_loss = torch.zeros(1, dtype=torch.float32).pin_memory()
+
+        def step_host():
+            ctx.grpo_step_host(h_hidden, h_targets, h_cu, h_rewards, h_old, b.n_groups, b.G, b.W, dW, loss_h=h_loss,
+                               logp_h=h_logp, dhidden_h=h_dh)
+
+        for _ in range(2):
+            step_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step_host()                     # synchronises its stream before returning: the host has the results
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        barrier()
+        h2d = sum(t.numel() * t.element_size() for t in (h_hidden, h_targets, h_cu, h_rewards, h_old))
+        d2h = sum(t.numel() * t.element_size() for t in (h_logp, h_dh, h_loss))
+
 
     # ---- the same K steps once more with a CUDA event pair around every kernel launch (recorded by the library on
     # the launch stream): per-kernel times for the roofline; the pass's own total is reported beside the headline
@@ -390,7 +428,7 @@ def run_ours(args):
 
     # ---- the other variant of the step, timed the same way (reported beside the headline, never as it)
     args.other_variant = None
-    if not args.no_variants:
+    if not args.no_variants and not args.prenorm:
         other = step_recompute if args.stash else step_stash
         for _ in range(3):
             other()
@@ -407,9 +445,8 @@ def run_ours(args):
                               "value": v_tok * args.steps / (v_ms * 1e-3), "unit": UNIT,
                               "ms_per_step": v_ms / args.steps}
 
-    # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step
-    # (headline workload only; --config 3/4/5 are informational device-resident runs)
-    if args.config != 2:
+    # ---- informational runs (--config 3/4/5, --prenorm) are device-resident: no e2e / cpu_baseline legs
+    if args.config != 2 or args.prenorm:
         ms_total, _, tokens_all = reduce_over_ranks(ms_total, 0.0, T, world, dev)
         if rank == 0:
             line = build_line(args, b, world, tokens_all * args.steps / (ms_total * 1e-3), ms_total, None, 0, 0,
@@ -419,29 +456,6 @@ def run_ours(args):
         if world > 1:
             dist.destroy_process_group()
         return 0
-    pin = lambda t: None if t is None else t.cpu().pin_memory()
-    h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
-                                                   pin(b.old_logp))
-    h_logp = torch.empty(T, dtype=torch.float32).pin_memory()
-    h_dh = torch.empty(T, d, dtype=torch.bfloat16).pin_memory()
-    h_loss = torch.zeros(1, dtype=torch.float32).pin_memory()
-
-    def step_host():
-        ctx.grpo_step_host(h_hidden, h_targets, h_cu, h_rewards, h_old, b.n_groups, b.G, b.W, dW, loss_h=h_loss,
-                           logp_h=h_logp, dhidden_h=h_dh)
-
-    for _ in range(2):
-        step_host()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step_host()                     # synchronises its stream before returning: the host has the results
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    barrier()
-    h2d = sum(t.numel() * t.element_size() for t in (h_hidden, h_targets, h_cu, h_rewards, h_old))
-    d2h = sum(t.numel() * t.element_size() for t in (h_logp, h_dh, h_loss))
-
     # ---- reduce over ranks: max time, sum tokens
     ms_total, e2e_s, tokens_all = reduce_over_ranks(ms_total, e2e_s, T, world, dev)
     value = tokens_all * args.steps / (ms_total * 1e-3)
@@ -645,7 +659,8 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config],
-                   "variant": "stash_logits (3 contractions, DESIGN.md section 11)" if args.stash
+                   "variant": "prenorm (informational, NEXT-4): RMSNorm fwd + north_star path + RMSNorm bwd fused behind A5"
+                   if args.prenorm else "stash_logits (3 contractions, DESIGN.md section 11)" if args.stash
                    else "recompute (north_star: 4 contractions)",
                    "tokens_per_step": int(tokens_all), "tokens_rank0": T, "d": d, "V": V, "G": b.G,
                    "parallelism": f"replicas x{world}: independent complete groups, no collective",
@@ -680,6 +695,9 @@ def main():
     ap.add_argument("--stash", action="store_true",
                     help="time grpo_fused_logprob_loss_fwd_bwd (3-contraction variant) as the step instead of the "
                          "north_star forward + recomputing backward")
+    ap.add_argument("--prenorm", action="store_true",
+                    help="informational (NEXT-4): the step starts from pre-norm activations (grpo_rmsnorm_fwd, forward, "
+                         "grpo_fused_logprob_loss_bwd_prenorm); no e2e / cpu_baseline legs")
     ap.add_argument("--no-variants", action="store_true", help="do not time the other variant beside the headline")
     ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")

@@ -147,6 +147,32 @@ int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden, const voi
  * grpo_enqueue_groups / grpo_step_host. */
 int32_t grpo_set_entropy_out(grpo_ctx* ctx, float* entropy_out);
 
+/* ---- NEXT-4: the step before the path, the final RMSNorm, and its backward ----------
+ * BASELINE.json configs describe the path's input as "hidden ... after RMSNorm-like scaling"; these calls take the
+ * PRE-norm activations x bf16 [T, d] and the norm weight gamma bf16 [d] instead (R29-R31).
+ *
+ * grpo_rmsnorm_fwd: rstd_t = 1 / sqrt(mean_k x_tk^2 + eps_rms);  hidden_out[t,:] = bf16(gamma * x[t,:] * rstd_t)
+ * (fp32 arithmetic, rounded once: the contraction kernels consume H as bf16 tiles through TMA, so H is materialised
+ * by this one-pass HBM-bound kernel - 4 d bytes of traffic per token against 8 V d FLOPs).  rstd_out fp32 [T] is kept
+ * for the backward.  x, gamma, hidden_out 8-byte aligned.
+ *
+ * grpo_fused_logprob_loss_bwd_prenorm: grpo_fused_logprob_loss_bwd with the RMSNorm backward fused behind A5: the
+ * fp32 dHidden row coming out of the split-K reduction is turned, in registers, into
+ *     dx[t,:] = rstd_t (g - xh mean_k(g xh)),   g = gamma * dH[t,:],  xh = x[t,:] rstd_t,
+ * and dgamma_accum fp32 [d] += sum_t dH[t,:] * xh (ADDED to, like dW).  dHidden itself is never written.
+ * dx_out [T, d] (bf16, or fp32 if cfg.dhidden_fp32) is OVERWRITTEN.  d <= 8192.
+ *
+ * grpo_rmsnorm_bwd: the same backward as a stand-alone HBM-bound kernel for a dHidden that already exists
+ * (e.g. the per-group dhidden_out of grpo_enqueue_groups): dhidden bf16 [T, d], or fp32 if dhidden_is_fp32. */
+int32_t grpo_rmsnorm_fwd(grpo_ctx* ctx, const void* x, const void* gamma, float eps_rms, int64_t T, void* hidden_out,
+                         float* rstd_out, void* stream);
+int32_t grpo_rmsnorm_bwd(grpo_ctx* ctx, const void* x, const void* gamma, const float* rstd, const void* dhidden,
+                         int32_t dhidden_is_fp32, int64_t T, void* dx_out, float* dgamma_accum, void* stream);
+int32_t grpo_fused_logprob_loss_bwd_prenorm(grpo_ctx* ctx, const void* x, const void* gamma, const float* rstd,
+                                            const void* hidden, const void* W, const int32_t* targets,
+                                            const float* lse, const float* coeff, int64_t T, float grad_scale,
+                                            void* dx_out, float* dgamma_accum, float* dW_accum, void* stream);
+
 /* 3-contraction variant of forward + backward in ONE call.
  * Per chunk of bwd_chunk_tokens tokens: the forward contraction (A2) also writes the chunk's softmax numerators
  * as fp16 into the workspace chunk buffer, A3 runs on the chunk, an HBM-bound pass turns the stashed logits into
@@ -243,8 +269,10 @@ enum {
   GRPO_KERNEL_TILE_SCAN = 8,   /* backward: zero-coefficient tile scan + zero fill of skipped dHidden rows */
   GRPO_KERNEL_STASH_DZ = 9,    /* 3-contraction variant: stashed logits -> dZ in place */
   GRPO_KERNEL_COMPACT = 10,    /* backward: zero-coefficient row compaction, gather of active rows, zero fill */
-  GRPO_KERNEL_DH_REDUCE = 11,  /* A5: fixed-order sum of the split-K partials (+ scatter of compacted rows) */
-  GRPO_NUM_KERNEL_KINDS = 12
+  GRPO_KERNEL_DH_REDUCE = 11,  /* A5: fixed-order sum of the split-K partials (+ scatter of compacted rows; + the
+                                  RMSNorm backward of the pre-norm calls) */
+  GRPO_KERNEL_RMSNORM = 12,    /* NEXT-4: final RMSNorm forward */
+  GRPO_NUM_KERNEL_KINDS = 13
 };
 
 /* Token tiles the 3-contraction backward calls of workspace slot 0 walked (active) and saw (total) since the last
@@ -264,6 +292,12 @@ int32_t grpo_kernel_launches(const grpo_ctx* ctx, int64_t* counts_out);
  * (HOST int64 [GRPO_NUM_KERNEL_KINDS]), and clears the records.  Disabling discards records. */
 int32_t grpo_profile_enable(grpo_ctx* ctx, int32_t on);
 int32_t grpo_profile_read_sync(grpo_ctx* ctx, double* ms_out, int64_t* launches_out);
+
+/* Diagnostic: how many thread-block clusters of `cluster_size` CTAs of the contraction kernel (224 threads, its
+ * full shared-memory ring) the device can hold at once (cudaOccupancyMaxActiveClusters).  clusters_out HOST.
+ * The kernels run as 74 CTA pairs; DESIGN.md section 5 records why larger multicast clusters are not used
+ * (148 CTAs co-resident at cluster size 2, 132 at 4, 120 at 8 on B200). */
+int32_t grpo_debug_max_active_clusters(grpo_ctx* ctx, int32_t cluster_size, int32_t* clusters_out);
 
 /* Test hook: C[M,N] (fp32, row-major, pitch N) = A * B with the production tcgen05 kernel.
  * layout 0: A [M,K] K-major, B [N,K] K-major;  1: A [M,K] K-major, B [K,N] MN-major;

@@ -21,12 +21,13 @@ EXPORTS = [
     "grpo_default_config", "grpo_create", "grpo_destroy", "grpo_last_error", "grpo_workspace_bytes",
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
     "grpo_fused_logprob_loss_fwd_bwd", "grpo_set_entropy_out", "grpo_set_seq_denom", "grpo_bwd_row_stats_sync",
+    "grpo_rmsnorm_fwd", "grpo_rmsnorm_bwd", "grpo_fused_logprob_loss_bwd_prenorm", "grpo_debug_max_active_clusters",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
     "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
 ]
 KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan", "stash_dz",
-                "compact", "dh_reduce"]
+                "compact", "dh_reduce", "rmsnorm"]
 
 
 class GrpoError(RuntimeError):
@@ -95,6 +96,10 @@ def load_library() -> C.CDLL:
     lib.grpo_bwd_tile_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     lib.grpo_set_entropy_out.argtypes = [vp, vp]
     lib.grpo_set_seq_denom.argtypes = [vp, i32]
+    lib.grpo_debug_max_active_clusters.argtypes = [vp, i32, C.POINTER(i32)]
+    lib.grpo_rmsnorm_fwd.argtypes = [vp, vp, vp, f32, i64, vp, vp, vp]
+    lib.grpo_rmsnorm_bwd.argtypes = [vp, vp, vp, vp, vp, i32, i64, vp, vp, vp]
+    lib.grpo_fused_logprob_loss_bwd_prenorm.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, f32, vp, vp, vp, vp]
     lib.grpo_bwd_row_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     _LIB = lib
     return lib
@@ -243,6 +248,44 @@ class GrpoContext:
             _dev(dW_accum, torch.float32, "dW_accum", self.cfg.V * self.cfg.d), _stream(stream)))
         return dhidden_out
 
+    # ------------------------------------------------------------------ NEXT-4: final RMSNorm in front of the path
+    def grpo_rmsnorm_fwd(self, x, gamma, eps_rms: float = 1e-6, stream=None):
+        T, d = x.shape
+        H = torch.empty(T, d, dtype=torch.bfloat16, device=x.device)
+        rstd = torch.empty(T, dtype=torch.float32, device=x.device)
+        _check(self.lib.grpo_rmsnorm_fwd(self.h, _dev(x, torch.bfloat16, "x", T * self.cfg.d),
+                                         _dev(gamma, torch.bfloat16, "gamma", self.cfg.d), float(eps_rms), T,
+                                         _dev(H, torch.bfloat16, "H"), _dev(rstd, torch.float32, "rstd"), _stream(stream)))
+        return H, rstd
+
+    def _dx_like(self, x):
+        return torch.empty(x.shape, dtype=torch.float32 if self.cfg.dhidden_fp32 else torch.bfloat16, device=x.device)
+
+    def grpo_rmsnorm_bwd(self, x, gamma, rstd, dhidden, dgamma_accum, stream=None):
+        T, d = x.shape
+        dx = self._dx_like(x)
+        if dhidden.dtype not in (torch.float32, torch.bfloat16) or not dhidden.is_contiguous():
+            raise TypeError("dhidden: need a contiguous bf16 or fp32 CUDA tensor")
+        _check(self.lib.grpo_rmsnorm_bwd(self.h, _dev(x, torch.bfloat16, "x", T * d), _dev(gamma, torch.bfloat16, "gamma", d),
+                                         _dev(rstd, torch.float32, "rstd", T), C.c_void_p(dhidden.data_ptr()),
+                                         int(dhidden.dtype == torch.float32), T, C.c_void_p(dx.data_ptr()),
+                                         _dev(dgamma_accum, torch.float32, "dgamma_accum", d), _stream(stream)))
+        return dx
+
+    def grpo_fused_logprob_loss_bwd_prenorm(self, x, gamma, rstd, hidden, W, targets, lse, coeff, dgamma_accum,
+                                            dW_accum=None, grad_scale: float = 1.0, stream=None):
+        T, d = hidden.shape
+        self.ensure_workspace(T, 1)
+        dx = self._dx_like(x)
+        _check(self.lib.grpo_fused_logprob_loss_bwd_prenorm(
+            self.h, _dev(x, torch.bfloat16, "x", T * d), _dev(gamma, torch.bfloat16, "gamma", d),
+            _dev(rstd, torch.float32, "rstd", T), _dev(hidden, torch.bfloat16, "hidden", T * d), _dev(W, torch.bfloat16, "W"),
+            _dev(targets, torch.int32, "targets", T), _dev(lse, torch.float32, "lse", T),
+            _dev(coeff, torch.float32, "coeff", T), T, float(grad_scale), C.c_void_p(dx.data_ptr()),
+            _dev(dgamma_accum, torch.float32, "dgamma_accum", d),
+            _dev(dW_accum, torch.float32, "dW_accum", self.cfg.V * self.cfg.d), _stream(stream)))
+        return dx
+
     # ------------------------------------------------------------------ A2 - A6 in one call (3-contraction variant)
     def grpo_fused_logprob_loss_fwd_bwd(self, hidden, W, targets, cu_seqlens, adv, old_logp, ref_logp=None, mask=None,
                                         loss_denom: float = 0.0, grad_scale: float = 1.0, loss_accum=None,
@@ -380,6 +423,11 @@ class GrpoContext:
         a, t = C.c_int64(0), C.c_int64(0)
         _check(self.lib.grpo_bwd_tile_stats_sync(self.h, C.byref(a), C.byref(t)))
         return a.value, t.value
+
+    def grpo_debug_max_active_clusters(self, cluster_size: int) -> int:
+        n = C.c_int32(0)
+        _check(self.lib.grpo_debug_max_active_clusters(self.h, int(cluster_size), C.byref(n)))
+        return n.value
 
     # ------------------------------------------------------------------ test hook
     def grpo_debug_gemm(self, layout: int, A, B, M: int, N: int, K: int, C_out=None, accumulate: bool = False,

@@ -690,9 +690,40 @@ struct HostPipe {
 //     on that panel with the row count read from device memory, and the split-K reduction of A5 scatters the
 //     dHidden rows back; rows with coeff == 0 are written as zeros.  Nothing is decided on the host.
 //   3-contraction variant: per 256-row token tile (the chunk's logits are stashed before its coefficients exist).
+// RMSNorm in front of the path: when given, the A5 reduction turns each dHidden row into
+// dx (written to `dhidden_out`, which is then the dx buffer) and adds its share of dgamma.
+struct PrenormArgs { const void* x; const void* gamma; const float* rstd; float* dgamma; };
+
+static int32_t launch_prenorm_bwd(grpo_ctx* ctx, bool in_bf16, const void* parts, int k_split, int64_t split_stride_vec,
+                                  int rows, const int* dyn_rows, const int* row_idx, int64_t row0, const PrenormArgs& pn,
+                                  void* dx_out, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  const int row_vec = c.d / 4;
+  const int J = (row_vec + 255) / 256;
+  if (J > 8) return fail(GRPO_ERR_SHAPE, "RMSNorm backward supports d <= 8192 (got %d)", c.d);
+  const int grid = std::min(rows, 4 * ctx->num_sms);
+  if (grid <= 0) return GRPO_OK;
+  LaunchScope ls(ctx, GRPO_KERNEL_DH_REDUCE, st);
+#define GRPO_PN(JJ)                                                                                                   \
+  do {                                                                                                                \
+    if (in_bf16)                                                                                                      \
+      prenorm_bwd_kernel<JJ, true><<<grid, 256, 0, st>>>(parts, k_split, split_stride_vec, row_vec, rows, dyn_rows,   \
+          row_idx, row0, static_cast<const uint2*>(pn.x), static_cast<const uint2*>(pn.gamma), pn.rstd, 1.f / c.d,    \
+          dx_out, c.dhidden_fp32, pn.dgamma);                                                                         \
+    else                                                                                                              \
+      prenorm_bwd_kernel<JJ, false><<<grid, 256, 0, st>>>(parts, k_split, split_stride_vec, row_vec, rows, dyn_rows,  \
+          row_idx, row0, static_cast<const uint2*>(pn.x), static_cast<const uint2*>(pn.gamma), pn.rstd, 1.f / c.d,    \
+          dx_out, c.dhidden_fp32, pn.dgamma);                                                                         \
+  } while (0)
+  if (J <= 1) GRPO_PN(1); else if (J <= 2) GRPO_PN(2); else if (J <= 4) GRPO_PN(4); else GRPO_PN(8);
+#undef GRPO_PN
+  return GRPO_OK;
+}
+
 static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
                         const float* lse, const float* coeff, int64_t T, float grad_scale, void* dhidden_out,
-                        float* dW_accum, cudaStream_t st, const FwdArgs* fused = nullptr, HostPipe* pipe = nullptr) {
+                        float* dW_accum, cudaStream_t st, const FwdArgs* fused = nullptr, HostPipe* pipe = nullptr,
+                        const PrenormArgs* pn = nullptr) {
   const grpo_config& c = ctx->cfg;
   if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
   if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
@@ -815,7 +846,11 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p,
                                                     p.m_tiles * p.n_tiles * k_split, st)));
-      {  // fixed-order sum of the partials (+ scatter of compacted rows) -> dHidden
+      if (pn) {  // ... -> dx, dgamma (RMSNorm backward fused behind the reduction; dHidden is never written)
+        if (tile_list) return fail(GRPO_ERR_INVALID_ARG, "the pre-norm backward is not available for the stash variant");
+        GRPO_TRY(launch_prenorm_bwd(ctx, false, dh_part, k_split, L.chunk_rows * c.d / 4, static_cast<int>(rows), dyn_rows,
+                                    compact ? row_idx + t0 : nullptr, t0, *pn, dhidden_out, st));
+      } else {  // fixed-order sum of the partials (+ scatter of compacted rows) -> dHidden
         LaunchScope ls(ctx, GRPO_KERNEL_DH_REDUCE, st);
         splitk_reduce_kernel<<<static_cast<unsigned>(rows), 128, 0, st>>>(
             reinterpret_cast<const float4*>(dh_part), k_split, L.chunk_rows * c.d / 4, c.d / 4, static_cast<int>(rows),
@@ -860,6 +895,53 @@ extern "C" int32_t grpo_fused_logprob_loss_bwd(grpo_ctx* ctx, const void* hidden
   if (T <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0");
   return bwd_impl(ctx, 0, hidden, W, targets, lse, coeff, T, grad_scale, dhidden_out, dW_accum,
                   static_cast<cudaStream_t>(stream));
+}
+
+// ------------------------------------------------------------------------------------- NEXT-4: final RMSNorm
+extern "C" int32_t grpo_rmsnorm_fwd(grpo_ctx* ctx, const void* x, const void* gamma, float eps_rms, int64_t T,
+                                    void* hidden_out, float* rstd_out, void* stream) {
+  if (!ctx || !x || !gamma || !hidden_out || !rstd_out) return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0");
+  if (!(eps_rms >= 0.f)) return fail(GRPO_ERR_INVALID_ARG, "eps_rms must be >= 0");
+  if ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(gamma) | reinterpret_cast<uintptr_t>(hidden_out)) & 7)
+    return fail(GRPO_ERR_SHAPE, "x / gamma / hidden_out must be 8-byte aligned");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int warps_per_block = 8;
+  const int64_t blocks = std::min<int64_t>((T + warps_per_block - 1) / warps_per_block, 32LL * ctx->num_sms);
+  {
+    LaunchScope ls(ctx, GRPO_KERNEL_RMSNORM, st);
+    rmsnorm_fwd_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(
+        static_cast<const uint2*>(x), static_cast<const uint2*>(gamma), T, ctx->cfg.d / 4, 1.f / ctx->cfg.d, eps_rms,
+        static_cast<uint2*>(hidden_out), rstd_out);
+  }
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_rmsnorm_bwd(grpo_ctx* ctx, const void* x, const void* gamma, const float* rstd,
+                                    const void* dhidden, int32_t dhidden_is_fp32, int64_t T, void* dx_out,
+                                    float* dgamma_accum, void* stream) {
+  if (!ctx || !x || !gamma || !rstd || !dhidden || !dx_out || !dgamma_accum)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0 || T > INT32_MAX - 256) return fail(GRPO_ERR_SHAPE, "need 0 < T < 2^31");
+  const PrenormArgs pn{x, gamma, rstd, dgamma_accum};
+  GRPO_TRY(launch_prenorm_bwd(ctx, dhidden_is_fp32 == 0, dhidden, 1, 0, static_cast<int>(T), nullptr, nullptr, 0, pn,
+                              dx_out, static_cast<cudaStream_t>(stream)));
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_fused_logprob_loss_bwd_prenorm(grpo_ctx* ctx, const void* x, const void* gamma,
+                                                       const float* rstd, const void* hidden, const void* W,
+                                                       const int32_t* targets, const float* lse, const float* coeff,
+                                                       int64_t T, float grad_scale, void* dx_out, float* dgamma_accum,
+                                                       float* dW_accum, void* stream) {
+  if (!ctx || !x || !gamma || !rstd || !hidden || !W || !targets || !lse || !coeff || !dx_out || !dgamma_accum)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0");
+  const PrenormArgs pn{x, gamma, rstd, dgamma_accum};
+  return bwd_impl(ctx, 0, hidden, W, targets, lse, coeff, T, grad_scale, dx_out, dW_accum,
+                  static_cast<cudaStream_t>(stream), nullptr, nullptr, &pn);
 }
 
 extern "C" int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hidden, const void* W,
@@ -1261,6 +1343,32 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   if (logp_host) CU_OK(cudaMemcpyAsync(logp_host, logp, T * 4, cudaMemcpyDeviceToHost, st));
   CU_OK(cudaStreamSynchronize(pipe.cs));
   CU_OK(cudaStreamSynchronize(st));
+  return GRPO_OK;
+}
+
+// ------------------------------------------------------------------------------------- diagnostics
+extern "C" int32_t grpo_debug_max_active_clusters(grpo_ctx* ctx, int32_t cluster_size, int32_t* clusters_out) {
+  if (!ctx || !clusters_out || cluster_size < 1 || cluster_size > 16 || (cluster_size & 1 && cluster_size != 1))
+    return fail(GRPO_ERR_INVALID_ARG, "need ctx, clusters_out and cluster_size in {1, 2, 4, ..., 16}");
+  auto kern = grpo_gemm_kernel<2, false, false, EPI_LSE>;
+  constexpr int smem = GemmShape<2>::kSmemBytes;
+  CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  if (cluster_size > 8) CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  cudaLaunchConfig_t lc;
+  std::memset(&lc, 0, sizeof(lc));
+  lc.gridDim = dim3(static_cast<unsigned>(ctx->num_sms / cluster_size * cluster_size * 4));
+  lc.blockDim = dim3(kGemmThreads);
+  lc.dynamicSmemBytes = smem;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = static_cast<unsigned>(cluster_size);
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
+  int n = 0;
+  CU_OK(cudaOccupancyMaxActiveClusters(&n, kern, &lc));
+  *clusters_out = n;
   return GRPO_OK;
 }
 

@@ -348,6 +348,132 @@ __global__ void __launch_bounds__(128) zero_coeff_rows_kernel(const float* __res
   for (int64_t i = threadIdx.x; i < row_bytes / 16; i += blockDim.x) dst[i] = make_uint4(0u, 0u, 0u, 0u);
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-4 (R29-R31): the final RMSNorm in front of the path.
+__device__ __forceinline__ float4 bf16x4_to_float4(uint2 v) {
+  float4 f;
+  f.x = __uint_as_float(v.x << 16);
+  f.y = __uint_as_float(v.x & 0xffff0000u);
+  f.z = __uint_as_float(v.y << 16);
+  f.w = __uint_as_float(v.y & 0xffff0000u);
+  return f;
+}
+
+// H[t,:] = bf16(gamma * x[t,:] * rstd_t),  rstd_t = 1 / sqrt(mean_k x_tk^2 + eps)   (fp32 arithmetic, one rounding).
+// One warp per row, 8-byte loads (4 bf16); the second pass re-reads the row from L1.  HBM-bound: 2 d bytes read +
+// 2 d bytes written per token.
+__global__ void __launch_bounds__(256) rmsnorm_fwd_kernel(const uint2* __restrict__ x, const uint2* __restrict__ gamma,
+                                                          int64_t T, int row_vec /* d / 4 */, float inv_d, float eps,
+                                                          uint2* __restrict__ H, float* __restrict__ rstd_out) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warps = static_cast<int64_t>(gridDim.x) * (blockDim.x >> 5);
+  for (int64_t t = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5); t < T; t += warps) {
+    const uint2* row = x + t * row_vec;
+    float ss = 0.f;
+    for (int i = lane; i < row_vec; i += 32) {
+      const float4 v = bf16x4_to_float4(row[i]);
+      ss = fmaf(v.x, v.x, fmaf(v.y, v.y, fmaf(v.z, v.z, fmaf(v.w, v.w, ss))));
+    }
+    ss = warp_sum(ss);
+    const float rstd = 1.f / sqrtf(ss * inv_d + eps);
+    if (lane == 0) rstd_out[t] = rstd;
+    uint2* dst = H + t * row_vec;
+    for (int i = lane; i < row_vec; i += 32) {
+      const float4 v = bf16x4_to_float4(row[i]);
+      const float4 g = bf16x4_to_float4(gamma[i]);
+      dst[i] = make_uint2(pack_bf16x2(g.x * (v.x * rstd), g.y * (v.y * rstd)),
+                          pack_bf16x2(g.z * (v.z * rstd), g.w * (v.w * rstd)));
+    }
+  }
+}
+
+// RMSNorm backward, fused behind A5: the split-K reduction of the dHidden row (fixed order, fp32) is followed in
+// registers by   g = gamma * dH,  xh = x rstd,  dx = rstd (g - xh mean_k(g xh)),  dgamma += dH * xh,
+// so dHidden is never written: the row goes straight to dx (scattered to its packed position under compaction).
+// IN_BF16: `parts` is a bf16 [rows, d] dHidden instead (the standalone grpo_rmsnorm_bwd; k_split = 1).
+// Blocks loop over rows and keep their dgamma partial sums in registers (J float4 per thread: d <= 1024 J), then
+// add them to dgamma_accum with one atomic per column and block.
+template <int J, bool IN_BF16>
+__global__ void __launch_bounds__(256) prenorm_bwd_kernel(const void* __restrict__ parts, int k_split,
+                                                          int64_t split_stride_vec, int row_vec /* d / 4 */,
+                                                          int rows_static, const int* __restrict__ dyn_rows,
+                                                          const int* __restrict__ row_idx, int64_t row0,
+                                                          const uint2* __restrict__ x, const uint2* __restrict__ gamma,
+                                                          const float* __restrict__ rstd, float inv_d,
+                                                          void* __restrict__ dx_out, int out_fp32,
+                                                          float* __restrict__ dgamma_accum) {
+  __shared__ float red[8];
+  const int rows = dyn_rows ? min(rows_static, *dyn_rows) : rows_static;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float4 acc[J], gm[J];
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    acc[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+    const int i = threadIdx.x + j * 256;
+    gm[j] = i < row_vec ? bf16x4_to_float4(gamma[i]) : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  for (int r = blockIdx.x; r < rows; r += gridDim.x) {
+    const int64_t t = row_idx ? row_idx[r] : row0 + r;           // packed row of the call
+    const float rs = rstd[t];
+    float4 dh[J], xh[J];
+    float dot = 0.f;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int i = threadIdx.x + j * 256;
+      dh[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+      xh[j] = dh[j];
+      if (i < row_vec) {
+        if constexpr (IN_BF16) {
+          dh[j] = bf16x4_to_float4(reinterpret_cast<const uint2*>(parts)[static_cast<int64_t>(r) * row_vec + i]);
+        } else {
+          const float4* src = reinterpret_cast<const float4*>(parts) + static_cast<int64_t>(r) * row_vec + i;
+          dh[j] = src[0];
+          for (int k = 1; k < k_split; ++k) {
+            const float4 b = src[k * split_stride_vec];
+            dh[j].x += b.x; dh[j].y += b.y; dh[j].z += b.z; dh[j].w += b.w;
+          }
+        }
+        const float4 xv = bf16x4_to_float4(x[t * row_vec + i]);
+        xh[j] = make_float4(xv.x * rs, xv.y * rs, xv.z * rs, xv.w * rs);
+        dot += gm[j].x * dh[j].x * xh[j].x + gm[j].y * dh[j].y * xh[j].y + gm[j].z * dh[j].z * xh[j].z +
+               gm[j].w * dh[j].w * xh[j].w;
+      }
+    }
+    dot = warp_sum(dot);
+    __syncthreads();                                             // red[] of the previous row has been read
+    if (lane == 0) red[warp] = dot;
+    __syncthreads();
+    float mean = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) mean += red[w];
+    mean *= inv_d;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int i = threadIdx.x + j * 256;
+      if (i < row_vec) {
+        const float4 o = make_float4(rs * (gm[j].x * dh[j].x - xh[j].x * mean), rs * (gm[j].y * dh[j].y - xh[j].y * mean),
+                                     rs * (gm[j].z * dh[j].z - xh[j].z * mean), rs * (gm[j].w * dh[j].w - xh[j].w * mean));
+        if (out_fp32) reinterpret_cast<float4*>(dx_out)[t * row_vec + i] = o;
+        else reinterpret_cast<uint2*>(dx_out)[t * row_vec + i] = make_uint2(pack_bf16x2(o.x, o.y), pack_bf16x2(o.z, o.w));
+        acc[j].x = fmaf(dh[j].x, xh[j].x, acc[j].x);
+        acc[j].y = fmaf(dh[j].y, xh[j].y, acc[j].y);
+        acc[j].z = fmaf(dh[j].z, xh[j].z, acc[j].z);
+        acc[j].w = fmaf(dh[j].w, xh[j].w, acc[j].w);
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    const int i = threadIdx.x + j * 256;
+    if (i < row_vec && static_cast<int>(blockIdx.x) < rows) {
+      atomicAdd(dgamma_accum + 4 * i + 0, acc[j].x);
+      atomicAdd(dgamma_accum + 4 * i + 1, acc[j].y);
+      atomicAdd(dgamma_accum + 4 * i + 2, acc[j].z);
+      atomicAdd(dgamma_accum + 4 * i + 3, acc[j].w);
+    }
+  }
+}
+
 // 3-contraction variant: turn the stashed exponentials e = 2^(z2 - m) (fp16, written by the
 // EPI_LSE_STASH epilogue together with m per (row, 256-column tile) in `shift`) into
 // dZ = k_t (1[v = y_t] - e 2^(m - lse2_t)) (bf16) in place; k_t = coeff_t * coeff_mul.  HBM-bound: 2 B read + 2 B

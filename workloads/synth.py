@@ -51,6 +51,9 @@ class GrpoBatch:
     loss_agg: int = 0
     arrival_order: Optional[np.ndarray] = None   # cfg 5: order groups are enqueued in
     zero_var_frac: float = 0.0
+    x_prenorm: Optional[torch.Tensor] = None     # bf16 [T, d]: pre-norm activations (prenorm=True only)
+    gamma: Optional[torch.Tensor] = None         # bf16 [d]: RMSNorm weight (prenorm=True only)
+    eps_rms: float = 1e-6
 
     @property
     def T(self) -> int:
@@ -77,7 +80,8 @@ class GrpoBatch:
                     y=self.targets.cpu().numpy().astype(np.int64),
                     cu_seqlens=self.cu_seqlens.cpu().numpy().astype(np.int64),
                     rewards=f(self.rewards), old_logp=f(self.old_logp), ref_logp=f(self.ref_logp),
-                    mask=None if self.mask is None else self.mask.cpu().numpy())
+                    mask=None if self.mask is None else self.mask.cpu().numpy(),
+                    x=f(self.x_prenorm), gamma=f(self.gamma))
 
 
 # ------------------------------------------------------------------ small draws (numpy)
@@ -149,11 +153,16 @@ def make_config(cfg: int, seed: int = 0, device="cpu", *, d: int | None = None, 
                 n_groups: int | None = None, G: int | None = None, len_div: float = 1.0,
                 old_sigma: float | None = None, kl_beta: float | None = None,
                 mask_frac: float = 0.0, loss_agg: int = 0, variant: str = "", w_std: float = 0.02,
-                bad_target_frac: float = 0.0) -> GrpoBatch:
+                bad_target_frac: float = 0.0, prenorm: bool = False) -> GrpoBatch:
     """Build config ``cfg`` (1-5).  Keyword overrides shrink it for CPU-sized parity cases.
 
     variant "1b": config 1 with old-logprob noise sigma = 0.3 so both clip regions are
     populated (the BASELINE configs never exercise the clip).
+
+    prenorm=True (NEXT-4): the batch also carries pre-norm activations ``x_prenorm`` (rows N(0,1) times a
+    per-row lognormal scale, bf16) and a norm weight ``gamma`` (1 + 0.1 N(0,1), bf16); ``hidden`` is then the
+    stock-torch fp32 ``rms_norm(x, gamma)`` rounded to bf16 - input synthesis, so that old / ref log-probs are
+    those of the normalised states; neither the oracle nor the kernels read ``hidden`` in the pre-norm tests.
     """
     ng0, G0, d0, V0 = _SHAPES[cfg]
     n_groups = n_groups or ng0
@@ -172,7 +181,12 @@ def make_config(cfg: int, seed: int = 0, device="cpu", *, d: int | None = None, 
     gen.manual_seed(base_seed)
     W = (torch.randn(V, d, generator=gen, device=dev, dtype=torch.float32) * w_std).to(torch.bfloat16)
     Hf = torch.randn(T, d, generator=gen, device=dev, dtype=torch.float32)
-    if cfg != 1:   # "after RMSNorm-like scaling": unit-RMS rows (R16)
+    x_pre = gamma = None
+    if prenorm:
+        x_pre = (Hf * torch.exp(0.5 * torch.randn(T, 1, generator=gen, device=dev))).to(torch.bfloat16)
+        gamma = (1.0 + 0.1 * torch.randn(d, generator=gen, device=dev)).to(torch.bfloat16)
+        Hf = torch.nn.functional.rms_norm(x_pre.float(), (d,), gamma.float(), 1e-6)
+    elif cfg != 1:   # "after RMSNorm-like scaling": unit-RMS rows (R16)
         Hf = Hf * torch.rsqrt(Hf.pow(2).mean(dim=1, keepdim=True) + 1e-12)
     H = Hf.to(torch.bfloat16)
     del Hf
@@ -195,7 +209,8 @@ def make_config(cfg: int, seed: int = 0, device="cpu", *, d: int | None = None, 
         name=f"cfg{cfg}{variant}", n_groups=n_groups, G=G, d=d, V=V, seqlens=seqlens,
         cu_seqlens=torch.from_numpy(cu).to(dev), rewards=torch.from_numpy(rewards).to(dev),
         hidden=H, W=W, targets=y, old_logp=old.float(), ref_logp=None if ref is None else ref.float(),
-        mask=mask, kl_beta=beta, loss_agg=loss_agg, arrival_order=arrival, zero_var_frac=zero_var_frac)
+        mask=mask, kl_beta=beta, loss_agg=loss_agg, arrival_order=arrival, zero_var_frac=zero_var_frac,
+        x_prenorm=x_pre, gamma=gamma)
 
 
 def slice_groups(b: GrpoBatch, groups) -> GrpoBatch:
