@@ -454,10 +454,14 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             tmem_ld32(t_addr + c * 32, v);
             tmem_ld_wait();
             const int nvalid = p.n_total - cbase;
+            if (nvalid < 32) {
 #pragma unroll
-            for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, i < nvalid ? v[i] * p.scale_log2e : -INFINITY);
+              for (int i = 0; i < 32; ++i) v[i] = i < nvalid ? v[i] : -INFINITY;
+            }
+#pragma unroll
+            for (int i = 0; i < 32; i += 2) tmax = max3(tmax, v[i], v[i + 1]);
           }
-          const float new_m = fmaxf(run_m, tmax);
+          const float new_m = fmaxf(run_m, tmax * p.scale_log2e);   // scale_log2e > 0: the max commutes with the scale
           const float rescale = ex2_approx(run_m - new_m);
           run_s *= rescale;
           run_u *= rescale;
@@ -474,29 +478,42 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           const int nvalid = p.n_total - cbase;                   // >= 1; columns >= nvalid are padding
 
           if constexpr (is_lse(EPI)) {
-            float cmax = -INFINITY;
-            if (nvalid >= 32) {
+            // z2 = v s log2(e) is never formed on its own: the running maximum is taken over the raw accumulator
+            // (the scale is positive) and every exponent is ONE fused multiply-add, 2^(v s log2e - m), issued two
+            // logits per instruction (FFMA2 / FADD2 / FMNMX3).  Padding columns hold -inf: 2^-inf = 0.
+            if (nvalid < 32) {
 #pragma unroll
-              for (int i = 0; i < 32; ++i) { v[i] *= p.scale_log2e; cmax = fmaxf(cmax, v[i]); }
-            } else {
-#pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                v[i] = i < nvalid ? v[i] * p.scale_log2e : -INFINITY;
-                cmax = fmaxf(cmax, v[i]);
-              }
+              for (int i = 0; i < 32; ++i) v[i] = i < nvalid ? v[i] : -INFINITY;
             }
-            const float new_m = EPI == EPI_LSE_STASH ? run_m : fmaxf(run_m, cmax);   // stash: tile max already in
-            float s = 0.f;
-            const float rescale = ex2_approx(run_m - new_m);
-            if constexpr (EPI == EPI_LSE_STASH) {
-              float e[32], uc = 0.f;
+            float new_m = run_m;                                   // stash: the tile max is already in run_m
+            if constexpr (EPI != EPI_LSE_STASH) {
+              float cmax = v[0];
 #pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                e[i] = ex2_approx(v[i] - new_m);                   // padding columns: 2^-inf = 0
-                s += e[i];
-                if (p.part_u != nullptr) uc = fmaf(e[i], i < nvalid ? v[i] : 0.f, uc);
-              }
-              run_u += uc;
+              for (int i = 1; i < 31; i += 2) cmax = max3(cmax, v[i], v[i + 1]);
+              new_m = fmaxf(run_m, fmaxf(cmax, v[31]) * p.scale_log2e);
+            }
+            const float rescale = ex2_approx(run_m - new_m);
+            const f32x2 sc2 = pack2(p.scale_log2e, p.scale_log2e), nm2 = pack2(-new_m, -new_m);
+            float e[32];
+            f32x2 acc = pack2(0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < 32; i += 2) {
+              float t0, t1;
+              unpack2(fma2(pack2(v[i], v[i + 1]), sc2, nm2), t0, t1);
+              e[i] = ex2_approx(t0);
+              e[i + 1] = ex2_approx(t1);
+              acc = add2(acc, pack2(e[i], e[i + 1]));
+            }
+            float s0, s1;
+            unpack2(acc, s0, s1);
+            const float s = s0 + s1;
+            if (p.part_u != nullptr) {   // entropy = lse - sum_v p_v z_v: one more running sum, rescaled like run_s
+              float uc = 0.f;
+#pragma unroll
+              for (int i = 0; i < 32; ++i) uc = fmaf(e[i], i < nvalid ? v[i] * p.scale_log2e : 0.f, uc);   // 0 * -inf is NaN
+              run_u = (EPI == EPI_LSE_STASH ? run_u : run_u * rescale) + uc;
+            }
+            if constexpr (EPI == EPI_LSE_STASH) {
               if (row_ok) {
                 __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
 #pragma unroll
@@ -504,32 +521,25 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                   st_global_v4(dst + g * 8, pack_f16x2(e[g * 8 + 0], e[g * 8 + 1]), pack_f16x2(e[g * 8 + 2], e[g * 8 + 3]),
                                pack_f16x2(e[g * 8 + 4], e[g * 8 + 5]), pack_f16x2(e[g * 8 + 6], e[g * 8 + 7]));
               }
-            } else if (p.part_u == nullptr) {
-#pragma unroll
-              for (int i = 0; i < 32; ++i) s += ex2_approx(v[i] - new_m);
-            } else {   // entropy = lse - sum_v p_v z_v: one more running sum, rescaled like the sum of exponentials
-              float uc = 0.f;
-#pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                const float e = ex2_approx(v[i] - new_m);
-                s += e;
-                uc = fmaf(e, i < nvalid ? v[i] : 0.f, uc);        // padding columns hold -inf: 0 * -inf is NaN
-              }
-              run_u = run_u * rescale + uc;
             }
             run_s = run_s * rescale + s;
             run_m = new_m;
             if (static_cast<uint32_t>(y - cbase) < 32u) {          // rare: target column in this chunk
-              float zy2 = 0.f;
+              float zy = 0.f;
 #pragma unroll
-              for (int i = 0; i < 32; ++i) zy2 = (y - cbase == i) ? v[i] : zy2;
-              p.zy[row_g] = zy2 * kLn2;                            // back to natural units: s * z
+              for (int i = 0; i < 32; ++i) zy = (y - cbase == i) ? v[i] : zy;
+              p.zy[row_g] = zy * p.logit_scale;                    // natural units: s * z
             }
           } else if constexpr (EPI == EPI_DZ) {
             // dz = k (1[v = y] - p),  p = 2^(z s log2e - lse log2e)
             float dzv[32];
+            const f32x2 sc2 = pack2(p.scale_log2e, p.scale_log2e), nl2 = pack2(-lse2, -lse2), nk2 = pack2(-kcoef, -kcoef);
 #pragma unroll
-            for (int i = 0; i < 32; ++i) dzv[i] = -kcoef * ex2_approx(fmaf(v[i], p.scale_log2e, -lse2));
+            for (int i = 0; i < 32; i += 2) {
+              float t0, t1;
+              unpack2(fma2(pack2(v[i], v[i + 1]), sc2, nl2), t0, t1);
+              unpack2(mul2(pack2(ex2_approx(t0), ex2_approx(t1)), nk2), dzv[i], dzv[i + 1]);
+            }
             if (static_cast<uint32_t>(y - cbase) < 32u) {
 #pragma unroll
               for (int i = 0; i < 32; ++i) dzv[i] = (y - cbase == i) ? dzv[i] + kcoef : dzv[i];

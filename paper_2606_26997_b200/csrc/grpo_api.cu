@@ -345,6 +345,8 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
     return fail(GRPO_ERR_INVALID_ARG, "gemm_cta_group must be 0 (default), 1 or 2");
   if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
     return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
+  if (!(cfg->logit_scale > 0.f))
+    return fail(GRPO_ERR_INVALID_ARG, "logit_scale (1 / temperature) must be > 0 (got %g)", (double)cfg->logit_scale);
   if (cfg->kl_type < 0 || cfg->kl_type > 2 || (cfg->dual_clip != 0.f && !(cfg->dual_clip > 1.f)))
     return fail(GRPO_ERR_INVALID_ARG, "kl_type must be 0, 1 or 2 and dual_clip 0 or > 1");
   int dev = 0;
@@ -1294,35 +1296,51 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   float* coeff = slot_ptr<float>(ctx, 0, L.off_coeff);
   uint8_t* dh = slot_ptr<uint8_t>(ctx, 0, L.off_dh);
   float* loss_dev = slot_ptr<float>(ctx, 0, L.off_total) + 8;   // scratch scalar inside the 256-byte cell
-  // copy pipeline: hidden states arrive chunk by chunk on the copy stream while the compute stream works
+  // copy pipeline: the hidden states arrive in pieces on the copy stream while the compute stream works.  Pieces:
+  // a short first one (so that A2 starts after ~0.15 ms of transfer instead of a whole chunk's 0.7 ms: with the
+  // V-only vocab split a launch of a few token tiles still fills the SMs), the rest of backward chunk 0, then one
+  // piece per backward chunk.  piece_of_chunk[i] = the last piece backward chunk i needs.
   const int64_t rpc = rows_per_chunk_for(ctx, T);
   const size_t n_chunks = static_cast<size_t>((T + rpc - 1) / rpc);
+  const int64_t first_rows = std::min<int64_t>(2048, std::min<int64_t>(rpc, T));
+  std::vector<std::pair<int64_t, int64_t>> pieces;             // [begin, end) packed rows
+  std::vector<size_t> piece_of_chunk(n_chunks);
+  pieces.emplace_back(0, first_rows);
+  if (first_rows < std::min<int64_t>(rpc, T)) pieces.emplace_back(first_rows, std::min<int64_t>(rpc, T));
+  piece_of_chunk[0] = pieces.size() - 1;
+  for (size_t i = 1; i < n_chunks; ++i) {
+    pieces.emplace_back(static_cast<int64_t>(i) * rpc, std::min<int64_t>(T, static_cast<int64_t>(i + 1) * rpc));
+    piece_of_chunk[i] = pieces.size() - 1;
+  }
   HostPipe pipe;
   pipe.cs = ctx->copy_stream;
   pipe.dh_host = static_cast<uint8_t*>(dhidden_host);
-  // events live in the context and are created once (1 fence + n_chunks in + n_chunks out)
-  while (ctx->pipe_events.size() < 1 + 2 * n_chunks) {
+  // events live in the context and are created once (1 fence + one per piece + one per chunk of dHidden)
+  while (ctx->pipe_events.size() < 1 + pieces.size() + n_chunks) {
     cudaEvent_t e = nullptr;
     CU_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     ctx->pipe_events.push_back(e);
   }
   const cudaEvent_t fence = ctx->pipe_events[0];
-  pipe.in.assign(ctx->pipe_events.begin() + 1, ctx->pipe_events.begin() + 1 + n_chunks);
-  if (dhidden_host) pipe.out.assign(ctx->pipe_events.begin() + 1 + n_chunks, ctx->pipe_events.begin() + 1 + 2 * n_chunks);
-  CU_OK(cudaEventRecord(fence, st));                         // staging buffers are free once st reaches here
-  CU_OK(cudaStreamWaitEvent(pipe.cs, fence, 0));
-  for (size_t i = 0; i < n_chunks; ++i) {
-    const int64_t t0 = static_cast<int64_t>(i) * rpc, rows = std::min<int64_t>(rpc, T - t0);
-    CU_OK(cudaMemcpyAsync(sh + t0 * c.d * 2, static_cast<const uint8_t*>(hidden_host) + t0 * c.d * 2, rows * c.d * 2,
-                          cudaMemcpyHostToDevice, pipe.cs));
-    CU_OK(cudaEventRecord(pipe.in[i], pipe.cs));
-  }
+  const cudaEvent_t* piece_ev = ctx->pipe_events.data() + 1;
+  for (size_t i = 0; i < n_chunks; ++i) pipe.in.push_back(piece_ev[piece_of_chunk[i]]);
+  if (dhidden_host)
+    pipe.out.assign(ctx->pipe_events.begin() + 1 + pieces.size(), ctx->pipe_events.begin() + 1 + pieces.size() + n_chunks);
+  // the small per-token arrays go first: they must not queue behind the hidden states on the copy engine
   CU_OK(cudaMemcpyAsync(stg, targets_host, T * 4, cudaMemcpyHostToDevice, st));
   CU_OK(cudaMemcpyAsync(so, old_logp_host, T * 4, cudaMemcpyHostToDevice, st));
   if (ref_logp_host) CU_OK(cudaMemcpyAsync(sr, ref_logp_host, T * 4, cudaMemcpyHostToDevice, st));
   if (mask_host) CU_OK(cudaMemcpyAsync(sm, mask_host, T, cudaMemcpyHostToDevice, st));
   CU_OK(cudaMemcpyAsync(d_cu, cu_seqlens_host, (S + 1) * 4, cudaMemcpyHostToDevice, st));
   CU_OK(cudaMemcpyAsync(d_rw, rewards_host, S * 4, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaEventRecord(fence, st));                         // staging buffers are free once st reaches here
+  CU_OK(cudaStreamWaitEvent(pipe.cs, fence, 0));
+  for (size_t i = 0; i < pieces.size(); ++i) {
+    const int64_t t0 = pieces[i].first, rows = pieces[i].second - pieces[i].first;
+    CU_OK(cudaMemcpyAsync(sh + t0 * c.d * 2, static_cast<const uint8_t*>(hidden_host) + t0 * c.d * 2, rows * c.d * 2,
+                          cudaMemcpyHostToDevice, pipe.cs));
+    CU_OK(cudaEventRecord(piece_ev[i], pipe.cs));
+  }
   CU_OK(cudaMemsetAsync(loss_dev, 0, 4, st));
   GRPO_TRY(grpo_group_advantage(ctx, d_rw, nullptr, n_groups, G, d_adv, nullptr, st));
   GRPO_TRY(fwd_check(ctx, S, T));
@@ -1332,10 +1350,9 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   if (c.stash_logits) {
     GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, &a, &pipe));
   } else {
-    for (size_t i = 0; i < n_chunks; ++i) {                  // A2 + A3 chunk by chunk, as the rows arrive
-      const int64_t t0 = static_cast<int64_t>(i) * rpc, rows = std::min<int64_t>(rpc, T - t0);
-      CU_OK(cudaStreamWaitEvent(st, pipe.in[i], 0));
-      GRPO_TRY(fwd_rows(ctx, 0, sh, W, stg, a, T, t0, rows, nullptr, st));
+    for (size_t i = 0; i < pieces.size(); ++i) {             // A2 + A3 piece by piece, as the rows arrive
+      CU_OK(cudaStreamWaitEvent(st, piece_ev[i], 0));
+      GRPO_TRY(fwd_rows(ctx, 0, sh, W, stg, a, T, pieces[i].first, pieces[i].second - pieces[i].first, nullptr, st));
     }
     GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, nullptr, &pipe));
   }
