@@ -1,0 +1,113 @@
+"""Data parallelism over complete groups.
+
+Complete groups are independent units of work, and the paper's trainer ran DP = 2.
+A logical update of U groups is dealt to the ranks by arrival position (group k of the update ->
+rank k mod world); every rank runs A1-A6 on its groups through ``grpo_enqueue_groups`` with the denominator of the
+WHOLE update (R10), accumulating into its local fp32 ``dW`` / loss; at the update boundary ONE sum
+all-reduce of ``dW`` (1.245 GB at the Qwen3-1.7B head) plus the scalars gives every rank the full-update gradient:
+by the additivity of the step over groups (P12) the result equals the single-rank full-batch step up to fp32
+summation order.
+
+The all-reduce is issued on a side stream behind an event of the compute stream and returns immediately, so it
+overlaps with the next update's contractions, which accumulate into the OTHER of two gradient buffers
+(``buffers()`` hands them out alternately).  ``torch.distributed`` is plumbing only (NCCL over NVLink 5 on the GPU
+box; gloo in the CPU tests): no arithmetic of the method lives here.  Nothing in this module was timed on more than
+one GPU (none is reachable from this build); DESIGN.md section 7 says so.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import List, Optional, Sequence
+
+import torch
+import torch.distributed as dist
+
+
+def assign_groups(n_groups_in_update: int, world: int, rank: int) -> List[int]:
+    """Positions (within the update, in FIFO order) of the groups rank `rank` trains: k with k mod world == rank."""
+    return [k for k in range(n_groups_in_update) if k % world == rank]
+
+
+@dataclass
+class BoundaryHandle:
+    """Outstanding reduction of one logical update's accumulators."""
+    works: list = field(default_factory=list)
+    done_event: Optional["torch.cuda.Event"] = None
+
+    def wait(self, stream: Optional["torch.cuda.Stream"] = None):
+        """Make `stream` (default: the current stream) wait for the reduced gradients; on CPU, block."""
+        for w in self.works:
+            w.wait()
+        if self.done_event is not None:
+            (stream or torch.cuda.current_stream()).wait_event(self.done_event)
+
+
+class GrpoDataParallel:
+    def __init__(self, process_group=None, comm_stream: Optional["torch.cuda.Stream"] = None):
+        self.pg = process_group
+        self.world = dist.get_world_size(process_group) if dist.is_initialized() else 1
+        self.rank = dist.get_rank(process_group) if dist.is_initialized() else 0
+        self._comm_stream = comm_stream
+        self._buf = None
+        self._turn = 0
+
+    # ------------------------------------------------------------------ work split
+    def local_positions(self, n_groups_in_update: int) -> List[int]:
+        return assign_groups(n_groups_in_update, self.world, self.rank)
+
+    def global_denominator(self, local_loss_tokens: int) -> float:
+        """Loss-bearing tokens of the WHOLE update (token-mean denominator, R10): sum over ranks of the
+        local counts (host integers: the sequence lengths are host data in the CGP handoff)."""
+        if self.world == 1:
+            return float(local_loss_tokens)
+        t = torch.tensor([float(local_loss_tokens)], dtype=torch.float64)
+        if dist.get_backend(self.pg) == "nccl":
+            t = t.cuda()
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.pg)
+        return float(t.item())
+
+    def global_sequences(self, local_sequences: int) -> int:
+        """Sequences of the whole update (loss_agg = 1 divides by it; ``GrpoContext.grpo_set_seq_denom``)."""
+        return int(round(self.global_denominator(local_sequences)))
+
+    # ------------------------------------------------------------------ double-buffered accumulators
+    def buffers(self, V: int, d: int, device="cuda"):
+        """(dW, loss, metrics) of the update about to be trained; alternates between two sets so that the previous
+        update's all-reduce can still be in flight.  The caller zeroes a set after consuming it."""
+        if self._buf is None:
+            mk = lambda: (torch.zeros(V, d, dtype=torch.float32, device=device),
+                          torch.zeros(1, dtype=torch.float32, device=device),
+                          torch.zeros(4, dtype=torch.float32, device=device))
+            self._buf = (mk(), mk())
+        out = self._buf[self._turn]
+        self._turn ^= 1
+        return out
+
+    # ------------------------------------------------------------------ the collective
+    def reduce_boundary(self, dW_accum: torch.Tensor, loss_accum: torch.Tensor,
+                        metrics_accum: Optional[torch.Tensor] = None,
+                        compute_stream: Optional["torch.cuda.Stream"] = None) -> BoundaryHandle:
+        """Sum `dW_accum`, `loss_accum` (and `metrics_accum`) over the ranks, in place, asynchronously.
+
+        CUDA tensors: the collectives are enqueued on the side stream behind an event recorded on `compute_stream`
+        (default: current), so everything the update's launches enqueued is reduced, and the call returns at once:
+        the next update's kernels run concurrently.  CPU tensors (gloo tests): asynchronous works."""
+        tensors = [t for t in (dW_accum, loss_accum, metrics_accum) if t is not None]
+        h = BoundaryHandle()
+        if self.world == 1:
+            return h
+        if dW_accum.is_cuda:
+            if self._comm_stream is None:
+                self._comm_stream = torch.cuda.Stream()
+            ev = torch.cuda.Event()
+            ev.record(compute_stream or torch.cuda.current_stream())
+            with torch.cuda.stream(self._comm_stream):
+                self._comm_stream.wait_event(ev)
+                for t in tensors:
+                    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.pg)
+                h.done_event = torch.cuda.Event()
+                h.done_event.record(self._comm_stream)
+        else:
+            for t in tensors:
+                h.works.append(dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.pg, async_op=True))
+        return h
