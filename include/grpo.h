@@ -132,6 +132,28 @@ int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const voi
  * use it: it counts the sequences of the update's groups itself (R10). */
 int32_t grpo_set_seq_denom(grpo_ctx* ctx, int32_t n_sequences);
 
+/* ---- NEXT-3(b): vocab-parallel (tensor-parallel) forward -------------------------
+ * The paper's trainer ran TP = 4, which shards W by rows.  Rank r holds W_shard = W[v0_r : v1_r, :]
+ * and a context created with V = v1_r - v0_r.
+ *
+ * grpo_vocab_shard_partials: A2 on the shard.  targets_local[t] = y_t - v0_r (any value outside [0, V_shard) means
+ * the target column lives in another shard).  Outputs, fp32 [T]: m2_out / s2_out = running maximum and sum of
+ * 2^(z2 - m2) over the shard's columns in the log2 domain (z2 = s z log2 e), zy_out = s z_t[y_t] where this shard
+ * holds the target column, else 0.  The three arrays are what the ranks exchange (one all-gather of [T] x 3 fp32).
+ *
+ * grpo_loss_from_partials: A3 on the gathered partials [n_shards, T] (shard-major): combines them in shard order into
+ * lse / logp and runs the loss arithmetic of grpo_fused_logprob_loss_fwd (same arguments; targets are GLOBAL ids,
+ * V_global the full vocabulary).  Every rank then calls grpo_fused_logprob_loss_bwd on its shard with targets_local,
+ * the global lse and coeff: dW_accum is the shard's rows of dW, and dhidden_out the shard's PARTIAL dHidden, which
+ * the ranks sum (all-reduce of [T, d]).  DESIGN.md section 7. */
+int32_t grpo_vocab_shard_partials(grpo_ctx* ctx, const void* hidden, const void* W_shard, const int32_t* targets_local,
+                                  int64_t T, float* m2_out, float* s2_out, float* zy_out, void* stream);
+int32_t grpo_loss_from_partials(grpo_ctx* ctx, int32_t n_shards, const float* m2, const float* s2, const float* zy,
+                                const int32_t* targets, int32_t V_global, const int32_t* cu_seqlens, int32_t S, int64_t T,
+                                const float* adv, const float* old_logp, const float* ref_logp, const uint8_t* mask,
+                                double loss_denom, float* logp_out, float* lse_out, float* coeff_out, float* loss_accum,
+                                float* metrics_accum, void* stream);
+
 /* A4-A6.  lse, coeff from the forward.  grad_scale multiplies both gradients (upstream dLoss).
  * dhidden_out [T, d] (bf16, or fp32 if cfg.dhidden_fp32) is OVERWRITTEN; dW_accum fp32 [V, d] is
  * ADDED to with atomics (caller zeroes it at the optimizer boundary).  Either may be NULL to skip. */

@@ -22,6 +22,7 @@ EXPORTS = [
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
     "grpo_fused_logprob_loss_fwd_bwd", "grpo_set_entropy_out", "grpo_set_seq_denom", "grpo_bwd_row_stats_sync",
     "grpo_rmsnorm_fwd", "grpo_rmsnorm_bwd", "grpo_fused_logprob_loss_bwd_prenorm", "grpo_debug_max_active_clusters",
+    "grpo_vocab_shard_partials", "grpo_loss_from_partials",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
     "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
@@ -96,6 +97,9 @@ def load_library() -> C.CDLL:
     lib.grpo_bwd_tile_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     lib.grpo_set_entropy_out.argtypes = [vp, vp]
     lib.grpo_set_seq_denom.argtypes = [vp, i32]
+    lib.grpo_vocab_shard_partials.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
+    lib.grpo_loss_from_partials.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, i32, i64, vp, vp, vp, vp, f64, vp, vp, vp,
+                                            vp, vp, vp]
     lib.grpo_debug_max_active_clusters.argtypes = [vp, i32, C.POINTER(i32)]
     lib.grpo_rmsnorm_fwd.argtypes = [vp, vp, vp, f32, i64, vp, vp, vp]
     lib.grpo_rmsnorm_bwd.argtypes = [vp, vp, vp, vp, vp, i32, i64, vp, vp, vp]
@@ -230,6 +234,36 @@ class GrpoContext:
             _dev(logp, torch.float32, "logp"), _dev(lse, torch.float32, "lse"), _dev(coeff, torch.float32, "coeff"),
             _dev(loss_accum, torch.float32, "loss_accum"), _dev(metrics_accum, torch.float32, "metrics_accum"),
             _stream(stream)))
+        return dict(logp=logp, lse=lse, coeff=coeff, loss=loss_accum)
+
+    # ------------------------------------------------------------------ NEXT-3(b): vocab-parallel forward
+    def grpo_vocab_shard_partials(self, hidden, W_shard, targets_local, stream=None):
+        T = hidden.shape[0]
+        self.ensure_workspace(T, 1)
+        out = [torch.empty(T, dtype=torch.float32, device=hidden.device) for _ in range(3)]
+        _check(self.lib.grpo_vocab_shard_partials(
+            self.h, _dev(hidden, torch.bfloat16, "hidden", T * self.cfg.d), _dev(W_shard, torch.bfloat16, "W_shard", self.cfg.V * self.cfg.d),
+            _dev(targets_local, torch.int32, "targets_local", T), T, *[_dev(o, torch.float32, "out") for o in out],
+            _stream(stream)))
+        return tuple(out)
+
+    def grpo_loss_from_partials(self, m2, s2, zy, targets, V_global: int, cu_seqlens, adv, old_logp, ref_logp=None,
+                                mask=None, loss_denom: float = 0.0, loss_accum=None, metrics_accum=None, stream=None):
+        n_shards, T = m2.shape
+        S = cu_seqlens.numel() - 1
+        self.ensure_workspace(T, 1)
+        dev = m2.device
+        logp, lse, coeff = [torch.empty(T, dtype=torch.float32, device=dev) for _ in range(3)]
+        if loss_accum is None:
+            loss_accum = torch.zeros(1, dtype=torch.float32, device=dev)
+        _check(self.lib.grpo_loss_from_partials(
+            self.h, n_shards, _dev(m2, torch.float32, "m2", n_shards * T), _dev(s2, torch.float32, "s2", n_shards * T),
+            _dev(zy, torch.float32, "zy", n_shards * T), _dev(targets, torch.int32, "targets", T), int(V_global),
+            _dev(cu_seqlens, torch.int32, "cu_seqlens"), S, T, _dev(adv, torch.float32, "adv", S),
+            _dev(old_logp, torch.float32, "old_logp", T), _dev(ref_logp, torch.float32, "ref_logp", T),
+            _dev(mask, torch.uint8, "mask", T), float(loss_denom), _dev(logp, torch.float32, "logp"),
+            _dev(lse, torch.float32, "lse"), _dev(coeff, torch.float32, "coeff"), _dev(loss_accum, torch.float32, "loss_accum"),
+            _dev(metrics_accum, torch.float32, "metrics_accum"), _stream(stream)))
         return dict(logp=logp, lse=lse, coeff=coeff, loss=loss_accum)
 
     # ------------------------------------------------------------------ A4 - A6

@@ -536,8 +536,10 @@ static int32_t fwd_check(grpo_ctx* ctx, int32_t S, int64_t T) {
 }
 
 // Loss-bearing token counts that define the mean (whole call, before any row is processed).
-static int32_t fwd_counts(grpo_ctx* ctx, int slot, const int32_t* targets, const FwdArgs& a, cudaStream_t st) {
+static int32_t fwd_counts(grpo_ctx* ctx, int slot, const int32_t* targets, const FwdArgs& a, cudaStream_t st,
+                          int V = 0) {
   const grpo_config& c = ctx->cfg;
+  if (V <= 0) V = c.V;
   const SlotLayout& L = ctx->lay;
   float* total = slot_ptr<float>(ctx, slot, L.off_total);
   float* seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
@@ -548,22 +550,22 @@ static int32_t fwd_counts(grpo_ctx* ctx, int slot, const int32_t* targets, const
     const int blocks = (a.S * 32 + threads - 1) / threads;
     {
       LaunchScope ls(ctx, GRPO_KERNEL_TOKEN_COUNT, st);
-      token_count_kernel<<<blocks, threads, 0, st>>>(a.mask, targets, c.V, a.cu_seqlens, a.S, seq_count, total);
+      token_count_kernel<<<blocks, threads, 0, st>>>(a.mask, targets, V, a.cu_seqlens, a.S, seq_count, total);
     }
     CU_OK(cudaGetLastError());
   }
   return GRPO_OK;
 }
 
-// A2 + A3 over packed rows [t0, t0 + rows) of a call of T tokens.  stash != nullptr: the 3-contraction
-// variant's forward, which also writes the chunk's scaled logits (fp16) to `stash`.
-static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
-                        const FwdArgs& a, int64_t T, int64_t t0, int64_t rows, __nv_bfloat16* stash, cudaStream_t st) {
+// A2 alone over packed rows [t0, t0 + rows): the per-split (max, sum-exp) partials land in the slot's partial
+// buffers ([n_split, rows], log2 domain), the target logit in zy[t] (rows whose target is not a column of W are
+// left untouched).
+static int32_t a2_rows(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets, float* zy,
+                       bool entropy, int64_t t0, int64_t rows, __nv_bfloat16* stash, cudaStream_t st, int* n_split_out) {
   const grpo_config& c = ctx->cfg;
   const SlotLayout& L = ctx->lay;
   float* part_m = slot_ptr<float>(ctx, slot, L.off_part_m);
   float* part_s = slot_ptr<float>(ctx, slot, L.off_part_s);
-  float* zy = slot_ptr<float>(ctx, slot, L.off_zy);
 
   CUtensorMap tmH, tmW;
   const void* Hc = static_cast<const uint8_t*>(hidden) + t0 * c.d * 2;
@@ -586,7 +588,7 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
   p.logit_scale = c.logit_scale;
   p.part_m = part_m;
   p.part_s = part_s;
-  p.part_u = a.entropy_out ? slot_ptr<float>(ctx, slot, L.off_part_u) : nullptr;
+  p.part_u = entropy ? slot_ptr<float>(ctx, slot, L.off_part_u) : nullptr;
   p.part_stride = rows;
   p.zy = zy;
   p.dz = stash; p.dz_pitch = L.v_pad;
@@ -596,12 +598,24 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
     GRPO_TRY((launch_gemm<false, false, EPI_LSE_STASH>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
   else
     GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
+  *n_split_out = p.n_split;
+  return GRPO_OK;
+}
 
+// A3 over packed rows [t0, t0 + rows): combines `n_parts` (max, sum-exp) partials per token (part arrays
+// [n_parts, part_stride], indexed by the launch's own row) and n_zy target-logit arrays (summed; stride zy_stride,
+// indexed by the packed row), then the loss / coefficient arithmetic.  V = the GLOBAL vocabulary size.
+static int32_t loss_rows(grpo_ctx* ctx, int slot, const float* part_m, const float* part_s, const float* part_u,
+                         int n_parts, int64_t part_stride, const float* zy, int n_zy, int64_t zy_stride, int V,
+                         const int32_t* targets, const FwdArgs& a, int64_t t0, int64_t rows, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  const SlotLayout& L = ctx->lay;
   LossParams lp;
   std::memset(&lp, 0, sizeof(lp));
-  lp.T = rows; lp.t_begin = t0; lp.S = a.S; lp.S_norm = a.S_norm > 0 ? a.S_norm : a.S; lp.V = c.V;
-  lp.n_split = p.n_split; lp.part_stride = rows;
-  lp.part_m = part_m; lp.part_s = part_s; lp.part_u = p.part_u; lp.entropy = a.entropy_out; lp.zy = zy; lp.targets = targets; lp.cu_seqlens = a.cu_seqlens;
+  lp.T = rows; lp.t_begin = t0; lp.S = a.S; lp.S_norm = a.S_norm > 0 ? a.S_norm : a.S; lp.V = V;
+  lp.n_split = n_parts; lp.part_stride = part_stride;
+  lp.part_m = part_m; lp.part_s = part_s; lp.part_u = part_u; lp.entropy = a.entropy_out; lp.zy = zy;
+  lp.n_zy = n_zy; lp.zy_stride = zy_stride; lp.targets = targets; lp.cu_seqlens = a.cu_seqlens;
   lp.adv = a.adv; lp.old_logp = a.old_logp; lp.ref_logp = a.ref_logp; lp.mask = a.mask;
   lp.seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
   lp.total_count = a.denom_dev ? a.denom_dev : slot_ptr<float>(ctx, slot, L.off_total);
@@ -618,6 +632,20 @@ static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void*
   }
   CU_OK(cudaGetLastError());
   return GRPO_OK;
+}
+
+// A2 + A3 over packed rows [t0, t0 + rows) of a call of T tokens.  stash != nullptr: the 3-contraction
+// variant's forward, which also writes the chunk's softmax numerators (fp16) to `stash`.
+static int32_t fwd_rows(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
+                        const FwdArgs& a, int64_t T, int64_t t0, int64_t rows, __nv_bfloat16* stash, cudaStream_t st) {
+  const SlotLayout& L = ctx->lay;
+  (void)T;
+  float* zy = slot_ptr<float>(ctx, slot, L.off_zy);
+  int n_split = 1;
+  GRPO_TRY(a2_rows(ctx, slot, hidden, W, targets, zy, a.entropy_out != nullptr, t0, rows, stash, st, &n_split));
+  return loss_rows(ctx, slot, slot_ptr<float>(ctx, slot, L.off_part_m), slot_ptr<float>(ctx, slot, L.off_part_s),
+                   a.entropy_out ? slot_ptr<float>(ctx, slot, L.off_part_u) : nullptr, n_split, rows, zy, 1, 0,
+                   ctx->cfg.V, targets, a, t0, rows, st);
 }
 
 static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void* W, const int32_t* targets,
@@ -652,6 +680,65 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden
   return fwd_impl(ctx, 0, hidden, W, targets, cu_seqlens, S, T, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
                   logp_out, lse_out, coeff_out, loss_accum, metrics_accum, static_cast<cudaStream_t>(stream),
                   ctx->entropy_out, ctx->seq_denom);
+}
+
+// ------------------------------------------------------------------------------------- NEXT-3(b): vocab-parallel LSE
+// (max, sum-exp) of one token over the splits of a launch, in split order (log2 domain).
+__global__ void combine_partials_kernel(const float* __restrict__ part_m, const float* __restrict__ part_s, int n_split,
+                                        int64_t stride, int64_t rows, float* __restrict__ m2_out,
+                                        float* __restrict__ s2_out) {
+  const int64_t r = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (r >= rows) return;
+  float M = -INFINITY;
+  for (int i = 0; i < n_split; ++i) M = fmaxf(M, part_m[i * stride + r]);
+  float sum = 0.f;
+  for (int i = 0; i < n_split; ++i) sum += part_s[i * stride + r] * exp2f(part_m[i * stride + r] - M);
+  m2_out[r] = M;
+  s2_out[r] = sum;
+}
+
+extern "C" int32_t grpo_vocab_shard_partials(grpo_ctx* ctx, const void* hidden, const void* W_shard,
+                                             const int32_t* targets_local, int64_t T, float* m2_out, float* s2_out,
+                                             float* zy_out, void* stream) {
+  if (!ctx || !hidden || !W_shard || !targets_local || !m2_out || !s2_out || !zy_out)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (T <= 0) return fail(GRPO_ERR_SHAPE, "need T > 0");
+  GRPO_TRY(fwd_check(ctx, 1, T));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const SlotLayout& L = ctx->lay;
+  CU_OK(cudaMemsetAsync(zy_out, 0, static_cast<size_t>(T) * 4, st));   // rows whose target lives in another shard
+  for (int64_t t0 = 0; t0 < T; t0 += L.fwd_block_rows) {
+    const int64_t rows = std::min<int64_t>(L.fwd_block_rows, T - t0);
+    int n_split = 1;
+    GRPO_TRY(a2_rows(ctx, 0, hidden, W_shard, targets_local, zy_out, false, t0, rows, nullptr, st, &n_split));
+    {
+      LaunchScope ls(ctx, GRPO_KERNEL_LOSS, st);
+      combine_partials_kernel<<<static_cast<unsigned>((rows + 255) / 256), 256, 0, st>>>(
+          slot_ptr<float>(ctx, 0, L.off_part_m), slot_ptr<float>(ctx, 0, L.off_part_s), n_split, rows, rows, m2_out + t0,
+          s2_out + t0);
+    }
+    CU_OK(cudaGetLastError());
+  }
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_loss_from_partials(grpo_ctx* ctx, int32_t n_shards, const float* m2, const float* s2,
+                                           const float* zy, const int32_t* targets, int32_t V_global,
+                                           const int32_t* cu_seqlens, int32_t S, int64_t T, const float* adv,
+                                           const float* old_logp, const float* ref_logp, const uint8_t* mask,
+                                           double loss_denom, float* logp_out, float* lse_out, float* coeff_out,
+                                           float* loss_accum, float* metrics_accum, void* stream) {
+  if (!ctx || !m2 || !s2 || !zy || !targets || !cu_seqlens || !adv || !old_logp || !logp_out || !lse_out || !coeff_out ||
+      !loss_accum)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (n_shards < 1 || V_global < 1 || T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need n_shards, V_global, T, S > 0");
+  GRPO_TRY(fwd_check(ctx, S, T));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
+            logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
+  a.S_norm = ctx->seq_denom;
+  GRPO_TRY(fwd_counts(ctx, 0, targets, a, st, V_global));
+  return loss_rows(ctx, 0, m2, s2, nullptr, n_shards, T, zy, n_shards, T, V_global, targets, a, 0, T, st);
 }
 
 extern "C" int32_t grpo_set_seq_denom(grpo_ctx* ctx, int32_t n_sequences) {

@@ -90,7 +90,9 @@ struct LossParams {
   const float* part_m;
   const float* part_s;
   const float* part_u;       // nullable (entropy output)
-  const float* zy;
+  const float* zy;           // target logit s z_t[y_t]: n_zy arrays of stride zy_stride are summed (vocab shards:
+  int n_zy;                  // exactly one shard holds the target column, the others hold 0)
+  int64_t zy_stride;
   const int32_t* targets;
   const int32_t* cu_seqlens;
   const float* adv;
@@ -135,7 +137,12 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
     const int y = p.targets[t];
     const bool valid = y >= 0 && y < p.V;
     if (y >= p.V) atomicOr(p.err_flag, 1);
-    const float logp = valid ? p.zy[t] - lse : 0.f;
+    float zy = 0.f;
+    if (valid) {
+      zy = p.zy[t];
+      for (int i = 1; i < p.n_zy; ++i) zy += p.zy[i * p.zy_stride + t];
+    }
+    const float logp = valid ? zy - lse : 0.f;
     // sequence of this token: largest s with cu_seqlens[s] <= t
     int lo = 0, hi = p.S;
     while (hi - lo > 1) {
