@@ -25,7 +25,8 @@ NEXT-4 (R29-R31): the final RMSNorm in front of the 
 (``rmsnorm_fwd`` / ``rmsnorm_bwd`` / ``grpo_step_from_prenorm``) — pinned in tests/test_oracle_rmsnorm.py by a
 hand-worked example, ``torch.nn.functional.rms_norm`` and its autograd, scale invariance / orthogonality
 identities and finite differences of the whole step w.r.t. the pre-norm activations and the norm weight;
-"parity unpinned" by the paper (it never mentions the norm).
+"parity unpinned" by the paper (it never mentions the norm).  FP8 precision study (R32): ``e4m3_round`` is pinned
+against torch's float8_e4m3fn conversion on every representable value, its midpoints and random inputs.
 
 Pins (tests/test_oracle_pins.py): P1-P14 of SURVEY.md §8(c).  The paper prints no
 worked number for the loss, so every pin is a closed form, invariant, library special
@@ -44,6 +45,7 @@ __all__ = [
     "token_logprobs", "loss_terms", "backward", "grpo_step", "grpo_step_loops",
     "token_rows", "dH_rows", "dW_rows", "token_entropy",
     "round_to_bf16", "rmsnorm_fwd", "rmsnorm_bwd", "grpo_step_from_prenorm",
+    "e4m3_round", "fp8_dequantized_operands",
 ]
 
 
@@ -348,6 +350,36 @@ def grpo_step_from_prenorm(x, gamma, W, y, cu_seqlens, rewards, old_logp, ref_lo
     out["H"], out["rstd"] = H, rstd
     out["dx"], out["dgamma"] = rmsnorm_bwd(x, gamma, rstd, out["dH"])
     return out
+
+
+# ------------------------------------------------------ NEXT-4: FP8 precision study (R32)
+def e4m3_round(y):
+    """Nearest value of the 8-bit float format E4M3 (1 sign, 4 exponent bits with bias 7, 3 mantissa bits; no
+    infinities; largest finite 448; smallest normal 2^-6; subnormals k 2^-9), round to nearest, ties to even,
+    saturating at +-448.  Input: any float array; returns float64 values on the E4M3 grid."""
+    y = np.asarray(y, dtype=np.float64)
+    a = np.abs(y)
+    e = np.floor(np.log2(np.maximum(a, 2.0 ** -6)))          # binade of |y| (>= the smallest normal's)
+    step = 2.0 ** (e - 3)                                     # spacing inside that binade: 3 mantissa bits
+    q = np.rint(a / step) * step                              # np.rint rounds halves to even
+    q = np.minimum(q, 448.0)
+    return np.sign(y) * q
+
+
+def fp8_dequantized_operands(H, W):
+    """The operands the FP8 study contracts (cfg.fp8_logits; R32), dequantised back to float64:
+    every hidden row t is scaled by s_t = amax_t / 448 (1 for an all-zero row) and rounded to E4M3, the vocab matrix
+    by ONE scale amax(W) / 448.  The rounding decision is taken in the kernel's precision (fp32:
+    inv = 1 / s, y = x * inv - IEEE single operations, reproduced here with numpy float32), so both sides quantise
+    to the same codes; everything after the decision is float64.  Returns (H~ = q s_t, W~ = q s_W)."""
+    def quant(x, per_row):
+        x32 = np.asarray(x, dtype=np.float32)
+        amax = np.abs(x32).max(axis=1, keepdims=True) if per_row else np.abs(x32).max(keepdims=True).reshape(1, 1)
+        s = np.where(amax > 0, amax * np.float32(1.0 / 448.0), np.float32(1.0)).astype(np.float32)
+        inv = (np.float32(1.0) / s).astype(np.float32)
+        q = e4m3_round((x32 * inv).astype(np.float32))
+        return q * s.astype(np.float64)
+    return quant(H, True), quant(W, False)
 
 
 # ------------------------------------------------------------------------ whole step

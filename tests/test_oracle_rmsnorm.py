@@ -140,3 +140,31 @@ def test_prenorm_step_is_the_plain_step_on_the_normalised_hidden_state():
     np.testing.assert_allclose(a["loss"], loss.item(), rtol=1e-12)
     np.testing.assert_allclose(a["dx"], x.grad.numpy(), rtol=1e-9, atol=1e-15)
     np.testing.assert_allclose(a["dgamma"], g.grad.numpy(), rtol=1e-9, atol=1e-15)
+
+
+# ------------------------------------------------------------------ FP8 study: the E4M3 rounding of the oracle
+def test_e4m3_round_is_torch_float8_e4m3fn():
+    """Library routine: torch's float8_e4m3fn conversion (round to nearest even).  Every representable magnitude,
+    every midpoint between neighbours (ties), random values over the whole range, and saturation at 448."""
+    from oracle.grpo_oracle import e4m3_round, fp8_dequantized_operands
+    grid = torch.arange(0, 256, dtype=torch.uint8).view(torch.float8_e4m3fn).float()
+    grid = np.sort(np.unique(grid[torch.isfinite(grid)].double().numpy()))
+    assert grid.max() == 448.0 and 2.0 ** -9 in grid and len(grid) == 253                  # 2 x 126 + zero
+    mids = (grid[1:] + grid[:-1]) / 2
+    rng = np.random.default_rng(0)
+    rand = rng.normal(size=20000) * 10.0 ** rng.uniform(-4, 2.6, size=20000)
+    x = np.concatenate([grid, mids, rand, [447.9, 448.0, 463.9, 1e-12, -1e-12, 0.0]])
+    x = x[np.abs(x) <= 464.0]                  # beyond the last midpoint torch's e4m3fn gives NaN; the kernel saturates
+    want = torch.tensor(x, dtype=torch.float32).to(torch.float8_e4m3fn).double().numpy()
+    got = e4m3_round(np.float32(x))
+    np.testing.assert_array_equal(got, want)
+    np.testing.assert_array_equal(e4m3_round(np.array([500.0, -1e6, 449.0])), [448.0, -448.0, 448.0])   # satfinite
+    # the recipe: per-row scale amax/448 for H, one scale for W; the row maximum itself is represented exactly
+    H = rng.normal(size=(5, 16))
+    H[3] = 0.0
+    W = rng.normal(size=(7, 16)) * 0.02
+    Hq, Wq = fp8_dequantized_operands(H, W)
+    np.testing.assert_allclose(np.abs(Hq).max(axis=1), np.abs(np.float32(H)).max(axis=1), rtol=1e-6)
+    assert np.all(Hq[3] == 0.0)
+    np.testing.assert_allclose(np.abs(Wq).max(), np.abs(np.float32(W)).max(), rtol=1e-6)
+    assert np.abs(Hq - H).max() <= np.abs(H).max() * 2.0 ** -4 and np.abs(Wq - W).max() <= np.abs(W).max() * 2.0 ** -4
