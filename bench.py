@@ -295,6 +295,8 @@ def run_ours(args):
         extra["bwd_skip_zero_tiles"] = -1
     if args.no_drift_gate:
         extra["gemm_drift_epoch_kb"] = -1
+    if args.fp8:
+        extra["fp8_logits"] = 1
     if args.stash:
         extra["stash_logits"] = 1           # grpo_step_host (the e2e leg) then uses the same variant
     ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
@@ -356,7 +358,7 @@ def run_ours(args):
     # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step.  Timed
     # right after the headline region so that both see the same thermal / power state of the board.
     e2e_s, h2d, d2h = 0.0, 0, 0
-    if args.config == 2 and not args.prenorm:
+    if args.config == 2 and not args.prenorm and not args.fp8:
         pin = lambda t: None if t is None else t.cpu().pin_memory()
         h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
                                                        pin(b.old_logp))
@@ -428,7 +430,7 @@ def run_ours(args):
 
     # ---- the other variant of the step, timed the same way (reported beside the headline, never as it)
     args.other_variant = None
-    if not args.no_variants and not args.prenorm:
+    if not args.no_variants and not args.prenorm and not args.fp8:
         other = step_recompute if args.stash else step_stash
         for _ in range(3):
             other()
@@ -446,7 +448,7 @@ def run_ours(args):
                               "ms_per_step": v_ms / args.steps}
 
     # ---- informational runs (--config 3/4/5, --prenorm) are device-resident: no e2e / cpu_baseline legs
-    if args.config != 2 or args.prenorm:
+    if args.config != 2 or args.prenorm or args.fp8:
         ms_total, _, tokens_all = reduce_over_ranks(ms_total, 0.0, T, world, dev)
         if rank == 0:
             line = build_line(args, b, world, tokens_all * args.steps / (ms_total * 1e-3), ms_total, None, 0, 0,
@@ -625,7 +627,10 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         e = {"ms_per_step": v["ms"] / steps, "launches_per_step": v["launches"] / steps}
         if k in GEMM_KINDS:
             e["tflops"] = kind_flops[k] * steps / (v["ms"] * 1e-3) / 1e12
-            e["frac_of_peak"] = e["tflops"] / peak
+            # --fp8: A2 / A4 run on e4m3 operands; their peak is the measured bf16 peak x the nominal fp8 : bf16
+            # ratio of 2 (4.5 vs 2.25 PFLOP/s dense, B200_PROFILING.md)
+            k_peak = peak * (2.0 if getattr(args, "fp8", False) and k in ("gemm_lse", "gemm_dz") else 1.0)
+            e["frac_of_peak"] = e["tflops"] / k_peak
         if k == "loss" and world == 1 and args.config == 2 and not args.stash:
             # A3 reads / writes >= 56 B per token (one LSE split); launch-latency bound at this size
             e["gbps_at_least"] = 56.0 * T * steps / (v["ms"] * 1e-3) / 1e9
@@ -657,9 +662,10 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
+        "dtype": "e4m3 (A2, A4 operands) + bf16" if getattr(args, "fp8", False) else "bf16", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config],
-                   "variant": "prenorm (informational, NEXT-4): RMSNorm fwd + north_star path + RMSNorm bwd fused behind A5"
+                   "variant": "fp8_logits (informational PRECISION STUDY, NEXT-4: e4m3 operands for A2 / A4; does not meet "
+                   "north_star's log-prob tolerance)" if args.fp8 else "prenorm (informational, NEXT-4): RMSNorm fwd + north_star path + RMSNorm bwd fused behind A5"
                    if args.prenorm else "stash_logits (3 contractions, DESIGN.md section 11)" if args.stash
                    else "recompute (north_star: 4 contractions)",
                    "tokens_per_step": int(tokens_all), "tokens_rank0": T, "d": d, "V": V, "G": b.G,
@@ -698,6 +704,9 @@ def main():
     ap.add_argument("--prenorm", action="store_true",
                     help="informational (NEXT-4): the step starts from pre-norm activations (grpo_rmsnorm_fwd, forward, "
                          "grpo_fused_logprob_loss_bwd_prenorm); no e2e / cpu_baseline legs")
+    ap.add_argument("--fp8", action="store_true",
+                    help="informational precision study (NEXT-4): grpo_config.fp8_logits = 1 (e4m3 operands for the two "
+                         "logit contractions); no e2e / cpu_baseline legs")
     ap.add_argument("--no-variants", action="store_true", help="do not time the other variant beside the headline")
     ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")

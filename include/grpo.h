@@ -86,6 +86,14 @@ typedef struct {
   int32_t stash_logits;      /* 0 = default: grpo_enqueue_groups / grpo_step_host run forward then backward with
                                 the logits RECOMPUTED chunk by chunk (north_star, 4 contractions); 1 = they run
                                 grpo_fused_logprob_loss_fwd_bwd instead (3 contractions) */
+  int32_t fp8_logits;        /* 0 = default (bf16).  1 = FP8 PRECISION STUDY (DESIGN.md
+                                section 13): the two logit contractions (A2 and the A4 recompute) run on e4m3 operands
+                                (tcgen05 kind::f8f6f4, twice the bf16 tensor rate): every hidden row is quantised with
+                                its own scale amax/448, the vocab matrix with one scale for the tensor, both folded
+                                into the epilogue; dZ, A5 and A6 stay bf16 x bf16 -> fp32.  Log-probs then carry the
+                                e4m3 rounding of the operands (2^-4 relative per element): this does NOT meet
+                                north_star's 2e-3 log-prob tolerance and is never the default or the headline.
+                                Needs d % 16 == 0; not with stash_logits. */
 } grpo_config;
 
 /* Fill *cfg with the defaults above (d, V must still be set). */
@@ -294,7 +302,8 @@ enum {
   GRPO_KERNEL_DH_REDUCE = 11,  /* A5: fixed-order sum of the split-K partials (+ scatter of compacted rows; + the
                                   RMSNorm backward of the pre-norm calls) */
   GRPO_KERNEL_RMSNORM = 12,    /* NEXT-4: final RMSNorm forward */
-  GRPO_NUM_KERNEL_KINDS = 13
+  GRPO_KERNEL_QUANTIZE = 13,   /* FP8 study: e4m3 quantisation of hidden rows / the vocab matrix */
+  GRPO_NUM_KERNEL_KINDS = 14
 };
 
 /* Token tiles the 3-contraction backward calls of workspace slot 0 walked (active) and saw (total) since the last

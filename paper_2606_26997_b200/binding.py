@@ -28,7 +28,7 @@ EXPORTS = [
     "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
 ]
 KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan", "stash_dz",
-                "compact", "dh_reduce", "rmsnorm"]
+                "compact", "dh_reduce", "rmsnorm", "quantize"]
 
 
 class GrpoError(RuntimeError):
@@ -44,7 +44,7 @@ class GrpoConfig(C.Structure):
                 ("groups_per_update", C.c_int32), ("groups_per_round", C.c_int32), ("token_budget", C.c_int64),
                 ("bwd_chunk_tokens", C.c_int64), ("max_pending_groups", C.c_int32), ("gemm_cta_group", C.c_int32),
                 ("gemm_drift_epoch_kb", C.c_int32), ("kl_type", C.c_int32), ("dual_clip", C.c_float),
-                ("bwd_skip_zero_tiles", C.c_int32), ("stash_logits", C.c_int32)]
+                ("bwd_skip_zero_tiles", C.c_int32), ("stash_logits", C.c_int32), ("fp8_logits", C.c_int32)]
 
 
 class GroupDesc(C.Structure):

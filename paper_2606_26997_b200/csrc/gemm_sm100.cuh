@@ -86,6 +86,10 @@ struct GemmParams {
   const int32_t* targets;
   float scale_log2e;                 // logit_scale * log2(e)
   float logit_scale;
+  // FP8 study (DT = 1): the accumulator is (H8 W8^T)[t, v]; the logit is that times the
+  // token's quantisation scale row_scale[t] times the vocab matrix' scale *w_scale.  nullptr: 1.
+  const float* row_scale;
+  const float* w_scale;
   // EPI_LSE outputs (log2 domain running max / sum per split) + the target logit
   float* part_m;
   float* part_s;
@@ -230,7 +234,10 @@ __device__ __forceinline__ void st_volatile_shared_i32(int* p, int v) {
   asm volatile("st.volatile.shared.b32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
 }
 
-template <int CG, bool A_MN, bool B_MN, int EPI>
+// DT: operand type of the contraction: 0 = bf16 (kind::f16, 64 elements per 128-byte k block), 1 = e4m3
+// (kind::f8f6f4, 128 elements per k block; K-major operands only).  Shared-memory layout, descriptors and the four
+// K = 32-byte MMAs per k block are byte-identical.
+template <int CG, bool A_MN, bool B_MN, int EPI, int DT = 0>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                  const __grid_constant__ CUtensorMap tmC, const GemmParams p, const int n_units_dense) {
@@ -238,6 +245,8 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   constexpr int kStages = Shape::kStages;
   constexpr int kStageBytes = Shape::kStageBytes;
   constexpr int kBRows = Shape::kBRows;
+  constexpr int kBKe = DT == 1 ? 2 * BK : BK;                    // elements per k block (128 bytes)
+  static_assert(DT == 0 || (!A_MN && !B_MN), "the e4m3 instance is K-major only");
   extern __shared__ uint8_t smem_raw[];
   // SWIZZLE_128B atoms need 1024-byte alignment of the tile bases (same offset in both CTAs of a pair)
   const uint32_t raw_addr = smem_u32(smem_raw);
@@ -320,13 +329,13 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               const uint32_t b_dst = a_dst + kABytes;
               const uint32_t bar = full0 + stage * 8;
               if constexpr (!A_MN) {
-                tma_load_2d_t<CG>(a_dst, &tmA, bar, kb * BK, a_row);
+                tma_load_2d_t<CG>(a_dst, &tmA, bar, kb * kBKe, a_row);
               } else {
 #pragma unroll
                 for (int i = 0; i < BM / 64; ++i) tma_load_2d_t<CG>(a_dst + i * 8192, &tmA, bar, a_row + i * 64, kb * BK);
               }
               if constexpr (!B_MN) {
-                tma_load_2d_t<CG>(b_dst, &tmB, bar, kb * BK, b_row);
+                tma_load_2d_t<CG>(b_dst, &tmB, bar, kb * kBKe, b_row);
               } else {
 #pragma unroll
                 for (int i = 0; i < kBRows / 64; ++i) tma_load_2d_t<CG>(b_dst + i * 8192, &tmB, bar, b_row + i * 64, kb * BK);
@@ -348,7 +357,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     // LBO field never change, the start-address field advances by (bytes >> 4) and cannot carry out of
     // its 14 bits (shared memory is < 256 KB).
     if (cta_rank == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(BM * CG, BN, A_MN ? 1 : 0, B_MN ? 1 : 0);
+      constexpr uint32_t idesc = DT == 1 ? make_idesc_e4m3(BM * CG, BN) : make_idesc_bf16(BM * CG, BN, A_MN ? 1 : 0, B_MN ? 1 : 0);
       constexpr uint32_t kDescHi = smem_desc_hi(1024);
       constexpr uint32_t kAdvA = (A_MN ? 2048u : 32u) >> 4, kAdvB = (B_MN ? 2048u : 32u) >> 4;
       const uint32_t a_lo0 = smem_desc_lo(tiles_addr, A_MN ? 8192u : 16u);
@@ -372,9 +381,14 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               const uint32_t a_lo = a_lo0 + stage * (kStageBytes >> 4);
               const uint32_t b_lo = b_lo0 + stage * (kStageBytes >> 4);
 #pragma unroll
-              for (int k = 0; k < BK / 16; ++k)
-                umma_bf16<CG>(d_tmem, make_desc64(a_lo + k * kAdvA, kDescHi), make_desc64(b_lo + k * kAdvB, kDescHi),
+              for (int k = 0; k < BK / 16; ++k) {
+                if constexpr (DT == 1)
+                  umma_f8<CG>(d_tmem, make_desc64(a_lo + k * kAdvA, kDescHi), make_desc64(b_lo + k * kAdvB, kDescHi),
                               idesc, (kb | k) != 0 ? 1u : 0u);
+                else
+                  umma_bf16<CG>(d_tmem, make_desc64(a_lo + k * kAdvA, kDescHi), make_desc64(b_lo + k * kAdvB, kDescHi),
+                                idesc, (kb | k) != 0 ? 1u : 0u);
+              }
               umma_commit_t<CG>(&bars->empty[stage]);    // smem slot (of both CTAs) reusable once these MMAs retire
             }
             __syncwarp();
@@ -437,6 +451,16 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           kcoef = p.coeff[row_g] * p.coeff_mul;
         }
       }
+      // logit = accumulator x sl (natural units) = accumulator x sl2 (log2 domain); DT = 1 folds the row's and the
+      // vocab matrix' quantisation scales in
+      [[maybe_unused]] float sl2 = p.scale_log2e, sl = p.logit_scale;
+      if constexpr (DT == 1) {
+        if (row_ok) {
+          const float rs = p.row_scale[row_g] * *p.w_scale;
+          sl2 *= rs;
+          sl *= rs;
+        }
+      }
 
       for (int n_tile = n0; n_tile < n1; ++n_tile) {
         mbar_wait(&bars->tmem_full[acc], acc_phase);
@@ -461,7 +485,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll
             for (int i = 0; i < 32; i += 2) tmax = max3(tmax, v[i], v[i + 1]);
           }
-          const float new_m = fmaxf(run_m, tmax * p.scale_log2e);   // scale_log2e > 0: the max commutes with the scale
+          const float new_m = fmaxf(run_m, tmax * sl2);             // sl2 > 0: the max commutes with the scale
           const float rescale = ex2_approx(run_m - new_m);
           run_s *= rescale;
           run_u *= rescale;
@@ -490,10 +514,10 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               float cmax = v[0];
 #pragma unroll
               for (int i = 1; i < 31; i += 2) cmax = max3(cmax, v[i], v[i + 1]);
-              new_m = fmaxf(run_m, fmaxf(cmax, v[31]) * p.scale_log2e);
+              new_m = fmaxf(run_m, fmaxf(cmax, v[31]) * sl2);
             }
             const float rescale = ex2_approx(run_m - new_m);
-            const f32x2 sc2 = pack2(p.scale_log2e, p.scale_log2e), nm2 = pack2(-new_m, -new_m);
+            const f32x2 sc2 = pack2(sl2, sl2), nm2 = pack2(-new_m, -new_m);
             float e[32];
             f32x2 acc = pack2(0.f, 0.f);
 #pragma unroll
@@ -510,7 +534,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             if (p.part_u != nullptr) {   // entropy = lse - sum_v p_v z_v: one more running sum, rescaled like run_s
               float uc = 0.f;
 #pragma unroll
-              for (int i = 0; i < 32; ++i) uc = fmaf(e[i], i < nvalid ? v[i] * p.scale_log2e : 0.f, uc);   // 0 * -inf is NaN
+              for (int i = 0; i < 32; ++i) uc = fmaf(e[i], i < nvalid ? v[i] * sl2 : 0.f, uc);   // 0 * -inf is NaN
               run_u = (EPI == EPI_LSE_STASH ? run_u : run_u * rescale) + uc;
             }
             if constexpr (EPI == EPI_LSE_STASH) {
@@ -528,12 +552,12 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               float zy = 0.f;
 #pragma unroll
               for (int i = 0; i < 32; ++i) zy = (y - cbase == i) ? v[i] : zy;
-              p.zy[row_g] = zy * p.logit_scale;                    // natural units: s * z
+              p.zy[row_g] = zy * sl;                               // natural units: s * z
             }
           } else if constexpr (EPI == EPI_DZ) {
             // dz = k (1[v = y] - p),  p = 2^(z s log2e - lse log2e)
             float dzv[32];
-            const f32x2 sc2 = pack2(p.scale_log2e, p.scale_log2e), nl2 = pack2(-lse2, -lse2), nk2 = pack2(-kcoef, -kcoef);
+            const f32x2 sc2 = pack2(sl2, sl2), nl2 = pack2(-lse2, -lse2), nk2 = pack2(-kcoef, -kcoef);
 #pragma unroll
             for (int i = 0; i < 32; i += 2) {
               float t0, t1;

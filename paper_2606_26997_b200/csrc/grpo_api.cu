@@ -66,6 +66,7 @@ struct SlotLayout {
           off_row_stats = 0;
   int64_t n_chunks_max = 0;
   int64_t fwd_block_rows = 0;   // rows per A2 launch (bounds the LSE partials)
+  int64_t off_w8 = 0, off_h8 = 0, off_hscale = 0, off_wscale = 0;   // FP8 study (cfg.fp8_logits)
   int64_t bytes = 0;
 };
 
@@ -212,6 +213,12 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.off_coeffc = take(L.chunk_rows * 4);
   L.off_dh_part = take(static_cast<int64_t>(k_split) * L.chunk_rows * c.d * 4);
   L.off_row_stats = take(16);
+  if (c.fp8_logits) {
+    L.off_w8 = take(static_cast<int64_t>(c.V) * c.d);
+    L.off_h8 = take(std::max(L.fwd_block_rows, L.chunk_rows) * c.d);
+    L.off_hscale = take(max_T * 4 + 1024);
+    L.off_wscale = take(256);
+  }
   L.bytes = off;
   return L;
 }
@@ -240,6 +247,22 @@ static int32_t make_tmap(const grpo_ctx* ctx, CUtensorMap* m, const void* base, 
   return GRPO_OK;
 }
 
+// e4m3 operand (FP8 study): 2-D byte tensor, 128-byte k blocks, 128B swizzle.
+static int32_t make_tmap_u8(const grpo_ctx* ctx, CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer,
+                            uint64_t pitch_bytes, uint32_t box_outer) {
+  if ((reinterpret_cast<uintptr_t>(base) & 15) != 0 || (pitch_bytes & 15) != 0)
+    return fail(GRPO_ERR_SHAPE, "e4m3 tensor base/pitch not 16-byte aligned (need d %% 16 == 0)");
+  cuuint64_t dims[2] = {inner, outer};
+  cuuint64_t strides[1] = {pitch_bytes};
+  cuuint32_t box[2] = {128, box_outer};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(GRPO_ERR_CUDA, "cuTensorMapEncodeTiled (u8) failed with CUresult %d", (int)r);
+  return GRPO_OK;
+}
+
 // fp32 C tensor [outer, inner] for the A6 epilogue's TMA reduce-add: 32 x 32 boxes (128-byte rows), 128B swizzle.
 static int32_t make_tmap_c_f32(const grpo_ctx* ctx, CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer,
                                uint64_t pitch_bytes) {
@@ -258,13 +281,13 @@ static int32_t make_tmap_c_f32(const grpo_ctx* ctx, CUtensorMap* m, const void* 
 }
 
 
-template <int CG, bool A_MN, bool B_MN, int EPI>
+template <int CG, bool A_MN, bool B_MN, int EPI, int DT = 0>
 static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB,
                               const GemmParams& p, int n_units, cudaStream_t st, const CUtensorMap* tmC) {
   // the dynamic shared memory limit is a per-device attribute of the function: one flag bit per device and
   // template instantiation (setting it twice is harmless, so a relaxed atomic is enough)
   static std::atomic<uint64_t> attr_set{0};
-  auto kern = grpo_gemm_kernel<CG, A_MN, B_MN, EPI>;
+  auto kern = grpo_gemm_kernel<CG, A_MN, B_MN, EPI, DT>;
   constexpr int smem = GemmShape<CG>::kSmemBytes;
   const uint64_t dev_bit = 1ull << (ctx->device & 63);
   if (ctx->device >= 64 || !(attr_set.load(std::memory_order_relaxed) & dev_bit)) {
@@ -313,12 +336,43 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   return GRPO_OK;
 }
 
-template <bool A_MN, bool B_MN, int EPI>
+template <bool A_MN, bool B_MN, int EPI, int DT = 0>
 static int32_t launch_gemm(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB, const GemmParams& p,
                            int n_units, cudaStream_t st, const CUtensorMap* tmC = nullptr) {
   if (EPI == EPI_RED_F32 && tmC == nullptr) return fail(GRPO_ERR_INVALID_ARG, "EPI_RED_F32 needs the C tensor map");
-  if (ctx->cg == 2) return launch_gemm_cg<2, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
-  return launch_gemm_cg<1, A_MN, B_MN, EPI>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
+  if (ctx->cg == 2) return launch_gemm_cg<2, A_MN, B_MN, EPI, DT>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
+  return launch_gemm_cg<1, A_MN, B_MN, EPI, DT>(ctx, kind, tmA, tmB, p, n_units, st, tmC);
+}
+
+// FP8 study: quantise `rows` bf16 rows of width d to e4m3 (per-row scales, or the tensor's scale `fixed`).
+static int32_t quantize_rows(grpo_ctx* ctx, const void* x, int64_t rows, void* q, float* scales, const float* fixed,
+                             cudaStream_t st) {
+  if (rows <= 0) return GRPO_OK;
+  const int64_t blocks = std::min<int64_t>((rows + 7) / 8, 32LL * ctx->num_sms);
+  {
+    LaunchScope ls(ctx, GRPO_KERNEL_QUANTIZE, st);
+    quantize_rows_e4m3_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(
+        static_cast<const uint2*>(x), rows, ctx->cfg.d / 4, static_cast<uint32_t*>(q), scales, fixed);
+  }
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
+}
+// ... and the vocab matrix with ONE scale (amax / 448) into the slot's W8 buffer.
+static int32_t quantize_weights(grpo_ctx* ctx, int slot, const void* W, cudaStream_t st) {
+  const grpo_config& c = ctx->cfg;
+  float* wscale = slot_ptr<float>(ctx, slot, ctx->lay.off_wscale);
+  unsigned int* amax = reinterpret_cast<unsigned int*>(wscale) + 1;
+  CU_OK(cudaMemsetAsync(amax, 0, 4, st));
+  {
+    LaunchScope ls(ctx, GRPO_KERNEL_QUANTIZE, st);
+    amax_kernel<<<8 * ctx->num_sms, 256, 0, st>>>(static_cast<const uint2*>(W), static_cast<int64_t>(c.V) * c.d / 4, amax);
+  }
+  {
+    LaunchScope ls(ctx, GRPO_KERNEL_QUANTIZE, st);
+    scale_from_amax_kernel<<<1, 1, 0, st>>>(amax, wscale);
+  }
+  CU_OK(cudaGetLastError());
+  return quantize_rows(ctx, W, c.V, slot_ptr<uint8_t>(ctx, slot, ctx->lay.off_w8), nullptr, wscale, st);
 }
 
 // ------------------------------------------------------------------------------------- API: misc
@@ -345,6 +399,8 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
     return fail(GRPO_ERR_INVALID_ARG, "gemm_cta_group must be 0 (default), 1 or 2");
   if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
     return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
+  if (cfg->fp8_logits != 0 && (cfg->stash_logits != 0 || cfg->d % 16 != 0))
+    return fail(GRPO_ERR_INVALID_ARG, "fp8_logits needs d %% 16 == 0 and is not available with stash_logits");
   if (!(cfg->logit_scale > 0.f))
     return fail(GRPO_ERR_INVALID_ARG, "logit_scale (1 / temperature) must be > 0 (got %g)", (double)cfg->logit_scale);
   if (cfg->kl_type < 0 || cfg->kl_type > 2 || (cfg->dual_clip != 0.f && !(cfg->dual_clip > 1.f)))
@@ -594,10 +650,23 @@ static int32_t a2_rows(grpo_ctx* ctx, int slot, const void* hidden, const void* 
   p.dz = stash; p.dz_pitch = L.v_pad;
   p.stash_shift = slot_ptr<float>(ctx, slot, L.off_shift); p.shift_pitch = L.n_vtiles;
   p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
-  if (stash)
+  if (c.fp8_logits && !stash) {   // FP8 study: e4m3 operands, per-token and per-tensor scales folded into the epilogue
+    if (t0 == 0) GRPO_TRY(quantize_weights(ctx, slot, W, st));        // once per call (the first row block)
+    uint8_t* h8 = slot_ptr<uint8_t>(ctx, slot, L.off_h8);
+    float* hscale = slot_ptr<float>(ctx, slot, L.off_hscale);
+    GRPO_TRY(quantize_rows(ctx, Hc, rows, h8, hscale + t0, nullptr, st));
+    CUtensorMap tmH8, tmW8;
+    GRPO_TRY(make_tmap_u8(ctx, &tmH8, h8, c.d, rows, c.d, BM));
+    GRPO_TRY(make_tmap_u8(ctx, &tmW8, slot_ptr<uint8_t>(ctx, slot, L.off_w8), c.d, c.V, c.d, BN / ctx->cg));
+    p.k_blocks = (c.d + 2 * BK - 1) / (2 * BK);
+    p.row_scale = hscale;
+    p.w_scale = slot_ptr<float>(ctx, slot, L.off_wscale);
+    GRPO_TRY((launch_gemm<false, false, EPI_LSE, 1>(ctx, GRPO_KERNEL_GEMM_LSE, tmH8, tmW8, p, p.m_tiles * p.n_split, st)));
+  } else if (stash) {
     GRPO_TRY((launch_gemm<false, false, EPI_LSE_STASH>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
-  else
+  } else {
     GRPO_TRY((launch_gemm<false, false, EPI_LSE>(ctx, GRPO_KERNEL_GEMM_LSE, tmH, tmW, p, p.m_tiles * p.n_split, st)));
+  }
   *n_split_out = p.n_split;
   return GRPO_OK;
 }
@@ -921,7 +990,21 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.dz = dz; p.dz_pitch = L.v_pad; p.dyn_rows = dyn_rows;
       p.m_alloc = compact ? static_cast<int>(L.chunk_rows) : 0;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
-      GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, GRPO_KERNEL_GEMM_DZ, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
+      if (c.fp8_logits) {   // FP8 study: the logits are recomputed from the same e4m3 operands the forward used
+        if (t0 == 0) GRPO_TRY(quantize_weights(ctx, slot, W, st));
+        uint8_t* h8 = slot_ptr<uint8_t>(ctx, slot, L.off_h8);
+        float* hscale = slot_ptr<float>(ctx, slot, L.off_hscale);
+        GRPO_TRY(quantize_rows(ctx, Hc, map_rows, h8, hscale + row_off, nullptr, st));
+        CUtensorMap tmH8, tmW8;
+        GRPO_TRY(make_tmap_u8(ctx, &tmH8, h8, c.d, map_rows, c.d, BM));
+        GRPO_TRY(make_tmap_u8(ctx, &tmW8, slot_ptr<uint8_t>(ctx, slot, L.off_w8), c.d, c.V, c.d, BN / ctx->cg));
+        p.k_blocks = (c.d + 2 * BK - 1) / (2 * BK);
+        p.row_scale = hscale;
+        p.w_scale = slot_ptr<float>(ctx, slot, L.off_wscale);
+        GRPO_TRY((launch_gemm<false, false, EPI_DZ, 1>(ctx, GRPO_KERNEL_GEMM_DZ, tmH8, tmW8, p, p.m_tiles * p.n_tiles, st)));
+      } else {
+        GRPO_TRY((launch_gemm<false, false, EPI_DZ>(ctx, GRPO_KERNEL_GEMM_DZ, tmH_k, tmW_k, p, p.m_tiles * p.n_tiles, st)));
+      }
     }
     if (dhidden_out) {  // A5: dH[rows, d] = dZ[rows, V] W[V, d], K cut into k_split fixed ranges, fp32 partials
       GemmParams p;

@@ -481,6 +481,55 @@ __global__ void __launch_bounds__(256) prenorm_bwd_kernel(const void* __restrict
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// FP8 precision study: e4m3 operands for the two logit
+// contractions (A2, A4).  Hidden rows get one scale each (amax / 448), the vocab matrix one scale for the tensor.
+__global__ void __launch_bounds__(256) amax_kernel(const uint2* __restrict__ x, int64_t n_vec,
+                                                   unsigned int* __restrict__ amax_bits) {
+  float m = 0.f;
+  for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n_vec;
+       i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+    const float4 v = bf16x4_to_float4(x[i]);
+    m = fmaxf(fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+  }
+  m = warp_max(m);
+  if ((threadIdx.x & 31) == 0) atomicMax(amax_bits, __float_as_uint(m));   // non-negative floats order like uints
+}
+__global__ void scale_from_amax_kernel(const unsigned int* __restrict__ amax_bits, float* __restrict__ scale) {
+  const float a = __uint_as_float(*amax_bits);
+  *scale = a > 0.f ? a * (1.f / 448.f) : 1.f;
+}
+// q[r,:] = e4m3(x[r,:] / s_r).  fixed_scale != nullptr: s_r = *fixed_scale for every row (per-tensor); else
+// s_r = amax_r / 448 (1 for an all-zero row), written to scale_out[r].  One warp per row.
+__global__ void __launch_bounds__(256) quantize_rows_e4m3_kernel(const uint2* __restrict__ x, int64_t R, int row_vec,
+                                                                 uint32_t* __restrict__ q, float* __restrict__ scale_out,
+                                                                 const float* __restrict__ fixed_scale) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warps = static_cast<int64_t>(gridDim.x) * (blockDim.x >> 5);
+  for (int64_t r = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5); r < R; r += warps) {
+    const uint2* row = x + r * row_vec;
+    float s;
+    if (fixed_scale != nullptr) {
+      s = *fixed_scale;
+    } else {
+      float m = 0.f;
+      for (int i = lane; i < row_vec; i += 32) {
+        const float4 v = bf16x4_to_float4(row[i]);
+        m = fmaxf(fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+      }
+      m = warp_max(m);
+      s = m > 0.f ? m * (1.f / 448.f) : 1.f;
+      if (lane == 0) scale_out[r] = s;
+    }
+    const float inv = 1.f / s;
+    uint32_t* dst = q + r * row_vec;
+    for (int i = lane; i < row_vec; i += 32) {
+      const float4 v = bf16x4_to_float4(row[i]);
+      dst[i] = pack_e4m3x2(v.x * inv, v.y * inv) | (pack_e4m3x2(v.z * inv, v.w * inv) << 16);
+    }
+  }
+}
+
 // 3-contraction variant: turn the stashed exponentials e = 2^(z2 - m) (fp16, written by the
 // EPI_LSE_STASH epilogue together with m per (row, 256-column tile) in `shift`) into
 // dZ = k_t (1[v = y_t] - e 2^(m - lse2_t)) (bf16) in place; k_t = coeff_t * coeff_mul.  HBM-bound: 2 B read + 2 B
