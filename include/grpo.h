@@ -324,6 +324,26 @@ int32_t grpo_kernel_launches(const grpo_ctx* ctx, int64_t* counts_out);
 int32_t grpo_profile_enable(grpo_ctx* ctx, int32_t on);
 int32_t grpo_profile_read_sync(grpo_ctx* ctx, double* ms_out, int64_t* launches_out);
 
+/* ---- NEXT-3: a dW accumulator stitched from per-rank shards --------------------
+ * Data parallelism over complete groups needs the sum of the ranks' dW at the update boundary.
+ * Instead of an all-reduce after the GEMM, the accumulator itself is laid out across the GPUs with CUDA virtual
+ * memory management: every rank creates ONE physical chunk on its own GPU (grpo_shard_create; *fd_out is a POSIX
+ * file descriptor to hand to the other ranks over a Unix socket, the caller closes it), imports the others'
+ * (grpo_shard_import) and maps all chunks in rank order into one contiguous device range (grpo_stitch_map: shard i
+ * at byte offset i * bytes).  That range is an ordinary `dW_accum` for grpo_fused_logprob_loss_bwd /
+ * grpo_enqueue_groups: the A6 epilogue's fp32 reduce-adds (performed at the L2 of the memory's home GPU) are carried
+ * by NVLink to the peers' shards, so the reduce-scatter happens INSIDE the contraction kernel, overlapped with its
+ * MMAs tile by tile; after a barrier rank r holds the fully reduced rows [r R, (r+1) R), R = bytes / (4 d).
+ * bytes must be a multiple of grpo_shard_granularity (2 MiB on B200: 256 rows at d = 2048) and of 4 d.
+ * All pointers HOST except the mapped range.  grpo_stitch_unmap synchronises the device.  DESIGN.md section 7. */
+typedef struct grpo_shard grpo_shard;
+int32_t grpo_shard_granularity(grpo_ctx* ctx, int64_t* bytes_out);
+int32_t grpo_shard_create(grpo_ctx* ctx, int64_t bytes, grpo_shard** shard_out, int32_t* fd_out);
+int32_t grpo_shard_import(grpo_ctx* ctx, int32_t fd, int64_t bytes, grpo_shard** shard_out);
+int32_t grpo_shard_release(grpo_ctx* ctx, grpo_shard* shard);
+int32_t grpo_stitch_map(grpo_ctx* ctx, grpo_shard* const* shards, int32_t n, void** dev_ptr_out);
+int32_t grpo_stitch_unmap(grpo_ctx* ctx, void* dev_ptr);
+
 /* Diagnostic: how many thread-block clusters of `cluster_size` CTAs of the contraction kernel (224 threads, its
  * full shared-memory ring) the device can hold at once (cudaOccupancyMaxActiveClusters).  clusters_out HOST.
  * The kernels run as 74 CTA pairs; DESIGN.md section 5 records why larger multicast clusters are not used

@@ -23,6 +23,8 @@ EXPORTS = [
     "grpo_fused_logprob_loss_fwd_bwd", "grpo_set_entropy_out", "grpo_set_seq_denom", "grpo_bwd_row_stats_sync",
     "grpo_rmsnorm_fwd", "grpo_rmsnorm_bwd", "grpo_fused_logprob_loss_bwd_prenorm", "grpo_debug_max_active_clusters",
     "grpo_vocab_shard_partials", "grpo_loss_from_partials",
+    "grpo_shard_granularity", "grpo_shard_create", "grpo_shard_import", "grpo_shard_release", "grpo_stitch_map",
+    "grpo_stitch_unmap",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
     "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
@@ -97,6 +99,12 @@ def load_library() -> C.CDLL:
     lib.grpo_bwd_tile_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     lib.grpo_set_entropy_out.argtypes = [vp, vp]
     lib.grpo_set_seq_denom.argtypes = [vp, i32]
+    lib.grpo_shard_granularity.argtypes = [vp, C.POINTER(i64)]
+    lib.grpo_shard_create.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(i32)]
+    lib.grpo_shard_import.argtypes = [vp, i32, i64, C.POINTER(vp)]
+    lib.grpo_shard_release.argtypes = [vp, vp]
+    lib.grpo_stitch_map.argtypes = [vp, C.POINTER(vp), i32, C.POINTER(vp)]
+    lib.grpo_stitch_unmap.argtypes = [vp, vp]
     lib.grpo_vocab_shard_partials.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     lib.grpo_loss_from_partials.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, i32, i64, vp, vp, vp, vp, f64, vp, vp, vp,
                                             vp, vp, vp]
@@ -457,6 +465,34 @@ class GrpoContext:
         a, t = C.c_int64(0), C.c_int64(0)
         _check(self.lib.grpo_bwd_tile_stats_sync(self.h, C.byref(a), C.byref(t)))
         return a.value, t.value
+
+    # ------------------------------------------------------------------ NEXT-3: stitched dW accumulator (CUDA VMM)
+    def grpo_shard_granularity(self) -> int:
+        g = C.c_int64(0)
+        _check(self.lib.grpo_shard_granularity(self.h, C.byref(g)))
+        return g.value
+
+    def grpo_shard_create(self, nbytes: int, export: bool = True):
+        sh, fd = C.c_void_p(), C.c_int32(-1)
+        _check(self.lib.grpo_shard_create(self.h, int(nbytes), C.byref(sh), C.byref(fd) if export else None))
+        return sh, fd.value
+
+    def grpo_shard_import(self, fd: int, nbytes: int):
+        sh = C.c_void_p()
+        _check(self.lib.grpo_shard_import(self.h, int(fd), int(nbytes), C.byref(sh)))
+        return sh
+
+    def grpo_shard_release(self, shard):
+        _check(self.lib.grpo_shard_release(self.h, shard))
+
+    def grpo_stitch_map(self, shards) -> int:
+        arr = (C.c_void_p * len(shards))(*[s.value for s in shards])
+        ptr = C.c_void_p()
+        _check(self.lib.grpo_stitch_map(self.h, arr, len(shards), C.byref(ptr)))
+        return ptr.value
+
+    def grpo_stitch_unmap(self, ptr: int):
+        _check(self.lib.grpo_stitch_unmap(self.h, C.c_void_p(ptr)))
 
     def grpo_debug_max_active_clusters(self, cluster_size: int) -> int:
         n = C.c_int32(0)

@@ -8,7 +8,7 @@ import subprocess
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libgrpo_b200.so")
-SOURCES = ["grpo_api.cu", "rollout_pipe.cpp"]
+SOURCES = ["grpo_api.cu", "rollout_pipe.cpp", "stitched_memory.cpp"]
 HEADERS = ["gemm_sm100.cuh", "ptx_sm100.cuh", "token_kernels.cuh", "cgp_queue.h",
            os.path.join("..", "..", "include", "grpo.h"), os.path.join("..", "..", "include", "rollout_pipe.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

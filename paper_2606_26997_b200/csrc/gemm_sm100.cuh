@@ -168,7 +168,7 @@ __device__ __forceinline__ int walked_k_block(const GemmParams& p, const int* kl
   constexpr int kPerTile = BM * CG / BK;
   if (p.tile_list == nullptr) return kb;
   const int t = kb / kPerTile;
-  const int tile = t < kMaxTilesSmem ? klist[t] : p.tile_list[2 + t];
+  const int tile = klist[t];                  // t < kMaxTilesSmem: grpo_create bounds bwd_chunk_tokens accordingly
   return tile * kPerTile + kb % kPerTile;
 }
 

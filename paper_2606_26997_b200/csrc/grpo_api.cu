@@ -30,6 +30,14 @@ static int32_t fail(int32_t code, const char* fmt, ...) {
   va_end(ap);
   return code;
 }
+// for the other translation units of the library (stitched_memory.cpp)
+int32_t grpo_internal_fail(int32_t code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
 #define CU_OK(expr)                                                                                   \
   do {                                                                                                \
     cudaError_t e__ = (expr);                                                                         \
@@ -399,6 +407,9 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
     return fail(GRPO_ERR_INVALID_ARG, "gemm_cta_group must be 0 (default), 1 or 2");
   if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
     return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
+  if (cfg->bwd_chunk_tokens > static_cast<int64_t>(kMaxTilesSmem) * BM)
+    return fail(GRPO_ERR_INVALID_ARG, "bwd_chunk_tokens must be <= %d (the A6 producer keeps the chunk's active-tile list "
+                "in shared memory)", kMaxTilesSmem * BM);
   if (cfg->fp8_logits != 0 && (cfg->stash_logits != 0 || cfg->d % 16 != 0))
     return fail(GRPO_ERR_INVALID_ARG, "fp8_logits needs d %% 16 == 0 and is not available with stash_logits");
   if (!(cfg->logit_scale > 0.f))

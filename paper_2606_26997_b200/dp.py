@@ -16,6 +16,11 @@ one GPU (none is reachable from this build); DESIGN.md section 7 says so.
 """
 from __future__ import annotations
 
+import math
+import os
+import socket
+import threading
+import uuid
 from dataclasses import dataclass, field
 from typing import List, Optional, Sequence
 
@@ -111,3 +116,97 @@ class GrpoDataParallel:
             for t in tensors:
                 h.works.append(dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.pg, async_op=True))
         return h
+
+
+# ---------------------------------------------------------------------- fused GEMM -> reduce-scatter (stitched dW)
+class _RawCudaBuffer:
+    """A raw device range exposed through __cuda_array_interface__ so that torch can alias it."""
+
+    def __init__(self, ptr: int, n_float32: int):
+        self.__cuda_array_interface__ = {"shape": (n_float32,), "typestr": "<f4", "data": (ptr, False), "version": 2}
+
+
+def _exchange_fds(own_fd: int, dp: "GrpoDataParallel") -> List[int]:
+    """Every rank's exported shard descriptor, by rank (own at dp.rank).  POSIX file descriptors only cross process
+    boundaries as SCM_RIGHTS ancillary data: every rank serves its descriptor on a Unix socket, then fetches the
+    others'."""
+    if dp.world == 1:
+        return [own_fd]
+    tag = [uuid.uuid4().hex if dp.rank == 0 else None]
+    dist.broadcast_object_list(tag, src=0, group=dp.pg)
+    path = lambda r: f"/tmp/grpo_stitch_{tag[0]}_{r}.sock"
+    srv = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+    srv.bind(path(dp.rank))
+    srv.listen(dp.world)
+
+    def serve():
+        for _ in range(dp.world - 1):
+            conn, _ = srv.accept()
+            socket.send_fds(conn, [b"fd"], [own_fd])
+            conn.close()
+
+    th = threading.Thread(target=serve, daemon=True)
+    th.start()
+    dist.barrier(group=dp.pg)                      # every socket is listening
+    fds = []
+    for r in range(dp.world):
+        if r == dp.rank:
+            fds.append(own_fd)
+            continue
+        c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+        c.connect(path(r))
+        _, got, _, _ = socket.recv_fds(c, 16, 1)
+        c.close()
+        fds.append(got[0])
+    th.join()
+    srv.close()
+    os.unlink(path(dp.rank))
+    return fds
+
+
+class StitchedGradient:
+    """fp32 [V, d] gradient accumulator whose row range r R .. (r+1) R physically lives on rank r's GPU
+    (include/grpo.h: grpo_shard_* / grpo_stitch_*).  Passed as ``dW_accum`` it makes the A6 epilogue's reduce-adds
+    the data-parallel reduce-scatter: no collective follows the GEMM.  ``full`` is the [V, d] view every rank
+    accumulates into, ``local`` the rank's own (fully reduced after ``barrier()``) rows, ``local_rows`` their range.
+
+    n_local_shards > 0 builds the same layout from that many chunks of THIS process's GPU (one-GPU emulation)."""
+
+    def __init__(self, ctx, V: int, d: int, dp: Optional[GrpoDataParallel] = None, n_local_shards: int = 0):
+        self.ctx, self.dp = ctx, dp
+        n = n_local_shards if n_local_shards > 0 else (dp.world if dp else 1)
+        rank = 0 if n_local_shards > 0 or dp is None else dp.rank
+        gran, row_bytes = ctx.grpo_shard_granularity(), 4 * d
+        unit = gran * row_bytes // math.gcd(gran, row_bytes) // row_bytes      # rows per shard come in these units
+        self.rows_per_shard = -(-(-(-V // n)) // unit) * unit
+        nbytes = self.rows_per_shard * row_bytes
+        if n_local_shards > 0:
+            self._shards = [ctx.grpo_shard_create(nbytes, export=False)[0] for _ in range(n)]
+        else:
+            own, fd = ctx.grpo_shard_create(nbytes)
+            fds = _exchange_fds(fd, dp) if dp else [fd]
+            self._shards = [own if r == rank else ctx.grpo_shard_import(fds[r], nbytes) for r in range(n)]
+            for f in set(fds):
+                os.close(f)
+        self._ptr = ctx.grpo_stitch_map(self._shards)
+        flat = torch.as_tensor(_RawCudaBuffer(self._ptr, n * self.rows_per_shard * d), device="cuda")
+        self._all = flat.view(n * self.rows_per_shard, d)
+        self.full = self._all[:V]
+        self.local_rows = (rank * self.rows_per_shard, min(V, (rank + 1) * self.rows_per_shard))
+        self.local = self._all[rank * self.rows_per_shard:(rank + 1) * self.rows_per_shard]
+        self.local.zero_() if n_local_shards == 0 else self._all.zero_()
+        self.barrier()
+
+    def barrier(self):
+        """All ranks' launches into the accumulator have completed (device + host barrier)."""
+        torch.cuda.synchronize()
+        if self.dp is not None and self.dp.world > 1:
+            dist.barrier(group=self.dp.pg)
+
+    def close(self):
+        if getattr(self, "_ptr", None):
+            self.full = self.local = self._all = None
+            self.ctx.grpo_stitch_unmap(self._ptr)
+            for s in self._shards:
+                self.ctx.grpo_shard_release(s)
+            self._ptr = None
