@@ -385,8 +385,7 @@ def run_ours(args):
 
     # ---- the same K steps once more with a CUDA event pair around every kernel launch (recorded by the library on
     # the launch stream): per-kernel times for the roofline; the pass's own total is reported beside the headline
-    ctx.grpo_bwd_tile_stats_sync()          # clear
-    ctx.grpo_bwd_row_stats_sync()
+    ctx.grpo_bwd_row_stats_sync()           # clear
     ctx.grpo_profile_enable(True)
     p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -400,13 +399,8 @@ def run_ours(args):
     prof = ctx.grpo_profile_read_sync()
     ctx.grpo_profile_enable(False)
     rows_walked, rows_total = ctx.grpo_bwd_row_stats_sync()
-    tiles_walked, tiles_total = ctx.grpo_bwd_tile_stats_sync()
-    if args.stash:
-        args.bwd_active_frac = tiles_walked / tiles_total if tiles_total > 0 else 1.0
-    else:
-        args.bwd_active_frac = rows_walked / rows_total if rows_total > 0 else 1.0
-    args.bwd_rows = {"walked": rows_walked, "total": rows_total, "tiles_walked_stash": tiles_walked,
-                     "tiles_total_stash": tiles_total}
+    args.bwd_active_frac = rows_walked / rows_total if rows_total > 0 else 1.0
+    args.bwd_rows = {"walked": rows_walked, "total": rows_total}
 
     # ---- energy: NVML's board energy counter around a >= 2 s run of the same step (the counter is too coarse
     # for the 0.35 s headline region); joules per step, mean power, tokens per joule

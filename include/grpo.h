@@ -81,8 +81,7 @@ typedef struct {
                                 tokens, and zero-variance groups): the remaining rows are compacted
                                 on the device and A4-A6 run on the compact panel; skipped dHidden rows are
                                 written as zeros and add nothing to dW, which is what the dense computation
-                                gives.  The 3-contraction variant skips per 256-row token
-                                tile instead.  Decided on the device; no host synchronisation. */
+                                gives.  Decided on the device; no host synchronisation. */
   int32_t stash_logits;      /* 0 = default: grpo_enqueue_groups / grpo_step_host run forward then backward with
                                 the logits RECOMPUTED chunk by chunk (north_star, 4 contractions); 1 = they run
                                 grpo_fused_logprob_loss_fwd_bwd instead (3 contractions) */
@@ -296,7 +295,7 @@ enum {
   GRPO_KERNEL_GEMM_DH = 5,     /* A5: dH = dZ W */
   GRPO_KERNEL_GEMM_DW = 6,     /* A6: dW += dZ^T H */
   GRPO_KERNEL_DEBUG = 7,       /* grpo_debug_gemm */
-  GRPO_KERNEL_TILE_SCAN = 8,   /* backward: zero-coefficient tile scan + zero fill of skipped dHidden rows */
+  GRPO_KERNEL_RESERVED_8 = 8,  /* (round 1's per-tile zero scan; replaced by GRPO_KERNEL_COMPACT) */
   GRPO_KERNEL_STASH_DZ = 9,    /* 3-contraction variant: stashed logits -> dZ in place */
   GRPO_KERNEL_COMPACT = 10,    /* backward: zero-coefficient row compaction, gather of active rows, zero fill */
   GRPO_KERNEL_DH_REDUCE = 11,  /* A5: fixed-order sum of the split-K partials (+ scatter of compacted rows; + the
@@ -306,11 +305,7 @@ enum {
   GRPO_NUM_KERNEL_KINDS = 14
 };
 
-/* Token tiles the 3-contraction backward calls of workspace slot 0 walked (active) and saw (total) since the last
- * call of this function; both 0 when bwd_skip_zero_tiles is off.  Synchronises. */
-int32_t grpo_bwd_tile_stats_sync(grpo_ctx* ctx, int64_t* active_out /*HOST*/, int64_t* total_out /*HOST*/);
-
-/* Packed rows the north_star backward calls of all workspace slots ran A4-A6 over (active: coeff != 0) and saw
+/* Packed rows the backward calls of all workspace slots ran their contractions over (active: coeff != 0) and saw
  * (total) since the last call of this function; both 0 when bwd_skip_zero_tiles is off.  Synchronises. */
 int32_t grpo_bwd_row_stats_sync(grpo_ctx* ctx, int64_t* active_out /*HOST*/, int64_t* total_out /*HOST*/);
 

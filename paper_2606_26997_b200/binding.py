@@ -27,9 +27,9 @@ EXPORTS = [
     "grpo_stitch_unmap",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
     "grpo_check_errors_sync", "grpo_step_host", "grpo_debug_gemm", "grpo_kernel_launches",
-    "grpo_profile_enable", "grpo_profile_read_sync", "grpo_bwd_tile_stats_sync",
+    "grpo_profile_enable", "grpo_profile_read_sync",
 ]
-KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "tile_scan", "stash_dz",
+KERNEL_KINDS = ["advantage", "token_count", "gemm_lse", "loss", "gemm_dz", "gemm_dh", "gemm_dw", "debug", "reserved_8", "stash_dz",
                 "compact", "dh_reduce", "rmsnorm", "quantize"]
 
 
@@ -96,7 +96,6 @@ def load_library() -> C.CDLL:
     lib.grpo_kernel_launches.argtypes = [vp, C.POINTER(i64)]
     lib.grpo_profile_enable.argtypes = [vp, i32]
     lib.grpo_profile_read_sync.argtypes = [vp, C.POINTER(f64), C.POINTER(i64)]
-    lib.grpo_bwd_tile_stats_sync.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     lib.grpo_set_entropy_out.argtypes = [vp, vp]
     lib.grpo_set_seq_denom.argtypes = [vp, i32]
     lib.grpo_shard_granularity.argtypes = [vp, C.POINTER(i64)]
@@ -459,11 +458,6 @@ class GrpoContext:
     def grpo_bwd_row_stats_sync(self):
         a, t = C.c_int64(0), C.c_int64(0)
         _check(self.lib.grpo_bwd_row_stats_sync(self.h, C.byref(a), C.byref(t)))
-        return a.value, t.value
-
-    def grpo_bwd_tile_stats_sync(self):
-        a, t = C.c_int64(0), C.c_int64(0)
-        _check(self.lib.grpo_bwd_tile_stats_sync(self.h, C.byref(a), C.byref(t)))
         return a.value, t.value
 
     # ------------------------------------------------------------------ NEXT-3: stitched dW accumulator (CUDA VMM)

@@ -11,7 +11,7 @@
 // the highest warp ids of their scheduler partitions, so the arbiter never parks them behind an epilogue warp.
 //
 // Shared memory: ring stages | 16 KB staging for the A6 epilogue (one 32 x 32 fp32 block per epilogue warp,
-// reduced into dW by a TMA reduce-add) | barriers + the A6 producer's copy of the active-tile list.
+// reduced into dW by a TMA reduce-add) | barriers.
 //
 // CG = 1: one CTA per SM, C tile = 128 x 256, K block = 64 bf16 (one 128-byte swizzle row), 4-stage
 //         smem ring of 48 KB stages.
@@ -40,14 +40,12 @@ constexpr int kGemmThreads = 224;
 constexpr int kProducerWarp = 4, kMmaWarp = 5, kGateWarp = 6;
 constexpr int kTmemCols = 512;
 constexpr int kRedStageBytes = 4 * 32 * 32 * 4;   // A6 epilogue: one 32 x 32 fp32 block per epilogue warp (16 KB)
-constexpr int kMaxTilesSmem = 1024;         // active-tile indices the A6 producer keeps in shared memory
 template <int CG> struct GemmShape {
   static constexpr int kBRows = BN / CG;                       // B rows (N index) staged by one CTA
   static constexpr int kBBytes = kBRows * BK * 2;              // 32 KB / 16 KB
   static constexpr int kStageBytes = kABytes + kBBytes;        // 48 KB / 32 KB
   static constexpr int kStages = CG == 1 ? 4 : 6;
-  static constexpr int kSmemBytes = kStages * kStageBytes + kRedStageBytes + 1024 /*align slack*/ + 256 /*barriers*/ +
-                                    kMaxTilesSmem * 4 /*A6 tile list*/;
+  static constexpr int kSmemBytes = kStages * kStageBytes + kRedStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
 };
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -108,11 +106,6 @@ struct GemmParams {
   void* c_out;
   int64_t c_pitch;                   // elements
   int c_fp32;
-  // zero-coefficient tile skipping (A4-A6): device list written by
-  // active_tiles_kernel: [0] = number of active token tiles, [1] = tiles in the chunk, [2 ..] = their
-  // indices (ascending).  nullptr: every tile is active.  A4/A5 walk only active m tiles; A6 walks only the
-  // k blocks (token rows) of active tiles.
-  const int* tile_list;
   // drift bound between the CTA pairs of one launch (see the producer loop); sync == nullptr: off
   unsigned int* sync;
   int sync_epoch_kb;                 // k blocks per epoch
@@ -127,10 +120,9 @@ struct alignas(8) GemmBarriers {
   uint64_t tmem_empty[2];
   uint32_t tmem_base;
   int gate_open;                     // highest epoch the producer may enter (written by the gate warp)
-  int klist[kMaxTilesSmem];          // A6: active token tiles of the chunk, staged by the producer warp
 };
 
-// Effective extent of a launch under tile skipping / row compaction: the rows of C that exist, the number of m
+// Effective extent of a launch under row compaction: the rows of C that exist, the number of m
 // tiles walked (A4/A5), the k blocks per unit (A6) and the unit count.  Uniform over the grid (one global load).
 struct Extent { int m_total, m_tiles, k_blocks, n_units; };
 template <int CG, int EPI>
@@ -148,30 +140,9 @@ __device__ __forceinline__ Extent launch_extent(const GemmParams& p, int n_units
       e.m_tiles = min(p.m_tiles, (e.m_total + BM * CG - 1) / (BM * CG));
       e.n_units = e.m_tiles * p.n_tiles * ks;
     }
-  } else if (p.tile_list != nullptr) {
-    const int n_active = p.tile_list[0];
-    if constexpr (EPI == EPI_RED_F32) {
-      e.k_blocks = min(p.k_blocks, n_active * (BM * CG / BK));
-      if (e.k_blocks == 0) e.n_units = 0;
-    } else {
-      e.m_tiles = n_active;
-      e.n_units = n_active * p.n_tiles * ks;
-    }
   }
   return e;
 }
-// k block (in units of BK token rows) the kb-th walked k block of A6 maps to.  `klist` is the shared-memory
-// copy of the active-tile list (a global load per k block on the producer's critical path costs more than
-// the k block's MMAs take).
-template <int CG>
-__device__ __forceinline__ int walked_k_block(const GemmParams& p, const int* klist, int kb) {
-  constexpr int kPerTile = BM * CG / BK;
-  if (p.tile_list == nullptr) return kb;
-  const int t = kb / kPerTile;
-  const int tile = klist[t];                  // t < kMaxTilesSmem: grpo_create bounds bwd_chunk_tokens accordingly
-  return tile * kPerTile + kb % kPerTile;
-}
-
 // One scheduling unit: output tile(s) [m_tile] x [n0, n1) reduced over k blocks [kb0, kb1); `part` is the vocab
 // split (EPI_LSE) or the K split (split-K stores) the unit belongs to.
 struct Unit { int m_tile, n0, n1, kb0, kb1, part; };
@@ -207,7 +178,7 @@ __device__ __forceinline__ Unit unit_to_tiles(const GemmParams& p, const Extent&
     t.n0 = u / e.m_tiles;
   }
   t.n1 = t.n0 + 1;
-  t.m_tile = (EPI != EPI_RED_F32 && p.tile_list != nullptr && p.dyn_rows == nullptr) ? p.tile_list[2 + m_idx] : m_idx;
+  t.m_tile = m_idx;
   return t;
 }
 
@@ -289,13 +260,6 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     // address and coordinate is then warp-uniform and lives in uniform registers (a lane-0-only loop costs
     // an ELECT + four R2UR.BROADCAST per TMA instruction, which made this thread the bottleneck of A6).
     {
-      if constexpr (EPI == EPI_RED_F32) {
-        if (p.tile_list != nullptr) {
-          const int n_act = min(p.tile_list[0], kMaxTilesSmem);
-          for (int i = lane; i < n_act; i += 32) bars->klist[i] = p.tile_list[2 + i];
-          __syncwarp();
-        }
-      }
       const bool leader_lane = elect_one();
       const uint32_t full0 = CG == 2 ? mapa_cluster(smem_u32(&bars->full[0]), 0) : smem_u32(&bars->full[0]);
       int stage = 0;
@@ -308,7 +272,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         for (int n_tile = un.n0; n_tile < un.n1; ++n_tile) {
           const int b_row = n_tile * BN + static_cast<int>(cta_rank) * kBRows;
           for (int kbw = un.kb0; kbw < un.kb1; ++kbw) {
-            const int kb = EPI == EPI_RED_F32 ? walked_k_block<CG>(p, bars->klist, kbw) : kbw;
+            const int kb = kbw;
             if (sync_on && --to_epoch == 0) {
               to_epoch = p.sync_epoch_kb;
               if (leader_lane) red_add_u32(p.sync + epoch, 1u);

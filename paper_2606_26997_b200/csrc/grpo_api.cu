@@ -67,8 +67,7 @@ struct SlotLayout {
   int64_t off_part_m = 0, off_part_s = 0, off_zy = 0, off_total = 0, off_seq_count = 0, off_dz = 0;
   int64_t off_hidden = 0, off_targets = 0, off_old = 0, off_ref = 0, off_mask = 0, off_rewards = 0, off_adv = 0,
           off_cu_seq = 0, off_cu_grp = 0, off_logp = 0, off_lse = 0, off_coeff = 0, off_dh = 0, off_sync = 0,
-          off_tiles = 0, off_tile_stats = 0;
-  int64_t tile_cap = 0;   // token tiles per backward chunk
+          off_dz2 = 0;
   // token-granular compaction + split-K of A5
   int64_t off_row_idx = 0, off_meta = 0, off_hc = 0, off_yc = 0, off_lsec = 0, off_coeffc = 0, off_dh_part = 0,
           off_row_stats = 0;
@@ -209,12 +208,10 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.off_coeff = take(max_T * 4);
   L.off_dh = take(max_T * c.d * (c.dhidden_fp32 ? 4 : 2));
   L.off_sync = take(kSyncCap * 4);
-  L.tile_cap = L.chunk_rows / BM + 1;
-  L.off_tiles = take((2 + 2 * L.tile_cap) * 4);
-  L.off_tile_stats = take(16);
+  L.off_dz2 = take(L.chunk_rows * L.v_pad * 2);   // 3-contraction variant: compacted dZ rows of a chunk
   L.n_chunks_max = (max_T + L.chunk_rows - 1) / L.chunk_rows + 1;
   L.off_row_idx = take(max_T * 4);
-  L.off_meta = take((2 + L.n_chunks_max) * 4);
+  L.off_meta = take(4 * (L.n_chunks_max + 1) * 4);
   L.off_hc = take(L.chunk_rows * c.d * 2);
   L.off_yc = take(L.chunk_rows * 4);
   L.off_lsec = take(L.chunk_rows * 4);
@@ -407,9 +404,6 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
     return fail(GRPO_ERR_INVALID_ARG, "gemm_cta_group must be 0 (default), 1 or 2");
   if (cfg->groups_per_update < 1 || cfg->std_ddof < 0 || cfg->std_ddof > 1 || cfg->loss_agg < 0 || cfg->loss_agg > 1)
     return fail(GRPO_ERR_INVALID_ARG, "bad groups_per_update / std_ddof / loss_agg");
-  if (cfg->bwd_chunk_tokens > static_cast<int64_t>(kMaxTilesSmem) * BM)
-    return fail(GRPO_ERR_INVALID_ARG, "bwd_chunk_tokens must be <= %d (the A6 producer keeps the chunk's active-tile list "
-                "in shared memory)", kMaxTilesSmem * BM);
   if (cfg->fp8_logits != 0 && (cfg->stash_logits != 0 || cfg->d % 16 != 0))
     return fail(GRPO_ERR_INVALID_ARG, "fp8_logits needs d %% 16 == 0 and is not available with stash_logits");
   if (!(cfg->logit_scale > 0.f))
@@ -482,7 +476,6 @@ extern "C" int32_t grpo_set_workspace(grpo_ctx* ctx, void* dev_ptr, int64_t byte
   ctx->n_slots = n_slots;
   ctx->lay = L;
   for (int i = 0; i < n_slots; ++i) {
-    CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_tile_stats), 0, 16));
     CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_row_stats), 0, 16));
   }
   // pinned ring for run_launch's index arrays: cu_seqlens [S+1] + cu_groups [S+1] per entry
@@ -532,20 +525,6 @@ extern "C" int32_t grpo_profile_read_sync(grpo_ctx* ctx, double* ms_out, int64_t
     launches_out[r.kind]++;
   }
   prof_clear(ctx);
-  return GRPO_OK;
-}
-
-extern "C" int32_t grpo_bwd_tile_stats_sync(grpo_ctx* ctx, int64_t* active_out, int64_t* total_out) {
-  if (!ctx || !active_out || !total_out) return fail(GRPO_ERR_INVALID_ARG, "NULL pointer");
-  *active_out = *total_out = 0;
-  if (!ctx->ws) return GRPO_OK;
-  int h[2] = {0, 0};
-  int* stats = slot_ptr<int>(ctx, 0, ctx->lay.off_tile_stats);
-  CU_OK(cudaDeviceSynchronize());
-  CU_OK(cudaMemcpy(h, stats, 8, cudaMemcpyDeviceToHost));
-  CU_OK(cudaMemset(stats, 0, 8));
-  *active_out = h[0];
-  *total_out = h[1];
   return GRPO_OK;
 }
 
@@ -858,7 +837,8 @@ struct HostPipe {
 //     (compact_rows_kernel), each backward chunk gathers its active hidden rows into a dense panel, A4 - A6 run
 //     on that panel with the row count read from device memory, and the split-K reduction of A5 scatters the
 //     dHidden rows back; rows with coeff == 0 are written as zeros.  Nothing is decided on the host.
-//   3-contraction variant: per 256-row token tile (the chunk's logits are stashed before its coefficients exist).
+//   3-contraction variant: the same per chunk (a chunk's logits are stashed before its coefficients exist): the
+//     conversion pass writes the dZ rows of the chunk's active tokens, compacted, into a second chunk buffer.
 // RMSNorm in front of the path: when given, the A5 reduction turns each dHidden row into
 // dx (written to `dhidden_out`, which is then the dx buffer) and adds its share of dgamma.
 struct PrenormArgs { const void* x; const void* gamma; const float* rstd; float* dgamma; };
@@ -897,14 +877,14 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
   if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
   if (T > ctx->ws_max_T) return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds workspace max_T=%lld", (long long)T, (long long)ctx->ws_max_T);
   if (!dhidden_out && !dW_accum && !fused) return GRPO_OK;
+  if (pn && fused) return fail(GRPO_ERR_INVALID_ARG, "the pre-norm backward is not available for the stash variant");
   const SlotLayout& L = ctx->lay;
   __nv_bfloat16* dz = slot_ptr<__nv_bfloat16>(ctx, slot, L.off_dz);
   const int64_t rows_per_chunk = rows_per_chunk_for(ctx, T);
   const int n_chunks = static_cast<int>((T + rows_per_chunk - 1) / rows_per_chunk);
   const uint8_t* Hb = static_cast<const uint8_t*>(hidden);
   const int dh_elem = c.dhidden_fp32 ? 4 : 2;
-  const bool skip = c.bwd_skip_zero_tiles >= 0;
-  const bool compact = skip && !fused;
+  const bool compact = c.bwd_skip_zero_tiles >= 0;
   const int TM = BM * ctx->cg;
   int k_split, kb_per_split;
   dh_ksplit(c.V, &k_split, &kb_per_split);
@@ -916,22 +896,28 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
 
   int* row_idx = slot_ptr<int>(ctx, slot, L.off_row_idx);
   int* meta = slot_ptr<int>(ctx, slot, L.off_meta);
-  if (compact) {
-    if (n_chunks > L.n_chunks_max) return fail(GRPO_ERR_WORKSPACE, "too many backward chunks for the workspace");
+  long long* row_stats = slot_ptr<long long>(ctx, slot, L.off_row_stats);
+  if (compact && n_chunks > L.n_chunks_max) return fail(GRPO_ERR_WORKSPACE, "too many backward chunks for the workspace");
+  // Row compaction.  north_star path: once for the call (the forward has produced every coefficient), so that every
+  // chunk but the last is full.  3-contraction variant: per chunk, after the chunk's forward.
+  auto compact_rows = [&](const float* cf, int64_t n_rows, int64_t chunk_rows, int chunks, int* idx, int* m,
+                          uint8_t* dh_rows) -> int32_t {
     {
       LaunchScope ls(ctx, GRPO_KERNEL_COMPACT, st);
-      compact_rows_kernel<<<1, 1024, 0, st>>>(coeff, static_cast<int>(T), static_cast<int>(rows_per_chunk), n_chunks,
-                                              row_idx, meta, slot_ptr<long long>(ctx, slot, L.off_row_stats));
+      compact_rows_kernel<<<1, 1024, 0, st>>>(cf, static_cast<int>(n_rows), static_cast<int>(chunk_rows), chunks, idx, m,
+                                              row_stats);
     }
     CU_OK(cudaGetLastError());
-    if (dhidden_out) {
+    if (dh_rows) {
       LaunchScope ls(ctx, GRPO_KERNEL_COMPACT, st);
-      zero_coeff_rows_kernel<<<static_cast<unsigned>(T), 128, 0, st>>>(coeff, static_cast<int>(T),
-                                                                      static_cast<uint8_t*>(dhidden_out),
-                                                                      static_cast<int64_t>(c.d) * dh_elem);
+      zero_coeff_rows_kernel<<<static_cast<unsigned>(n_rows), 128, 0, st>>>(cf, static_cast<int>(n_rows), dh_rows,
+                                                                           static_cast<int64_t>(c.d) * dh_elem);
       CU_OK(cudaGetLastError());
     }
-  }
+    return GRPO_OK;
+  };
+  if (compact && !fused)
+    GRPO_TRY(compact_rows(coeff, T, rows_per_chunk, n_chunks, row_idx, meta, static_cast<uint8_t*>(dhidden_out)));
 
   for (int64_t t0 = 0; t0 < T; t0 += rows_per_chunk) {
     const int64_t rows = std::min<int64_t>(rows_per_chunk, T - t0);       // static upper bound of the chunk's rows
@@ -940,53 +926,45 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
     // compact: the chunk's operands live in dense panels of the workspace whose tails are zero-filled explicitly
     // (the row count is only known on the device); otherwise the tensor maps end at `rows` and TMA zero-fills.
     const int64_t map_rows = compact ? align_up(rows, 256) : rows;
-    const int* dyn_rows = compact ? meta + 2 + chunk_idx : nullptr;
+    // row_idx entries of this chunk: absolute packed rows (north_star) or chunk-local rows (3-contraction variant)
+    int* idx_c = row_idx + t0;
+    const int* dyn_rows = !compact ? nullptr : (fused ? meta + 4 * chunk_idx + 2 : meta + 2 + chunk_idx);
     const void* Hc = compact ? static_cast<const void*>(slot_ptr<uint8_t>(ctx, slot, L.off_hc))
                              : static_cast<const void*>(Hb + t0 * c.d * 2);
     const int32_t* y_c = compact ? slot_ptr<int32_t>(ctx, slot, L.off_yc) : targets;
     const float* lse_c = compact ? slot_ptr<float>(ctx, slot, L.off_lsec) : lse;
     const float* coeff_c = compact ? slot_ptr<float>(ctx, slot, L.off_coeffc) : coeff;
     const int64_t row_off = compact ? 0 : t0;
+    // where the dZ rows A5 / A6 contract live: the chunk buffer, or (compacted 3-contraction variant) the second one
+    __nv_bfloat16* dz_rows = (fused && compact) ? slot_ptr<__nv_bfloat16>(ctx, slot, L.off_dz2) : dz;
+    uint8_t* dh_chunk = dhidden_out ? static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem : nullptr;
 
     if (fused) {
       if (pipe && chunk_idx < pipe->in.size()) CU_OK(cudaStreamWaitEvent(st, pipe->in[chunk_idx], 0));
       GRPO_TRY(fwd_rows(ctx, slot, hidden, W, targets, *fused, T, t0, rows, dz, st));
     }
     if (!dhidden_out && !dW_accum) continue;
+    if (fused && compact)
+      GRPO_TRY(compact_rows(coeff + t0, rows, rows, 1, idx_c, meta + 4 * chunk_idx, dh_chunk));
 
-    const int* tile_list = nullptr;
     if (compact) {
       LaunchScope ls(ctx, GRPO_KERNEL_COMPACT, st);
       gather_rows_kernel<<<static_cast<unsigned>(map_rows), 128, 0, st>>>(
-          reinterpret_cast<const uint4*>(hidden), c.d / 8, row_idx + t0, dyn_rows, 256, static_cast<int>(L.chunk_rows),
-          targets, lse, coeff, slot_ptr<uint4>(ctx, slot, L.off_hc), slot_ptr<int32_t>(ctx, slot, L.off_yc),
+          reinterpret_cast<const uint4*>(fused ? Hb + t0 * c.d * 2 : Hb), c.d / 8, idx_c, dyn_rows, 256,
+          static_cast<int>(L.chunk_rows), fused ? targets + t0 : targets, fused ? lse + t0 : lse, fused ? coeff + t0 : coeff,
+          slot_ptr<uint4>(ctx, slot, L.off_hc), slot_ptr<int32_t>(ctx, slot, L.off_yc),
           slot_ptr<float>(ctx, slot, L.off_lsec), slot_ptr<float>(ctx, slot, L.off_coeffc));
       CU_OK(cudaGetLastError());
-    } else if (skip) {   // 3-contraction variant: scan this chunk's coefficients per token tile
-      int* list = slot_ptr<int>(ctx, slot, L.off_tiles);
-      {
-        LaunchScope ls(ctx, GRPO_KERNEL_TILE_SCAN, st);
-        active_tiles_kernel<<<1, 1024, 0, st>>>(coeff + t0, static_cast<int>(rows), TM, static_cast<int>(L.tile_cap), list,
-                                                slot_ptr<int>(ctx, slot, L.off_tile_stats));
-      }
-      CU_OK(cudaGetLastError());
-      if (dhidden_out) {
-        LaunchScope ls(ctx, GRPO_KERNEL_TILE_SCAN, st);
-        zero_inactive_rows_kernel<<<m_tiles, 256, 0, st>>>(static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem,
-                                                           static_cast<int64_t>(c.d) * dh_elem, static_cast<int>(rows), TM,
-                                                           list + 2 + L.tile_cap);
-        CU_OK(cudaGetLastError());
-      }
-      tile_list = list;
     }
 
     CUtensorMap tmH_k, tmH_mn, tmDZ_k, tmDZ_mn;
-    GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz, c.V, map_rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
-    if (fused) {  // stashed logits -> dZ in place (HBM-bound elementwise pass instead of the A4 contraction)
+    GRPO_TRY(make_tmap(ctx, &tmDZ_k, dz_rows, c.V, map_rows, static_cast<uint64_t>(L.v_pad) * 2, BK, BM));
+    if (fused) {  // stashed softmax numerators -> dZ (HBM-bound elementwise pass instead of the A4 contraction)
       LaunchScope ls(ctx, GRPO_KERNEL_STASH_DZ, st);
-      stash_to_dz_kernel<<<static_cast<unsigned>(rows), 256, 0, st>>>(
-          reinterpret_cast<uint16_t*>(dz), static_cast<int>(rows), c.V, L.v_pad, slot_ptr<float>(ctx, slot, L.off_shift),
-          L.n_vtiles, BN, targets + t0, lse + t0, coeff + t0, c.logit_scale * grad_scale, tile_list, TM);
+      stash_to_dz_kernel<<<static_cast<unsigned>(map_rows), 256, 0, st>>>(
+          reinterpret_cast<const uint16_t*>(dz), reinterpret_cast<uint16_t*>(dz_rows), static_cast<int>(rows), c.V, L.v_pad,
+          slot_ptr<float>(ctx, slot, L.off_shift), L.n_vtiles, BN, targets + t0, lse + t0, coeff + t0,
+          c.logit_scale * grad_scale, compact ? idx_c : nullptr, dyn_rows, 256, static_cast<int>(L.chunk_rows));
       CU_OK(cudaGetLastError());
     } else {  // A4: recompute logits, dZ = coeff (1[v=y] - p) * logit_scale * grad_scale  -> bf16 chunk
       GRPO_TRY(make_tmap(ctx, &tmH_k, Hc, c.d, map_rows, static_cast<uint64_t>(c.d) * 2, BK, BM));
@@ -1025,21 +1003,21 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.n_fastest = 1;
       p.k_split = k_split; p.kb_per_split = kb_per_split; p.c_split_stride = L.chunk_rows * c.d;
       p.c_out = dh_part; p.c_pitch = c.d; p.c_fp32 = 1;
-      p.tile_list = tile_list; p.dyn_rows = dyn_rows;
+      p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p,
                                                     p.m_tiles * p.n_tiles * k_split, st)));
+      // the reduction scatters compacted row r to packed row idx_c[r]: absolute for the north_star path (base = the
+      // call's dHidden), chunk-local for the 3-contraction variant (base = the chunk's rows)
+      void* scatter_base = (compact && !fused) ? dhidden_out : static_cast<void*>(dh_chunk);
       if (pn) {  // ... -> dx, dgamma (RMSNorm backward fused behind the reduction; dHidden is never written)
-        if (tile_list) return fail(GRPO_ERR_INVALID_ARG, "the pre-norm backward is not available for the stash variant");
         GRPO_TRY(launch_prenorm_bwd(ctx, false, dh_part, k_split, L.chunk_rows * c.d / 4, static_cast<int>(rows), dyn_rows,
-                                    compact ? row_idx + t0 : nullptr, t0, *pn, dhidden_out, st));
+                                    compact ? idx_c : nullptr, t0, *pn, dhidden_out, st));
       } else {  // fixed-order sum of the partials (+ scatter of compacted rows) -> dHidden
         LaunchScope ls(ctx, GRPO_KERNEL_DH_REDUCE, st);
         splitk_reduce_kernel<<<static_cast<unsigned>(rows), 128, 0, st>>>(
             reinterpret_cast<const float4*>(dh_part), k_split, L.chunk_rows * c.d / 4, c.d / 4, static_cast<int>(rows),
-            dyn_rows, compact ? row_idx + t0 : nullptr, tile_list ? tile_list + 2 + L.tile_cap : nullptr, TM,
-            compact ? dhidden_out : static_cast<void*>(static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem),
-            c.dhidden_fp32);
+            dyn_rows, compact ? idx_c : nullptr, scatter_base, c.dhidden_fp32);
       }
       CU_OK(cudaGetLastError());
       if (pipe && pipe->dh_host && chunk_idx < pipe->out.size()) {
@@ -1047,12 +1025,12 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
         // t0 + rows has a compact index below it as well, and rows with a zero coefficient were written first
         CU_OK(cudaEventRecord(pipe->out[chunk_idx], st));
         CU_OK(cudaStreamWaitEvent(pipe->cs, pipe->out[chunk_idx], 0));
-        CU_OK(cudaMemcpyAsync(pipe->dh_host + t0 * c.d * dh_elem, static_cast<uint8_t*>(dhidden_out) + t0 * c.d * dh_elem,
-                              rows * c.d * dh_elem, cudaMemcpyDeviceToHost, pipe->cs));
+        CU_OK(cudaMemcpyAsync(pipe->dh_host + t0 * c.d * dh_elem, dh_chunk, rows * c.d * dh_elem, cudaMemcpyDeviceToHost,
+                              pipe->cs));
       }
     }
     if (dW_accum) {  // A6: dW[V, d] += dZ^T[V, rows] H[rows, d]
-      GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz, c.V, map_rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
+      GRPO_TRY(make_tmap(ctx, &tmDZ_mn, dz_rows, c.V, map_rows, static_cast<uint64_t>(L.v_pad) * 2, 64, BK));
       GRPO_TRY(make_tmap(ctx, &tmH_mn, Hc, c.d, map_rows, static_cast<uint64_t>(c.d) * 2, 64, BK));
       GemmParams p;
       std::memset(&p, 0, sizeof(p));
@@ -1060,7 +1038,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
-      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.tile_list = tile_list; p.dyn_rows = dyn_rows;
+      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       CUtensorMap tmDW;
       GRPO_TRY(make_tmap_c_f32(ctx, &tmDW, dW_accum, c.d, c.V, static_cast<uint64_t>(c.d) * 4));

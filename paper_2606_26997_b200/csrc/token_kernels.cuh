@@ -216,33 +216,6 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
   }
 }
 
-// Zero-coefficient tile scan.  One block; warp w scans token tiles w, w + nwarps, ...
-// of `tile_rows` rows: a tile is active iff any coeff in it is non-zero.  Output list: [0] = n_active,
-// [1] = n_tiles, [2 .. 2 + n_active) = active tile indices ascending, [2 + cap .. 2 + cap + n_tiles) =
-// per-tile flags.  stats (nullable): [0] += n_active, [1] += n_tiles.
-__global__ void __launch_bounds__(1024) active_tiles_kernel(const float* __restrict__ coeff, int rows, int tile_rows,
-                                                            int cap, int* __restrict__ list, int* __restrict__ stats) {
-  const int n_tiles = (rows + tile_rows - 1) / tile_rows;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
-  int* flags = list + 2 + cap;
-  for (int tile = warp; tile < n_tiles; tile += n_warps) {
-    const int beg = tile * tile_rows, end = min(rows, beg + tile_rows);
-    bool any = false;
-    for (int r = beg + lane; r < end; r += 32) any |= coeff[r] != 0.f;
-    any = __any_sync(0xffffffffu, any);
-    if (lane == 0) flags[tile] = any ? 1 : 0;
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    int n = 0;
-    for (int tile = 0; tile < n_tiles; ++tile)
-      if (flags[tile]) list[2 + n++] = tile;
-    list[0] = n;
-    list[1] = n_tiles;
-    if (stats) { atomicAdd(stats, n); atomicAdd(stats + 1, n_tiles); }
-  }
-}
-
 // Token-granular zero-coefficient compaction.  coeff_t = dloss/dlogp_t is exactly zero for
 // masked / ignored tokens, for clipped tokens at kl_beta = 0 (the clipped surrogate has no gradient
 // there) and for every token of a zero-variance group at kl_beta = 0; their dZ rows are zero, so the backward
@@ -317,18 +290,15 @@ __global__ void __launch_bounds__(128) gather_rows_kernel(const uint4* __restric
 
 // Split-K reduction of A5 (and the scatter of compacted rows back to their packed positions):
 // out[dst(r), :] = ((part_0[r,:] + part_1[r,:]) + part_2[r,:]) + ...   in that fixed order, r < rows.
-// dst(r) = row_idx[r] if row_idx != nullptr, else r.  tile_flags (nullable): rows of token tiles with flag 0 were
-// never computed (tile skipping of the stash variant) and are left alone.  One block per row; 16-byte accesses.
+// dst(r) = row_idx[r] if row_idx != nullptr, else r.  One block per row; 16-byte accesses.
 __global__ void __launch_bounds__(128) splitk_reduce_kernel(const float4* __restrict__ parts, int k_split,
                                                             int64_t split_stride_vec, int64_t row_vec /* d / 4 */,
                                                             int rows_static, const int* __restrict__ dyn_rows,
                                                             const int* __restrict__ row_idx,
-                                                            const int* __restrict__ tile_flags, int tile_rows,
                                                             void* __restrict__ out, int out_fp32) {
   const int r = blockIdx.x;
   const int rows = dyn_rows ? min(rows_static, *dyn_rows) : rows_static;
   if (r >= rows) return;
-  if (tile_flags != nullptr && tile_flags[r / tile_rows] == 0) return;
   const int64_t dst_row = row_idx ? row_idx[r] : r;
   const float4* src = parts + static_cast<int64_t>(r) * row_vec;
   for (int64_t i = threadIdx.x; i < row_vec; i += blockDim.x) {
@@ -532,28 +502,41 @@ __global__ void __launch_bounds__(256) quantize_rows_e4m3_kernel(const uint2* __
 
 // 3-contraction variant: turn the stashed exponentials e = 2^(z2 - m) (fp16, written by the
 // EPI_LSE_STASH epilogue together with m per (row, 256-column tile) in `shift`) into
-// dZ = k_t (1[v = y_t] - e 2^(m - lse2_t)) (bf16) in place; k_t = coeff_t * coeff_mul.  HBM-bound: 2 B read + 2 B
-// written per logit.  One block per walked row; 16-byte accesses; one ex2 per 8 logits.
-__global__ void __launch_bounds__(256) stash_to_dz_kernel(uint16_t* __restrict__ buf, int rows, int V, int64_t pitch,
+// dZ = k_t (1[v = y_t] - e 2^(m - lse2_t)) (bf16); k_t = coeff_t * coeff_mul.  HBM-bound: 2 B read + 2 B written
+// per logit.  One block per row; 16-byte accesses; one ex2 per 8 logits.
+// row_idx == nullptr: in place, every row of the chunk.  row_idx != nullptr (zero-coefficient compaction, DESIGN.md
+// section 10): destination row r < *dyn_rows is built from stash row row_idx[r] (chunk-local) and written to `out`,
+// a second chunk buffer; rows [*dyn_rows, round_up(*dyn_rows, tile_rows)) of `out` are zero-filled (the tail of the
+// last token tile A5 walks and of the last k block A6 reduces over).
+__global__ void __launch_bounds__(256) stash_to_dz_kernel(const uint16_t* stash, uint16_t* out /* may alias stash */,
+                                                          int rows_static, int V, int64_t pitch,
                                                           const float* __restrict__ shift, int64_t shift_pitch,
                                                           int tile_cols, const int32_t* __restrict__ targets,
                                                           const float* __restrict__ lse, const float* __restrict__ coeff,
-                                                          float coeff_mul, const int* __restrict__ tile_list,
-                                                          int tile_rows) {
-  int row = blockIdx.x;
-  if (tile_list != nullptr) {
-    const int w = row / tile_rows;
-    if (w >= tile_list[0]) return;
-    row = tile_list[2 + w] * tile_rows + row % tile_rows;
-  }
-  if (row >= rows) return;
-  const float lse2 = lse[row] * kLog2e;
-  const float k = coeff[row] * coeff_mul;
-  int y = targets[row];
-  if (y >= V) y = -1;
-  uint4* line = reinterpret_cast<uint4*>(buf + static_cast<int64_t>(row) * pitch);
-  const float* sh = shift + static_cast<int64_t>(row) * shift_pitch;
+                                                          float coeff_mul, const int* __restrict__ row_idx,
+                                                          const int* __restrict__ dyn_rows, int tile_rows, int rows_alloc) {
+  const int r = blockIdx.x;
   const int n_vec = (V + 7) / 8;
+  int src = r;
+  if (row_idx != nullptr) {
+    const int rows = *dyn_rows;
+    if (r >= min(rows_alloc, (rows + tile_rows - 1) / tile_rows * tile_rows)) return;
+    if (r >= rows) {
+      uint4* z = reinterpret_cast<uint4*>(out + static_cast<int64_t>(r) * pitch);
+      for (int i = threadIdx.x; i < n_vec; i += blockDim.x) z[i] = make_uint4(0u, 0u, 0u, 0u);
+      return;
+    }
+    src = row_idx[r];
+  } else if (r >= rows_static) {
+    return;
+  }
+  const float lse2 = lse[src] * kLog2e;
+  const float k = coeff[src] * coeff_mul;
+  int y = targets[src];
+  if (y >= V) y = -1;
+  const uint4* line = reinterpret_cast<const uint4*>(stash + static_cast<int64_t>(src) * pitch);
+  uint4* dst = reinterpret_cast<uint4*>(out + static_cast<int64_t>(r) * pitch);
+  const float* sh = shift + static_cast<int64_t>(src) * shift_pitch;
   for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
     const uint4 in = line[i];
     const float f = -k * ex2_approx(sh[i * 8 / tile_cols] - lse2);      // - k 2^(m - lse2) <= k in magnitude
@@ -569,21 +552,9 @@ __global__ void __launch_bounds__(256) stash_to_dz_kernel(uint16_t* __restrict__
 #pragma unroll
       for (int j = 0; j < 8; ++j) dz[j] = (y - i * 8 == j) ? dz[j] + k : dz[j];
     }
-    line[i] = make_uint4(pack_bf16x2(dz[0], dz[1]), pack_bf16x2(dz[2], dz[3]), pack_bf16x2(dz[4], dz[5]),
-                         pack_bf16x2(dz[6], dz[7]));
+    dst[i] = make_uint4(pack_bf16x2(dz[0], dz[1]), pack_bf16x2(dz[2], dz[3]), pack_bf16x2(dz[4], dz[5]),
+                        pack_bf16x2(dz[6], dz[7]));
   }
-}
-
-// dHidden rows of skipped tiles are zeros (what the dense A5 would have produced from an all-zero dZ
-// panel).  One block per tile; 16-byte stores (row_bytes is a multiple of 16: d % 8 == 0).
-__global__ void __launch_bounds__(256) zero_inactive_rows_kernel(uint8_t* __restrict__ out, int64_t row_bytes, int rows,
-                                                                 int tile_rows, const int* __restrict__ flags) {
-  const int tile = blockIdx.x;
-  if (flags[tile]) return;
-  const int beg = tile * tile_rows, end = min(rows, beg + tile_rows);
-  uint4* dst = reinterpret_cast<uint4*>(out + static_cast<int64_t>(beg) * row_bytes);
-  const int64_t n = static_cast<int64_t>(end - beg) * row_bytes / 16;
-  for (int64_t i = threadIdx.x; i < n; i += blockDim.x) dst[i] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 }  // namespace grpo

@@ -88,20 +88,37 @@ def test_agrees_with_the_recompute_path():
     assert rel_l2(to64(f["dW"]), to64(a["dW"])) < 5e-3
 
 
-def test_zero_tiles_are_skipped_in_the_stash_path_too():
+def test_zero_coefficient_rows_are_compacted_in_the_stash_path_too():
     b = _skippable_batch()
     ctx = make_ctx(b, bwd_chunk_tokens=2048, dhidden_fp32=1)
     try:
         ctx.ensure_workspace(b.T)
-        ctx.grpo_bwd_tile_stats_sync()
+        ctx.grpo_bwd_row_stats_sync()
         out = run_cuda(ctx, b, fused=True)
-        active, total = ctx.grpo_bwd_tile_stats_sync()
+        active, total = ctx.grpo_bwd_row_stats_sync()
     finally:
         ctx.close()
     ref = run_oracle(b)
     assert_gates(gates(b, out, ref))
-    assert 0 < active < total
+    assert total == b.T and active == int((ref["coeff"] != 0.0).sum()) < total
     assert torch.all(out["dH"][torch.from_numpy(ref["coeff"] == 0.0).cuda()] == 0)
+
+
+def test_scattered_zeros_and_the_dense_stash_backward_agree():
+    """config-1b recipe with beta = 0 and a mask: 20-40 % of the rows, scattered, have a zero coefficient; the
+    compacted 3-contraction backward equals the dense one (dHidden rows bit for bit) and the oracle."""
+    b = make_config(1, device="cuda", seed=7, variant="1b", n_groups=6, G=8, d=128, V=3000, len_div=0.1, w_std=0.1,
+                    kl_beta=0.0, mask_frac=0.15)
+    outs = []
+    for skip in (0, -1):
+        ctx = make_ctx(b, max_tokens=b.T, bwd_chunk_tokens=1024, bwd_skip_zero_tiles=skip, dhidden_fp32=1)
+        outs.append(run_cuda(ctx, b, fused=True))
+        ctx.close()
+    assert torch.equal(outs[0]["dH"], outs[1]["dH"])
+    assert rel_l2(to64(outs[0]["dW"]), to64(outs[1]["dW"])) < 1e-5
+    ref = run_oracle(b)
+    assert_gates(gates(b, outs[0], ref))
+    assert 0.15 * b.T < (ref["coeff"] == 0).sum() < 0.85 * b.T
 
 
 def test_step_host_with_stash_logits():
