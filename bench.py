@@ -15,7 +15,7 @@ Output: ONE JSON line on rank 0 (keys documented in DESIGN.md §6).  The headlin
 path (forward, then the backward that recomputes the logits chunk by chunk); `other_variant` times the
 3-contraction variant beside it.  Informational switches: `--stash` (make that variant the step),
 `--config 3|4|5` (the other BASELINE configs, device-resident), `--cgp-mode per_group|batch4` (configs[4] streamed
-through grpo_enqueue_groups), `--no-tile-skip`, `--no-drift-gate`, `--cta-group 1`, `--bwd-chunk N` (A/B runs).
+through grpo_enqueue_groups), `--no-tile-skip`, `--no-drift-gate`, `--cta-group 1`, `--bwd-chunk N`, `--max-ctas N` (A/B runs).
 `--impl reference` times the float64 CPU oracle (oracle/) on the host cores, on a bounded sample.
 """
 from __future__ import annotations
@@ -297,6 +297,8 @@ def run_ours(args):
         extra["gemm_drift_epoch_kb"] = -1
     if args.fp8:
         extra["fp8_logits"] = 1
+    if args.max_ctas:
+        extra["gemm_max_ctas"] = args.max_ctas
     if args.stash:
         extra["stash_logits"] = 1           # grpo_step_host (the e2e leg) then uses the same variant
     ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
@@ -704,6 +706,7 @@ def main():
     ap.add_argument("--no-variants", action="store_true", help="do not time the other variant beside the headline")
     ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")
+    ap.add_argument("--max-ctas", type=int, default=0, help="grpo_config.gemm_max_ctas (A/B runs; 0 = every SM)")
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-energy", action="store_true", help="skip the >= 2 s NVML energy leg (profiling runs)")

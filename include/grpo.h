@@ -93,6 +93,11 @@ typedef struct {
                                 e4m3 rounding of the operands (2^-4 relative per element): this does NOT meet
                                 north_star's 2e-3 log-prob tolerance and is never the default or the headline.
                                 Needs d % 16 == 0; not with stash_logits. */
+  int32_t gemm_max_ctas;     /* 0 = default: the persistent contraction kernels take every SM of the device.  n > 0:
+                                at most n CTAs (rounded down to whole CTA pairs), which leaves the other SMs to a
+                                kernel running concurrently on another stream — the all-reduce of the data-parallel
+                                update boundary.  Results do not depend on it bit for bit
+                                (every reduction is cut by the problem's shape alone). */
 } grpo_config;
 
 /* Fill *cfg with the defaults above (d, V must still be set). */

@@ -46,7 +46,8 @@ class GrpoConfig(C.Structure):
                 ("groups_per_update", C.c_int32), ("groups_per_round", C.c_int32), ("token_budget", C.c_int64),
                 ("bwd_chunk_tokens", C.c_int64), ("max_pending_groups", C.c_int32), ("gemm_cta_group", C.c_int32),
                 ("gemm_drift_epoch_kb", C.c_int32), ("kl_type", C.c_int32), ("dual_clip", C.c_float),
-                ("bwd_skip_zero_tiles", C.c_int32), ("stash_logits", C.c_int32), ("fp8_logits", C.c_int32)]
+                ("bwd_skip_zero_tiles", C.c_int32), ("stash_logits", C.c_int32), ("fp8_logits", C.c_int32),
+                ("gemm_max_ctas", C.c_int32)]
 
 
 class GroupDesc(C.Structure):

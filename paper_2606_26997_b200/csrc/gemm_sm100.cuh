@@ -218,6 +218,13 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   constexpr int kBRows = Shape::kBRows;
   constexpr int kBKe = DT == 1 ? 2 * BK : BK;                    // elements per k block (128 bytes)
   static_assert(DT == 0 || (!A_MN && !B_MN), "the e4m3 instance is K-major only");
+  // L2 eviction priorities (measured with ncu, profiles/r02c_l2_hints.md).  A6 streams its dZ column panel once
+  // (evict_first), re-reads the chunk's H rows for every vocab panel (evict_last) and touches every dW line once
+  // (reduce-add evict_first): DRAM reads per launch 6.7 -> 5.1 GB.  The other instances are best WITHOUT a hint:
+  // evict_first on the dZ panel of A5 or on the W tiles of A4 evicts lines before the other pairs of the wave
+  // have read them (A5 5.6 -> 9.7 GB, A4 0.7 -> 1.4 GB).
+  constexpr int kHintA = EPI == EPI_RED_F32 ? kL2EvictFirst : kL2None;
+  constexpr int kHintB = EPI == EPI_RED_F32 ? kL2EvictLast : kL2None;
   extern __shared__ uint8_t smem_raw[];
   // SWIZZLE_128B atoms need 1024-byte alignment of the tile bases (same offset in both CTAs of a pair)
   const uint32_t raw_addr = smem_u32(smem_raw);
@@ -261,6 +268,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     // an ELECT + four R2UR.BROADCAST per TMA instruction, which made this thread the bottleneck of A6).
     {
       const bool leader_lane = elect_one();
+      const uint64_t pol_a = l2_policy<kHintA>(), pol_b = l2_policy<kHintB>();
       const uint32_t full0 = CG == 2 ? mapa_cluster(smem_u32(&bars->full[0]), 0) : smem_u32(&bars->full[0]);
       int stage = 0;
       uint32_t phase = 0;
@@ -293,16 +301,16 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               const uint32_t b_dst = a_dst + kABytes;
               const uint32_t bar = full0 + stage * 8;
               if constexpr (!A_MN) {
-                tma_load_2d_t<CG>(a_dst, &tmA, bar, kb * kBKe, a_row);
+                tma_load_2d_t<CG, kHintA>(a_dst, &tmA, bar, kb * kBKe, a_row, pol_a);
               } else {
 #pragma unroll
-                for (int i = 0; i < BM / 64; ++i) tma_load_2d_t<CG>(a_dst + i * 8192, &tmA, bar, a_row + i * 64, kb * BK);
+                for (int i = 0; i < BM / 64; ++i) tma_load_2d_t<CG, kHintA>(a_dst + i * 8192, &tmA, bar, a_row + i * 64, kb * BK, pol_a);
               }
               if constexpr (!B_MN) {
-                tma_load_2d_t<CG>(b_dst, &tmB, bar, kb * kBKe, b_row);
+                tma_load_2d_t<CG, kHintB>(b_dst, &tmB, bar, kb * kBKe, b_row, pol_b);
               } else {
 #pragma unroll
-                for (int i = 0; i < kBRows / 64; ++i) tma_load_2d_t<CG>(b_dst + i * 8192, &tmB, bar, b_row + i * 64, kb * BK);
+                for (int i = 0; i < kBRows / 64; ++i) tma_load_2d_t<CG, kHintB>(b_dst + i * 8192, &tmB, bar, b_row + i * 64, kb * BK, pol_b);
               }
             }
             __syncwarp();
@@ -393,6 +401,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     const int row_in_tile = quad * 32 + lane;
     int acc = 0;
     uint32_t acc_phase = 0;
+    [[maybe_unused]] const uint64_t pol_c = l2_policy<kL2EvictFirst>();
     for (int u = unit0; u < n_units; u += unit_step) {
       const Unit un = unit_to_tiles<EPI>(p, ext, u);
       const int m_tile = un.m_tile, n0 = un.n0, n1 = un.n1;
@@ -581,7 +590,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) {
-              tma_reduce_add_2d(&tmC, red_buf, cbase, (m_tile * CG + static_cast<int>(cta_rank)) * BM + quad * 32);
+              tma_reduce_add_2d(&tmC, red_buf, cbase, (m_tile * CG + static_cast<int>(cta_rank)) * BM + quad * 32, pol_c);
               tma_store_commit();
             }
           }

@@ -301,7 +301,9 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   }
   if (n_units <= 0) return GRPO_OK;
   // persistent: one CTA (CG = 1) or one CTA pair (CG = 2, a 2-CTA cluster) per SM / SM pair
-  const int grid = CG * std::min(n_units, ctx->num_sms / CG);
+  // (gemm_max_ctas leaves SMs to a concurrent kernel; the unit -> reduction-range map never depends on the grid)
+  const int ctas = ctx->cfg.gemm_max_ctas > 0 ? std::min(ctx->cfg.gemm_max_ctas, ctx->num_sms) : ctx->num_sms;
+  const int grid = CG * std::min(n_units, std::max(ctas / CG, 1));
   GemmParams pl = p;
   pl.lse_block = grid / CG;
   // drift gate (gemm_sm100.cuh): epoch counters live in the launch's workspace slot, zeroed on the stream
@@ -408,6 +410,7 @@ extern "C" int32_t grpo_create(const grpo_config* cfg, grpo_ctx** out) {
     return fail(GRPO_ERR_INVALID_ARG, "fp8_logits needs d %% 16 == 0 and is not available with stash_logits");
   if (!(cfg->logit_scale > 0.f))
     return fail(GRPO_ERR_INVALID_ARG, "logit_scale (1 / temperature) must be > 0 (got %g)", (double)cfg->logit_scale);
+  if (cfg->gemm_max_ctas < 0) return fail(GRPO_ERR_INVALID_ARG, "gemm_max_ctas must be >= 0");
   if (cfg->kl_type < 0 || cfg->kl_type > 2 || (cfg->dual_clip != 0.f && !(cfg->dual_clip > 1.f)))
     return fail(GRPO_ERR_INVALID_ARG, "kl_type must be 0, 1 or 2 and dual_clip 0 or > 1");
   int dev = 0;

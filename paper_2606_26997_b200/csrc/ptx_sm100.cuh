@@ -74,25 +74,50 @@ __device__ __forceinline__ void tma_load_2d_cg2(uint32_t smem_dst, const CUtenso
       "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_cluster_addr), "r"(c0), "r"(c1)
       : "memory");
 }
-// CG = 1: `bar_addr` is this CTA's barrier; CG = 2: a shared::cluster barrier address (the leader's)
-template <int CG>
+// L2 eviction priority of a bulk-tensor instruction (.L2::cache_hint operand).  kL2None issues the instruction
+// without a hint, which is NOT the same as an explicit evict_normal policy (measured: A4 +20 % time with it).
+enum L2Hint : int { kL2None = 0, kL2EvictFirst = 1, kL2EvictLast = 2 };
+template <int HINT>
+__device__ __forceinline__ uint64_t l2_policy() {
+  uint64_t pol = 0;
+  if constexpr (HINT == kL2EvictFirst) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  if constexpr (HINT == kL2EvictLast) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+// CG = 1: `bar_addr` is this CTA's barrier; CG = 2: a shared::cluster barrier address (the leader's): the data
+// lands in this CTA's smem, complete_tx is signalled on the leader CTA's barrier.
+template <int CG, int HINT>
 __device__ __forceinline__ void tma_load_2d_t(uint32_t smem_dst, const CUtensorMap* m, uint32_t bar_addr, int c0,
-                                              int c1) {
-  if constexpr (CG == 2) {
-    tma_load_2d_cg2(smem_dst, m, bar_addr, c0, c1);
+                                              int c1, [[maybe_unused]] uint64_t pol) {
+  if constexpr (HINT == kL2None) {
+    if constexpr (CG == 2) tma_load_2d_cg2(smem_dst, m, bar_addr, c0, c1);
+    else
+      asm volatile(
+          "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+          ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_addr), "r"(c0), "r"(c1)
+          : "memory");
+  } else if constexpr (CG == 2) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+        "[%0], [%1, {%3, %4}], [%2], %5;" ::"r"(smem_dst),
+        "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_addr), "r"(c0), "r"(c1), "l"(pol)
+        : "memory");
   } else {
     asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-        ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_addr), "r"(c0), "r"(c1)
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+        "[%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_addr), "r"(c0), "r"(c1), "l"(pol)
         : "memory");
   }
 }
-// C[tile] += smem tile (element-wise fp32 add performed at L2; out-of-range rows / columns are clipped)
-__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* m, uint32_t smem_src, int c0, int c1) {
-  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3}], [%1];" ::"l"(
-                   reinterpret_cast<uint64_t>(m)),
-               "r"(smem_src), "r"(c0), "r"(c1)
-               : "memory");
+// C[tile] += smem tile (element-wise fp32 add performed at L2; out-of-range rows / columns are clipped).  The
+// reduced lines are marked evict_first: dW is touched once per launch and must not push the operand panels out of L2.
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* m, uint32_t smem_src, int c0, int c1,
+                                                  uint64_t pol) {
+  asm volatile(
+      "cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;"
+      ::"l"(reinterpret_cast<uint64_t>(m)), "r"(smem_src), "r"(c0), "r"(c1), "l"(pol)
+      : "memory");
 }
 __device__ __forceinline__ void st_shared_v4_f32(uint32_t addr, float a, float b, float c, float d) {
   asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");

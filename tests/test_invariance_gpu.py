@@ -68,6 +68,12 @@ def test_token_results_do_not_depend_on_the_launch_they_are_part_of(V, d):
     ctx2.close()
     for a, f in zip(other, full):
         assert torch.equal(a, f)
+    # (d) fewer CTAs (SMs left to a concurrent kernel, grpo_config.gemm_max_ctas): another unit-to-CTA deal, same bits
+    ctx3 = make_ctx(b, max_tokens=b.T, bwd_chunk_tokens=1024, gemm_max_ctas=36)
+    fewer = _fwd_bwd(ctx3, b, all_rows, denom, (adv, b.cu_seqlens))
+    ctx3.close()
+    for a, f in zip(fewer, full):
+        assert torch.equal(a, f)
 
 
 def _offpolicy_batch(beta=0.0, **kw):
