@@ -282,6 +282,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.power_study:
+        assert world == 1, "--power-study is a one-GPU informational run"
+        return run_power_study(args, dev)
     if args.sweep_T:
         assert world == 1, "--sweep-T is a one-GPU informational run"
         return run_sweep_T(args, dev)
@@ -535,6 +538,70 @@ def run_sweep_T(args, dev):
     return 0
 
 
+def run_power_study(args, dev):
+    """Informational (one JSON line): how much of the 1000 W board cap the OPERAND DATA costs.  The north_star step of
+    configs[1] is timed for >= 1.5 s on its synthetic operands and again with H and W replaced by zeros (same
+    launches, same tiles, same bytes moved: only the bits that toggle in the tensor-core datapath differ), and
+    cuBLAS (torch.matmul bf16 8192^3, the shape MEASURED_PEAKS.json was taken on) with N(0,1) and with zero
+    operands beside it.  DESIGN.md section 5, "Where the power goes"."""
+    import torch
+    from paper_2606_26997_b200 import GrpoContext
+    from workloads.synth import make_config
+    b = make_config(2, seed=0, device=dev)
+    T, d, V = b.T, b.d, b.V
+    # dense backward: with zero operands every ratio leaves the clip range and the row compaction would drop the rows
+    ctx = GrpoContext(d, V, max_tokens=T, group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
+                      bwd_skip_zero_tiles=-1)
+    dW = torch.zeros(V, d, dtype=torch.float32, device=dev)
+    loss = torch.zeros(1, dtype=torch.float32, device=dev)
+    dH = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
+
+    def sustained(fn, seconds, flops):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+        n = max(3, int(seconds * 1e3 / e0.elapsed_time(e1)))
+        sampler = ClockSampler(dev.index or 0)
+        sampler.start()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1) / n
+        return {"ms": ms, "tflops": flops / ms / 1e9, "sm_mhz": clocks.get("sm_mhz"),
+                "power_w": clocks.get("power_w_median"), "reasons": clocks.get("reasons"), "calls": n}
+
+    rows = {}
+    for name in ("synthetic", "zeros"):
+        H, W = (b.hidden, b.W) if name == "synthetic" else (torch.zeros_like(b.hidden), torch.zeros_like(b.W))
+
+        def step():
+            adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+            f = ctx.grpo_fused_logprob_loss_fwd(H, W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp, b.mask,
+                                                loss_accum=loss)
+            ctx.grpo_fused_logprob_loss_bwd(H, W, b.targets, f["lse"], f["coeff"], dW_accum=dW, dhidden_out=dH)
+
+        r = sustained(step, 1.5, 8.0 * T * V * d)
+        r["tokens_per_s"] = T / (r["ms"] * 1e-3)
+        rows["grpo_step_" + name] = r
+        del H, W
+    n = 8192
+    for name in ("randn", "zeros"):
+        A = (torch.randn if name == "randn" else torch.zeros)(n, n, device=dev, dtype=torch.bfloat16)
+        B = (torch.randn if name == "randn" else torch.zeros)(n, n, device=dev, dtype=torch.bfloat16)
+        C = torch.empty(n, n, device=dev, dtype=torch.bfloat16)
+        rows["cublas_8192_" + name] = sustained(lambda: torch.matmul(A, B, out=C), 1.5, 2.0 * n ** 3)
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "informational": "power_study", "n_gpus": 1, "dtype": "bf16",
+                      "data": "synthetic", "config": {"workload": "configs[1], north_star step; operands as drawn vs "
+                      "all-zero H and W; torch.matmul bf16 8192^3 beside it"}, "power_study": rows}), flush=True)
+    ctx.close()
+    return 0
+
+
 def run_cgp_stream(args, b, dev, world):
     """configs[4] (informational): the 32 complete groups are handed to grpo_enqueue_groups one at a time in their
     seeded arrival order, as CGP delivers them: `per_group` = U = 1, one launch per group on one
@@ -710,6 +777,9 @@ def main():
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-energy", action="store_true", help="skip the >= 2 s NVML energy leg (profiling runs)")
+    ap.add_argument("--power-study", action="store_true",
+                    help="informational: the step and cuBLAS on their operands vs all-zero operands (what the data costs "
+                         "under the board power cap)")
     ap.add_argument("--sweep-T", action="store_true",
                     help="informational: single-group launches (configs[1] recipe, lengths rescaled) at "
                          "T ~ 2k .. 33k tokens, the range CGP feeds one complete group at a time (PAPER.md:92)")
