@@ -95,7 +95,7 @@ class ClockSampler:
                0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
                0x10: "sync_boost"}
 
-    def __init__(self, torch_index: int, period_s: float = 0.05):
+    def __init__(self, torch_index: int, period_s: float = 0.02):
         self.period = period_s
         self.samples = []
         self.mask = 0
