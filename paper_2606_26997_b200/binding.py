@@ -175,7 +175,9 @@ class GrpoContext:
         self.h = h
         self.workspace = None
         self.max_tokens = 0
-        self._keep = []
+        self._keep = []                     # group descriptors queued in the library, FIFO order
+        self._inflight = []                 # (events, descriptors) of consumed groups whose launches may still run
+        self._consumed_seen = 0
         if max_tokens > 0:
             self.ensure_workspace(max_tokens, n_slots)
 
@@ -378,26 +380,51 @@ class GrpoContext:
         arr = (C.c_void_p * len(streams))(*[s.cuda_stream for s in streams])
         return arr, len(streams)
 
+    # Lifetime of the callers' tensors: a group's tensors must outlive the asynchronous launches that read them.
+    # Descriptors wait in `_keep` (FIFO order, like the library's queue) until the library reports them consumed;
+    # they then move to `_inflight` behind an event recorded on every launch stream and are dropped once it has
+    # completed - so a long-running trainer does not accumulate references to every group it ever enqueued.
+    def _retire(self, consumed_total: int, streams):
+        n = consumed_total - self._consumed_seen
+        self._consumed_seen = consumed_total
+        if n > 0:
+            done, self._keep = self._keep[:n], self._keep[n:]
+            evs = []
+            for s in (streams or [torch.cuda.current_stream()]):
+                e = torch.cuda.Event()
+                e.record(s)
+                evs.append(e)
+            self._inflight.append((evs, done))
+        while self._inflight and all(e.query() for e in self._inflight[0][0]):
+            self._inflight.pop(0)
+
     def grpo_enqueue_groups(self, groups: Sequence[GroupDesc], W, dW_accum, loss_accum, metrics_accum=None,
                             loss_denom: float = 0.0, streams=None):
         arr = (GroupDesc * max(len(groups), 1))(*groups)
-        self._keep.extend(groups)           # tensors must outlive the asynchronous work
         sarr, ns = self._streams(streams)
-        consumed, boundary = C.c_int32(0), C.c_int32(0)
-        _check(self.lib.grpo_enqueue_groups(self.h, arr, len(groups), _dev(W, torch.bfloat16, "W"),
-                                            _dev(dW_accum, torch.float32, "dW_accum"),
-                                            _dev(loss_accum, torch.float32, "loss_accum"),
-                                            _dev(metrics_accum, torch.float32, "metrics_accum"), float(loss_denom),
-                                            sarr, ns, C.byref(consumed), C.byref(boundary)))
+        consumed, boundary = C.c_int32(self._consumed_seen), C.c_int32(0)
+        pending_before = self.grpo_queue_state()["pending_groups"]
+        st = self.lib.grpo_enqueue_groups(self.h, arr, len(groups), _dev(W, torch.bfloat16, "W"),
+                                          _dev(dW_accum, torch.float32, "dW_accum"),
+                                          _dev(loss_accum, torch.float32, "loss_accum"),
+                                          _dev(metrics_accum, torch.float32, "metrics_accum"), float(loss_denom),
+                                          sarr, ns, C.byref(consumed), C.byref(boundary))
+        # the groups were appended unless the call was rejected before the queue was touched
+        if self.grpo_queue_state()["pending_groups"] + (consumed.value - self._consumed_seen) > pending_before:
+            self._keep.extend(groups)
+        self._retire(consumed.value, streams)
+        _check(st)
         return consumed.value, bool(boundary.value)
 
     def grpo_flush(self, W, dW_accum, loss_accum, metrics_accum=None, loss_denom: float = 0.0, streams=None):
         sarr, ns = self._streams(streams)
-        consumed, boundary = C.c_int32(0), C.c_int32(0)
-        _check(self.lib.grpo_flush(self.h, _dev(W, torch.bfloat16, "W"), _dev(dW_accum, torch.float32, "dW_accum"),
-                                   _dev(loss_accum, torch.float32, "loss_accum"),
-                                   _dev(metrics_accum, torch.float32, "metrics_accum"), float(loss_denom), sarr, ns,
-                                   C.byref(consumed), C.byref(boundary)))
+        consumed, boundary = C.c_int32(self._consumed_seen), C.c_int32(0)
+        st = self.lib.grpo_flush(self.h, _dev(W, torch.bfloat16, "W"), _dev(dW_accum, torch.float32, "dW_accum"),
+                                 _dev(loss_accum, torch.float32, "loss_accum"),
+                                 _dev(metrics_accum, torch.float32, "metrics_accum"), float(loss_denom), sarr, ns,
+                                 C.byref(consumed), C.byref(boundary))
+        self._retire(consumed.value, streams)
+        _check(st)
         return consumed.value, bool(boundary.value)
 
     def grpo_queue_state(self):
@@ -408,7 +435,8 @@ class GrpoContext:
 
     def grpo_reset_round(self):
         _check(self.lib.grpo_reset_round(self.h))
-        self._keep.clear()
+        self._keep.clear()                  # never launched: nothing reads them
+        self._consumed_seen = 0             # the library's counter restarts with the round
 
     def grpo_check_errors_sync(self) -> int:
         f = C.c_int32(0)

@@ -259,3 +259,31 @@ def test_an_update_that_cannot_run_is_rejected_before_anything_is_accumulated(ba
     ref = run_oracle(sub)
     assert abs(loss.item() - ref["loss"]) <= TOL_LOSS_REL * max(abs(ref["loss"]), ref["abs_loss"])
     assert rel_l2(to64(dW), ref["dW"]) <= TOL_GRAD_REL
+
+
+def test_binding_drops_group_tensors_once_their_launches_have_run(batch):
+    """The ctypes binding keeps a group's tensors alive while the library may still read them and not longer:
+    queued descriptors wait in FIFO order, consumed ones behind an event on the launch streams."""
+    b, _ = batch
+    order = list(b.arrival_order)
+    ctx = make_ctx(b, groups_per_update=2, max_tokens=b.T, bwd_chunk_tokens=1024)
+    dW = torch.zeros(b.V, b.d, dtype=torch.float32, device="cuda")
+    loss = torch.zeros(1, dtype=torch.float32, device="cuda")
+    descs, _ = _group_descs(ctx, b, order)
+    ctx.grpo_enqueue_groups(descs[:1], b.W, dW, loss, loss_denom=float(b.T))
+    assert len(ctx._keep) == 1 and not ctx._inflight            # U = 2: queued, nothing launched
+    ctx.grpo_enqueue_groups(descs[1:2], b.W, dW, loss, loss_denom=float(b.T))
+    assert len(ctx._keep) == 0 and sum(len(d) for _, d in ctx._inflight) in (0, 2)   # 0: already finished
+    torch.cuda.synchronize()
+    ctx.grpo_enqueue_groups(descs[2:3], b.W, dW, loss, loss_denom=float(b.T))
+    assert len(ctx._keep) == 1 and not ctx._inflight            # the first update has run: dropped
+    bad = ctx.make_group_desc(99, [0] * b.G, b.hidden, b.targets, b.old_logp, b.rewards[:b.G].contiguous())
+    with pytest.raises(Exception):
+        ctx.grpo_enqueue_groups([bad], b.W, dW, loss, loss_denom=float(b.T))
+    assert len(ctx._keep) == 1                                  # a rejected group is not kept
+    ctx.grpo_flush(b.W, dW, loss, loss_denom=float(b.T))
+    torch.cuda.synchronize()
+    ctx.grpo_flush(b.W, dW, loss, loss_denom=float(b.T))        # nothing pending; retires what has finished
+    assert not ctx._keep and not ctx._inflight
+    assert ctx.grpo_queue_state()["consumed_groups"] == 3
+    ctx.close()
