@@ -107,11 +107,15 @@ def _lengths(cfg: int, rng: np.random.Generator, S: int, len_div: float) -> np.n
 def _rewards(cfg: int, rng: np.random.Generator, n_groups: int, G: int) -> np.ndarray:
     if cfg == 2:
         # Bernoulli(0.5); redraw until the single group has variance (SURVEY §8(d) cfg 2)
+        if G < 2:
+            raise ValueError("config 2 redraws until the group has variance: needs G >= 2")
         while True:
             r = (rng.random((n_groups, G)) < 0.5).astype(np.float32)
             if np.all(r.std(axis=1) > 0):
                 return r.reshape(-1)
     need_mix = cfg == 3
+    if need_mix and n_groups < 2:
+        raise ValueError("config 3 keeps at least one zero-variance and one other group (R19): needs n_groups >= 2")
     while True:
         p = rng.beta(0.5, 0.5, size=n_groups)
         r = (rng.random((n_groups, G)) < p[:, None]).astype(np.float32)
