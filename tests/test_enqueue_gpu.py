@@ -56,8 +56,10 @@ def _gather(b, outs):
     return dH, lp
 
 
-def _stream_run(b, U, n_streams, token_budget=0, loss_denom=None, per_call=1, order=None):
-    """Enqueue groups `per_call` at a time in arrival order; returns accumulated outputs + bookkeeping."""
+def _stream_run(b, U, n_streams, token_budget=0, loss_denom=None, per_call=1, order=None, drain=False):
+    """Enqueue groups `per_call` at a time in arrival order; returns accumulated outputs + bookkeeping.
+    drain: a call runs at most ONE logical update, so with several groups per call keep calling with n = 0 while
+    a whole update is pending, and flush until the FIFO is empty."""
     order = list(b.arrival_order if order is None else order)
     ctx = make_ctx(b, groups_per_update=U, token_budget=token_budget, groups_per_round=len(order),
                    max_tokens=b.T, n_slots=n_streams, bwd_chunk_tokens=1024)
@@ -73,10 +75,13 @@ def _stream_run(b, U, n_streams, token_budget=0, loss_denom=None, per_call=1, or
         consumed, boundary = ctx.grpo_enqueue_groups(descs[i:i + per_call], b.W, dW, loss, metrics, loss_denom=denom,
                                                      streams=streams)
         log.append((consumed, boundary))
-    st = ctx.grpo_queue_state()
-    if st["pending_groups"]:
+        while drain and ctx.grpo_queue_state()["pending_groups"] >= U:
+            log.append(ctx.grpo_enqueue_groups([], b.W, dW, loss, metrics, loss_denom=denom, streams=streams))
+    while ctx.grpo_queue_state()["pending_groups"]:
         consumed, boundary = ctx.grpo_flush(b.W, dW, loss, metrics, loss_denom=denom, streams=streams)
         log.append((consumed, boundary))
+        if not drain:
+            break
     torch.cuda.synchronize()
     assert ctx.grpo_check_errors_sync() == 0
     state = ctx.grpo_queue_state()
@@ -287,3 +292,45 @@ def test_binding_drops_group_tensors_once_their_launches_have_run(batch):
     assert not ctx._keep and not ctx._inflight
     assert ctx.grpo_queue_state()["consumed_groups"] == 3
     ctx.close()
+
+
+@pytest.mark.parametrize("case", range(12))
+def test_random_dispatch_schedules_do_not_change_the_results(case):
+    """Seeded random CGP schedules (groups per update, token budget, number of streams, groups per call, arrival
+    order, both aggregations): whatever the schedule, every token's log-prob and dHidden row have the bits of the
+    single full-batch step, dW and the loss agree to summation order, the launches are the planner's, and the
+    result matches the oracle of the full batch."""
+    from paper_2606_26997_b200 import grpo_cgp_plan
+    rng = np.random.default_rng(9100 + case)
+    n_groups = int(rng.integers(3, 9))
+    loss_agg = int(rng.integers(0, 2))
+    b = make_config(5, device="cuda", seed=case, d=int(rng.choice([64, 128, 200])), V=int(rng.integers(300, 3000)),
+                    n_groups=n_groups, G=int(rng.integers(2, 5)), len_div=float(rng.choice([25.0, 60.0])), w_std=0.08,
+                    old_sigma=0.3, kl_beta=float(rng.choice([0.0, 0.002])), mask_frac=float(rng.choice([0.0, 0.2])),
+                    loss_agg=loss_agg)
+    order = list(rng.permutation(n_groups))
+    toks = [int(b.seqlens[g * b.G:(g + 1) * b.G].sum()) for g in order]
+    U = int(rng.integers(1, n_groups + 1))
+    budget = int(rng.choice([0, max(toks), max(toks) + min(toks), sum(toks) // 2 + 1]))
+    n_streams = int(rng.integers(1, 4))
+    ref = run_oracle(b, loss_denom=float(b.T))
+    out = _stream_run(b, U=U, n_streams=n_streams, token_budget=budget, per_call=int(rng.integers(1, 4)), order=order,
+                      drain=True)
+    ctx = make_ctx(b, bwd_chunk_tokens=1024)
+    full = run_cuda(ctx, b, loss_denom=float(b.T))
+    ctx.close()
+    if loss_agg == 0 or U >= n_groups:
+        # (per-sequence mean: the logical update is the unit the mean is taken over, so only a schedule with ONE
+        # update equals the full-batch step; the token mean has its denominator passed in)
+        _assert_oracle(b, out, ref)
+        assert torch.equal(out["logp"], full["logp"]) and torch.equal(out["dH"], full["dH"])
+        assert rel_l2(to64(out["dW"]), to64(full["dW"])) <= 1e-5
+    else:
+        assert torch.equal(out["logp"], full["logp"])
+    # the launches are the planner's: whole-group prefixes per update of U groups, the last update flushed short
+    expect, pos = 0, 0
+    while pos < n_groups:
+        plan = grpo_cgp_plan(toks[pos:], U=U, token_budget=budget, flush=True)
+        expect += len(plan)
+        pos += sum(plan)
+    assert out["launches"]["gemm_lse"] == expect and out["state"]["consumed_groups"] == n_groups
