@@ -16,8 +16,8 @@
 // CG = 1: one CTA per SM, C tile = 128 x 256, K block = 64 bf16 (one 128-byte swizzle row), 4-stage
 //         smem ring of 48 KB stages.
 // CG = 2: CTA pairs (cluster of 2 = one TPC), tcgen05 cta_group::2, pair tile = 256 x 256: CTA r of the
-//         pair stages A rows [r*128, +128) and B rows [r*128, +128) of the tile (32 KB per stage, 6-stage
-//         ring), the leader's MMA thread issues M=256 N=256 instructions that read both CTAs' smem, and
+//         pair stages A rows [r*128, +128) and B rows [r*128, +128) of the tile (32 KB per stage, 7-stage
+//         ring; 6 for A6), the leader's MMA thread issues M=256 N=256 instructions that read both CTAs' smem, and
 //         each CTA holds its own 128 accumulator rows in its TMEM.  Per-SM L2->smem traffic and smem
 //         operand reads drop by a third against CG = 1 at the same per-SM MMA rate.
 // Both: 2 x 256 TMEM columns so the epilogue of tile i overlaps the MMAs of tile i+1.
@@ -40,12 +40,15 @@ constexpr int kGemmThreads = 224;
 constexpr int kProducerWarp = 4, kMmaWarp = 5, kGateWarp = 6;
 constexpr int kTmemCols = 512;
 constexpr int kRedStageBytes = 4 * 32 * 32 * 4;   // A6 epilogue: one 32 x 32 fp32 block per epilogue warp (16 KB)
-template <int CG> struct GemmShape {
+// Ring depth: as many 32 KB stages as the 227 KB of shared memory hold - 7, or 6 for the A6 instance, whose
+// epilogue needs 16 KB of staging (A/B on one box, 3 runs each: 7 stages A4 -2 %, A2 / A5 -0.6 % against 6).
+template <int CG, int EPI> struct GemmShape {
   static constexpr int kBRows = BN / CG;                       // B rows (N index) staged by one CTA
   static constexpr int kBBytes = kBRows * BK * 2;              // 32 KB / 16 KB
   static constexpr int kStageBytes = kABytes + kBBytes;        // 48 KB / 32 KB
-  static constexpr int kStages = CG == 1 ? 4 : 6;
-  static constexpr int kSmemBytes = kStages * kStageBytes + kRedStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int kRedBytes = EPI == 3 ? kRedStageBytes : 0;   // only the A6 epilogue stages its blocks
+  static constexpr int kStages = CG == 1 ? 4 : (EPI == 3 ? 6 : 7);
+  static constexpr int kSmemBytes = kStages * kStageBytes + kRedBytes + 1024 /*align slack*/ + 256 /*barriers*/;
 };
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -212,7 +215,7 @@ template <int CG, bool A_MN, bool B_MN, int EPI, int DT = 0>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                  const __grid_constant__ CUtensorMap tmC, const GemmParams p, const int n_units_dense) {
-  using Shape = GemmShape<CG>;
+  using Shape = GemmShape<CG, EPI>;
   constexpr int kStages = Shape::kStages;
   constexpr int kStageBytes = Shape::kStageBytes;
   constexpr int kBRows = Shape::kBRows;
@@ -231,7 +234,7 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   const uint32_t pad = (1024u - (raw_addr & 1023u)) & 1023u;
   uint8_t* smem = smem_raw + pad;
   const uint32_t tiles_addr = raw_addr + pad;
-  GemmBarriers* bars = reinterpret_cast<GemmBarriers*>(smem + kStages * kStageBytes + kRedStageBytes);
+  GemmBarriers* bars = reinterpret_cast<GemmBarriers*>(smem + kStages * kStageBytes + Shape::kRedBytes);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;

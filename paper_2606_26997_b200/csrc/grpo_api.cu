@@ -293,7 +293,7 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   // template instantiation (setting it twice is harmless, so a relaxed atomic is enough)
   static std::atomic<uint64_t> attr_set{0};
   auto kern = grpo_gemm_kernel<CG, A_MN, B_MN, EPI, DT>;
-  constexpr int smem = GemmShape<CG>::kSmemBytes;
+  constexpr int smem = GemmShape<CG, EPI>::kSmemBytes;
   const uint64_t dev_bit = 1ull << (ctx->device & 63);
   if (ctx->device >= 64 || !(attr_set.load(std::memory_order_relaxed) & dev_bit)) {
     CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -1530,7 +1530,7 @@ extern "C" int32_t grpo_debug_max_active_clusters(grpo_ctx* ctx, int32_t cluster
   if (!ctx || !clusters_out || cluster_size < 1 || cluster_size > 16 || (cluster_size & 1 && cluster_size != 1))
     return fail(GRPO_ERR_INVALID_ARG, "need ctx, clusters_out and cluster_size in {1, 2, 4, ..., 16}");
   auto kern = grpo_gemm_kernel<2, false, false, EPI_LSE>;
-  constexpr int smem = GemmShape<2>::kSmemBytes;
+  constexpr int smem = GemmShape<2, EPI_RED_F32>::kSmemBytes;
   CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   if (cluster_size > 8) CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
   cudaLaunchConfig_t lc;
