@@ -127,6 +127,58 @@ def test_config2_full_size_bench_workload():
     assert _dense_part_rel(to64(dH32[torch.from_numpy(rows).cuda()]), dense_ref, entry, Wy) <= TOL_GRAD_REL
 
 
+# ------------------------------------------------------------------ configs[1] shape, LM-like logits, off-policy
+def test_full_size_lm_like_logits_off_policy():
+    """The BASELINE configs' synthetic softmax is near uniform (logit std 0.9) and their old log-probs never reach
+    the clip.  Same full shape with W ~ N(0, 0.1) (logit std 4.5, max ~ 20: a peaked,
+    LM-like distribution in which the dense softmax term of the gradient is no longer 2 % of it), old-log-prob noise
+    0.3 (both clip regions populated), KL on, a loss mask: every token's log-prob / lse / coefficient, the exact
+    clipped-token count, and sampled dH / dW rows incl. the never-target rows."""
+    b = make_config(2, seed=3, device="cuda", w_std=0.1, old_sigma=0.3, kl_beta=0.01, mask_frac=0.1)
+    assert (b.d, b.V) == (2048, 151936)
+    ctx = make_ctx(b, max_tokens=b.T)
+    out = run_cuda(ctx, b)
+    assert ctx.grpo_check_errors_sync() == 0
+    rows_walked, rows_total = ctx.grpo_bwd_row_stats_sync()
+    ctx.close()
+    x = b.numpy_f64()
+    lse, logp = token_logprobs(x["H"], x["W"], x["y"])
+    assert np.abs(lse).max() > 8 and np.exp(logp).max() > 0.5                # peaked: some tokens nearly certain
+    adv, _ = group_advantage(x["rewards"], G=b.G, eps_std=b.eps_std)
+    lt = loss_terms(logp, x["old_logp"], x["ref_logp"], x["mask"], token_advantage(adv, x["cu_seqlens"]),
+                    x["cu_seqlens"], _ocfg(b))
+    assert np.abs(to64(out["logp"]) - logp).max() <= TOL_LOGP_ABS
+    assert np.abs(to64(out["lse"]) - lse).max() <= TOL_LOGP_ABS
+    assert abs(out["loss"].item() - lt["loss"]) <= TOL_LOSS_REL * max(abs(lt["loss"]), lt["abs_loss"])
+    # the clip decision is taken in fp32 on the GPU and in float64 here (DESIGN.md R25): among 15k random tokens a
+    # few have rho within fp32 rounding of a bound and may fall on the other side; they are set aside, everything
+    # else must agree, and the clipped-token counts may differ by at most their number
+    rho = lt["rho"]
+    near = np.minimum(np.abs(rho - (1 - b.clip_lo)), np.abs(rho - (1 + b.clip_hi))) < 1e-4
+    assert near.sum() <= 0.002 * b.T
+    assert rel_l2(to64(out["coeff"])[~near], lt["coeff"][~near]) <= 1e-3
+    clipped = lt["metrics"][3]
+    assert 0.05 * b.T < clipped < 0.6 * b.T and abs(to64(out["metrics"])[3] - clipped) <= near.sum()
+    assert abs(rows_walked - int((lt["coeff"] != 0).sum())) <= near.sum() and rows_total == b.T
+    rows = _sample_tokens(b, 48, seed=4)
+    rows = rows[~near[rows]]
+    dH_ref = dH_rows(x["H"], x["W"], x["y"], lse[rows], lt["coeff"][rows], rows)
+    dH = to64(out["dH"][torch.from_numpy(rows).cuda()])
+    assert rel_l2(dH, dH_ref) <= TOL_GRAD_REL
+    assert np.all(dH[lt["coeff"][rows] == 0] == 0)
+    rng = np.random.default_rng(5)
+    tgt = np.unique(x["y"])
+    non = np.setdiff1d(np.arange(b.V), tgt)
+    vids = np.unique(np.concatenate([rng.choice(tgt, 24, replace=False), rng.choice(non, 24, replace=False),
+                                     [0, 255, 256, 151807, 151808, b.V - 1]]))
+    dW_ref = dW_rows(x["H"], x["W"], x["y"], lse, lt["coeff"], vids)
+    dW = to64(out["dW"][torch.from_numpy(vids).cuda()])
+    is_t = np.isin(vids, tgt)
+    assert rel_l2(dW[is_t], dW_ref[is_t]) <= TOL_GRAD_REL
+    assert rel_l2(dW[~is_t], dW_ref[~is_t]) <= TOL_GRAD_REL
+    assert _colsum_rel(out["dW"]) <= 2e-3
+
+
 # ------------------------------------------------------------------ configs[2]: 4 x G=8, KL, zero-variance groups
 def test_config3_full_size_sampled():
     b = make_config(3, seed=0, device="cuda")
