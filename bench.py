@@ -289,7 +289,8 @@ def run_ours(args):
         assert world == 1, "--sweep-T is a one-GPU informational run"
         return run_sweep_T(args, dev)
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
-    b = make_config(args.config, seed=rank_seed(rank), device=dev, prenorm=args.prenorm)
+    gen_kw = dict(old_sigma=0.3, mask_frac=0.1) if args.off_policy else {}
+    b = make_config(args.config, seed=rank_seed(rank), device=dev, prenorm=args.prenorm, **gen_kw)
     if args.cgp_mode != "full":
         return run_cgp_stream(args, b, dev, world)
     T, d, V = b.T, b.d, b.V
@@ -363,7 +364,7 @@ def run_ours(args):
     # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step.  Timed
     # right after the headline region so that both see the same thermal / power state of the board.
     e2e_s, h2d, d2h = 0.0, 0, 0
-    if args.config == 2 and not args.prenorm and not args.fp8:
+    if args.config == 2 and not args.prenorm and not args.fp8 and not args.off_policy:
         pin = lambda t: None if t is None else t.cpu().pin_memory()
         h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
                                                        pin(b.old_logp))
@@ -447,7 +448,7 @@ def run_ours(args):
                               "ms_per_step": v_ms / args.steps}
 
     # ---- informational runs (--config 3/4/5, --prenorm) are device-resident: no e2e / cpu_baseline legs
-    if args.config != 2 or args.prenorm or args.fp8:
+    if args.config != 2 or args.prenorm or args.fp8 or args.off_policy:
         ms_total, _, tokens_all = reduce_over_ranks(ms_total, 0.0, T, world, dev)
         if rank == 0:
             line = build_line(args, b, world, tokens_all * args.steps / (ms_total * 1e-3), ms_total, None, 0, 0,
@@ -726,7 +727,8 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "e4m3 (A2, A4 operands) + bf16" if getattr(args, "fp8", False) else "bf16", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config],
+        "config": {"workload": WORKLOADS[args.config] + (" (informational: --off-policy, old log-prob noise 0.3, "
+                                                         "10 % of the tokens masked)" if args.off_policy else ""),
                    "variant": "fp8_logits (informational PRECISION STUDY, NEXT-4: e4m3 operands for A2 / A4; does not meet "
                    "north_star's log-prob tolerance)" if args.fp8 else "prenorm (informational, NEXT-4): RMSNorm fwd + north_star path + RMSNorm bwd fused behind A5"
                    if args.prenorm else "stash_logits (3 contractions, DESIGN.md section 11)" if args.stash
@@ -770,6 +772,10 @@ def main():
     ap.add_argument("--fp8", action="store_true",
                     help="informational precision study (NEXT-4): grpo_config.fp8_logits = 1 (e4m3 operands for the two "
                          "logit contractions); no e2e / cpu_baseline legs")
+    ap.add_argument("--off-policy", action="store_true",
+                    help="informational: the workload in the off-policy regime of config 1b (old log-prob noise 0.3: "
+                         "20-40 %% of the tokens clipped; 10 %% masked; no KL), whose zero-coefficient rows the backward "
+                         "compacts away (DESIGN.md section 10); no e2e / cpu_baseline legs")
     ap.add_argument("--no-variants", action="store_true", help="do not time the other variant beside the headline")
     ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")
