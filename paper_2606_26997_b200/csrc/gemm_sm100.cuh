@@ -517,9 +517,11 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
               if (row_ok) {
                 __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
 #pragma unroll
-                for (int g = 0; g < 4; ++g)
-                  st_global_v4(dst + g * 8, pack_f16x2(e[g * 8 + 0], e[g * 8 + 1]), pack_f16x2(e[g * 8 + 2], e[g * 8 + 3]),
-                               pack_f16x2(e[g * 8 + 4], e[g * 8 + 5]), pack_f16x2(e[g * 8 + 6], e[g * 8 + 7]));
+                for (int g = 0; g < 2; ++g)
+                  st_global_v8(dst + g * 16, pack_f16x2(e[g * 16 + 0], e[g * 16 + 1]), pack_f16x2(e[g * 16 + 2], e[g * 16 + 3]),
+                               pack_f16x2(e[g * 16 + 4], e[g * 16 + 5]), pack_f16x2(e[g * 16 + 6], e[g * 16 + 7]),
+                               pack_f16x2(e[g * 16 + 8], e[g * 16 + 9]), pack_f16x2(e[g * 16 + 10], e[g * 16 + 11]),
+                               pack_f16x2(e[g * 16 + 12], e[g * 16 + 13]), pack_f16x2(e[g * 16 + 14], e[g * 16 + 15]));
               }
             }
             run_s = run_s * rescale + s;
@@ -549,25 +551,30 @@ grpo_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             for (int j = 0; j < 16; ++j) pk[j] = pack_bf16x2(dzv[2 * j], dzv[2 * j + 1]);
             if (row_ok) {
               __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
+              // 2 x 32-byte stores (STG.256): whole aligned sectors (the row pitch is a multiple of 128 bytes)
 #pragma unroll
-              for (int g = 0; g < 4; ++g) st_global_v4(dst + g * 8, pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+              for (int g = 0; g < 2; ++g)
+                st_global_v8(dst + g * 16, pk[8 * g], pk[8 * g + 1], pk[8 * g + 2], pk[8 * g + 3], pk[8 * g + 4],
+                             pk[8 * g + 5], pk[8 * g + 6], pk[8 * g + 7]);
             } else if (row_local < p.m_alloc) {
               // rows of the last walked tile beyond the (dynamic) row count: A6 reads them as the tail of its last
               // k block, so they must hold zeros, not what an earlier chunk left there
               __nv_bfloat16* dst = p.dz + static_cast<int64_t>(row_local) * p.dz_pitch + cbase;
 #pragma unroll
-              for (int g = 0; g < 4; ++g) st_global_v4(dst + g * 8, 0u, 0u, 0u, 0u);
+              for (int g = 0; g < 2; ++g) st_global_v8(dst + g * 16, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u);
             }
           } else if constexpr (EPI == EPI_STORE) {
             if (row_ok) {
               if (p.c_fp32) {
                 float* dst = reinterpret_cast<float*>(p.c_out) + un.part * p.c_split_stride +
                              static_cast<int64_t>(row_local) * p.c_pitch + cbase;
+                // 32-byte stores where the pitch keeps them aligned (c_pitch % 8 == 0: d % 8 == 0 always holds)
 #pragma unroll
-                for (int g = 0; g < 8; ++g)
-                  if (g * 4 < nvalid)
-                    *reinterpret_cast<float4*>(dst + g * 4) =
-                        make_float4(v[g * 4], v[g * 4 + 1], v[g * 4 + 2], v[g * 4 + 3]);
+                for (int g = 0; g < 4; ++g)
+                  if (g * 8 < nvalid)
+                    st_global_v8(dst + g * 8, __float_as_uint(v[g * 8]), __float_as_uint(v[g * 8 + 1]),
+                                 __float_as_uint(v[g * 8 + 2]), __float_as_uint(v[g * 8 + 3]), __float_as_uint(v[g * 8 + 4]),
+                                 __float_as_uint(v[g * 8 + 5]), __float_as_uint(v[g * 8 + 6]), __float_as_uint(v[g * 8 + 7]));
               } else {
                 __nv_bfloat16* dst =
                     reinterpret_cast<__nv_bfloat16*>(p.c_out) + static_cast<int64_t>(row_local) * p.c_pitch + cbase;
