@@ -73,6 +73,7 @@ struct SlotLayout {
           off_row_stats = 0;
   int64_t n_chunks_max = 0;
   int64_t fwd_block_rows = 0;   // rows per A2 launch (bounds the LSE partials)
+  int64_t off_loss_part = 0, off_loss_count = 0;                  // A3: per-block partial sums, arrival counter
   int64_t off_w8 = 0, off_h8 = 0, off_hscale = 0, off_wscale = 0;   // FP8 study (cfg.fp8_logits)
   int64_t bytes = 0;
 };
@@ -218,6 +219,8 @@ static SlotLayout make_layout(const grpo_config& c, int64_t max_T) {
   L.off_coeffc = take(L.chunk_rows * 4);
   L.off_dh_part = take(static_cast<int64_t>(k_split) * L.chunk_rows * c.d * 4);
   L.off_row_stats = take(16);
+  L.off_loss_part = take(((max_T + 255) / 256 + 1) * 5 * 4);
+  L.off_loss_count = take(16);
   if (c.fp8_logits) {
     L.off_w8 = take(static_cast<int64_t>(c.V) * c.d);
     L.off_h8 = take(std::max(L.fwd_block_rows, L.chunk_rows) * c.d);
@@ -480,6 +483,7 @@ extern "C" int32_t grpo_set_workspace(grpo_ctx* ctx, void* dev_ptr, int64_t byte
   ctx->lay = L;
   for (int i = 0; i < n_slots; ++i) {
     CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_row_stats), 0, 16));
+    CU_OK(cudaMemset(slot_ptr<int>(ctx, i, L.off_loss_count), 0, 16));
   }
   // pinned ring for run_launch's index arrays: cu_seqlens [S+1] + cu_groups [S+1] per entry
   const int64_t need = 2 * (L.s_max + 1);
@@ -686,6 +690,8 @@ static int32_t loss_rows(grpo_ctx* ctx, int slot, const float* part_m, const flo
   lp.kl_type = c.kl_type; lp.dual_clip = c.dual_clip;
   lp.logp = a.logp_out; lp.lse = a.lse_out; lp.coeff = a.coeff_out; lp.loss_accum = a.loss_accum;
   lp.metrics_accum = a.metrics_accum; lp.err_flag = ctx->err_dev;
+  lp.block_part = slot_ptr<float>(ctx, slot, L.off_loss_part);
+  lp.block_count = slot_ptr<unsigned int>(ctx, slot, L.off_loss_count);
   const int threads = 256;
   const int blocks = static_cast<int>((rows + threads - 1) / threads);
   {

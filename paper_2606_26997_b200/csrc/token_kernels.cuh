@@ -113,9 +113,14 @@ struct LossParams {
   float* loss_accum;
   float* metrics_accum;      // nullable, [4]
   int32_t* err_flag;
+  // fixed-order reduction over the launch's blocks: [gridDim.x][5] partial sums + an arrival counter (self-resetting)
+  float* block_part;
+  unsigned int* block_count;
 };
 
-// A3.  One thread per packed token; block-level reduction, then one atomic per block and quantity.
+// A3.  One thread per packed token; block-level reduction; the block sums go to a workspace array and the block
+// that arrives last adds them up in block order, so that a launch contributes ONE add per quantity and the scalar
+// loss / metrics are bit-reproducible run to run (like every per-token output and, on one stream, dW).
 __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) {
   const int64_t t = p.t_begin + static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   float loss_t = 0.f, m_cnt = 0.f, m_rho = 0.f, m_k3 = 0.f, m_clip = 0.f;
@@ -203,16 +208,33 @@ __global__ void __launch_bounds__(256) loss_epilogue_kernel(const LossParams p) 
     if (lane == 0) red[q][warp] = r;
   }
   __syncthreads();
+  __shared__ int is_last;
   if (warp == 0) {
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       float r = lane < 8 ? red[q][lane] : 0.f;
+      r = warp_sum(r);
+      if (lane == 0) p.block_part[blockIdx.x * 5 + q] = r;
+    }
+    if (lane == 0) {
+      __threadfence();
+      is_last = atomicAdd(p.block_count, 1u) == gridDim.x - 1 ? 1 : 0;
+    }
+  }
+  __syncthreads();
+  if (is_last && warp == 0) {
+    __threadfence();
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      float r = 0.f;
+      for (unsigned int b = lane; b < gridDim.x; b += 32) r += __ldcg(p.block_part + b * 5 + q);   // fixed order
       r = warp_sum(r);
       if (lane == 0 && r != 0.f) {
         if (q == 0) atomicAdd(p.loss_accum, r);
         else if (p.metrics_accum) atomicAdd(p.metrics_accum + (q - 1), r);
       }
     }
+    if (lane == 0) *p.block_count = 0u;           // ready for the slot's next launch (stream-ordered)
   }
 }
 
