@@ -245,6 +245,15 @@ def reduce_over_ranks(ms_total: float, e2e_s: float, tokens: int, world: int, de
     return ms, e2e, toks.item()
 
 
+# north_star: the throughput "sits next to ... the paper's rollout-to-train-end reductions ... quoted with the hardware the
+# paper states, as context only".  The paper has no number for this path: vs_baseline stays null.
+PAPER_CONTEXT = {
+    "rollout_to_train_end_reduction_vs_slime": "30.7 %-42.3 % (CGP+FGD over 12 settings; PAPER.md:9, 220)",
+    "trainer_waiting_ratio": "Slime 47-52 %, CGP+FGD 14-33 % (PAPER.md:46, 236)",
+    "hardware": "policy Qwen3-1.7B; trainer 8x RTX 4090 24 GB (TP=4, DP=2), rollout 2x A100 40 GB PCIe (TP=2) (PAPER.md:197)",
+    "note": "whole-system times of the paper's Slime/SGLang/Megatron stack on other hardware: context only, not a "
+            "target and not comparable with this line's tokens/s of the loss step alone",
+}
 GEMM_KINDS = ("gemm_lse", "gemm_dz", "gemm_dh", "gemm_dw")
 WORKLOADS = {
     2: "configs[1]: one complete group G=8, lengths U[512,4096], d=2048, V=151936, on-policy old log-probs, "
@@ -746,6 +755,7 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         "other_variant": getattr(args, "other_variant", None),
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
         "loss_after_steps": loss_val,
+        "paper_context": PAPER_CONTEXT,
     }
 
 
