@@ -1011,7 +1011,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
       p.n_fastest = 1;
       p.k_split = k_split; p.kb_per_split = kb_per_split; p.c_split_stride = L.chunk_rows * c.d;
-      p.c_out = dh_part; p.c_pitch = c.d; p.c_fp32 = 1;
+      p.c_out = dh_part; p.c_pitch = c.d;
       p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       GRPO_TRY((launch_gemm<false, true, EPI_STORE>(ctx, GRPO_KERNEL_GEMM_DH, tmDZ_k, tmW_mn, p,
@@ -1047,7 +1047,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
       p.n_fastest = 1;
-      p.c_out = dW_accum; p.c_pitch = c.d; p.c_fp32 = 1; p.dyn_rows = dyn_rows;
+      p.c_out = dW_accum; p.c_pitch = c.d; p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       CUtensorMap tmDW;
       GRPO_TRY(make_tmap_c_f32(ctx, &tmDW, dW_accum, c.d, c.V, static_cast<uint64_t>(c.d) * 4));
@@ -1570,7 +1570,7 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
   const int TM = BM * ctx->cg;
   p.m_tiles = (M + TM - 1) / TM; p.n_tiles = (N + BN - 1) / BN; p.k_blocks = (K + BK - 1) / BK;
   p.n_fastest = 1;
-  p.c_out = C; p.c_pitch = N; p.c_fp32 = 1;
+  p.c_out = C; p.c_pitch = N;
   if (ctx->ws) p.sync = slot_ptr<unsigned int>(ctx, 0, ctx->lay.off_sync);
   const int units = p.m_tiles * p.n_tiles;
   const bool a_mn = layout == 2, b_mn = layout >= 1;

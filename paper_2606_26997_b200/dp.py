@@ -22,7 +22,7 @@ import socket
 import threading
 import uuid
 from dataclasses import dataclass, field
-from typing import List, Optional, Sequence
+from typing import List, Optional
 
 import torch
 import torch.distributed as dist

@@ -2,7 +2,6 @@
 shard through a collective; `bench.py --gpus N` runs one independent complete group per rank):
 the whole-job reduction (MAX of the timed regions, SUM of tokens), the per-rank workload assignment, and
 the reference arm's "rank 0 alone prints" rule."""
-import json
 import os
 import socket
 import subprocess

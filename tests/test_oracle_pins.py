@@ -11,7 +11,7 @@ import pytest
 import scipy.special
 import torch
 
-from oracle.grpo_oracle import (OracleConfig, backward, bf16_bits_to_f64, group_advantage,
+from oracle.grpo_oracle import (OracleConfig, bf16_bits_to_f64, group_advantage,
                                 grpo_step, grpo_step_loops, loss_terms, token_advantage,
                                 token_logprobs)
 

@@ -5,9 +5,9 @@ import numpy as np
 import pytest
 import torch
 
-from tests.parity_util import (TOL_GRAD_REL, TOL_LOGP_ABS, assert_gates, gates, make_ctx, rel_l2, run_cuda,
+from tests.parity_util import (assert_gates, gates, make_ctx, rel_l2, run_cuda,
                                run_oracle, to64)
-from workloads.synth import make_config, slice_groups
+from workloads.synth import make_config
 
 pytestmark = pytest.mark.gpu
 

@@ -18,7 +18,7 @@ lengths -> p_g -> rewards -> W -> H -> base logits -> targets -> old noise -> re
 """
 from __future__ import annotations
 
-from dataclasses import dataclass, field
+from dataclasses import dataclass
 from typing import Optional
 
 import numpy as np
