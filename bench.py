@@ -605,6 +605,23 @@ def run_power_study(args, dev):
         B = (torch.randn if name == "randn" else torch.zeros)(n, n, device=dev, dtype=torch.bfloat16)
         C = torch.empty(n, n, device=dev, dtype=torch.bfloat16)
         rows["cublas_8192_" + name] = sustained(lambda: torch.matmul(A, B, out=C), 1.5, 2.0 * n ** 3)
+    # Which input of the multipliers the energy follows: ONE operand random, the other constant, both ways round,
+    # through cuBLAS and through this library's contraction kernel (grpo_debug_gemm: the production kernel with a
+    # plain fp32 epilogue; layout 0: A [M, K] and B [N, K] both K-major, like A2 / A4).  K = 2048 so that both
+    # operands stay in L2 and DRAM traffic is out of the picture.  torch.matmul(A, B^T) hands row-major operands to
+    # a column-major library, which swaps their roles: its expensive side is the other one.
+    K2 = 2048
+    mk = {"randn": lambda: torch.randn(n, K2, device=dev, dtype=torch.bfloat16),
+          "zeros": lambda: torch.zeros(n, K2, device=dev, dtype=torch.bfloat16),
+          "ones": lambda: torch.ones(n, K2, device=dev, dtype=torch.bfloat16)}
+    Cf = torch.empty(n, n, device=dev, dtype=torch.float32)
+    Cb = torch.empty(n, n, device=dev, dtype=torch.bfloat16)
+    for ka, kb in (("randn", "randn"), ("randn", "zeros"), ("zeros", "randn"), ("randn", "ones"), ("ones", "randn"),
+                   ("zeros", "zeros")):
+        A, B = mk[ka](), mk[kb]()
+        rows[f"grpo_gemm_A_{ka}_B_{kb}"] = sustained(lambda: ctx.grpo_debug_gemm(0, A, B, n, n, K2, C_out=Cf), 0.8,
+                                                     2.0 * n * n * K2)
+        rows[f"cublas_A_{ka}_B_{kb}"] = sustained(lambda: torch.matmul(A, B.t(), out=Cb), 0.8, 2.0 * n * n * K2)
     print(json.dumps({"metric": METRIC, "unit": UNIT, "informational": "power_study", "n_gpus": 1, "dtype": "bf16",
                       "data": "synthetic", "config": {"workload": "configs[1], north_star step; operands as drawn vs "
                       "all-zero H and W; torch.matmul bf16 8192^3 beside it"}, "power_study": rows}), flush=True)
