@@ -194,3 +194,63 @@ def test_odd_shapes(d, V, fused):
     finally:
         ctx.close()
     assert_gates(gates(b, out, run_oracle(b)))
+
+
+# ------------------------------------------------------------------ no write outside the caller's buffers
+@pytest.mark.parametrize("d,V,fp32", [(72, 1003, 1), (8, 9, 0), (200, 257, 0), (136, 5001, 1), (64, 1000, 0)])
+@pytest.mark.parametrize("fused", [False, True])
+def test_outputs_are_written_inside_their_buffers(d, V, fp32, fused):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are looked for directly: dHidden and dW
+    live inside a pool filled with a sentinel, with guard bands on both sides, for shapes whose tiles, 32-byte store
+    vectors and TMA reduce boxes all end ragged (d % 64 != 0, odd V, T not a multiple of the tile); the guard bands
+    must come back untouched and the results must be those of ordinary buffers."""
+    b = make_config(1, device="cuda", seed=31, variant="1b", d=d, V=V, w_std=0.3, mask_frac=0.2)
+    guard = 4096                                                       # elements on each side
+    dh_dtype = torch.float32 if fp32 else torch.bfloat16
+    pool_h = torch.full((2 * guard + b.T * d,), 7.0, dtype=dh_dtype, device="cuda")
+    pool_w = torch.full((2 * guard + V * d,), 7.0, dtype=torch.float32, device="cuda")
+    dH = pool_h[guard:guard + b.T * d].view(b.T, d)
+    dW = pool_w[guard:guard + V * d].view(V, d)
+    dW.zero_()
+    ctx = make_ctx(b, dhidden_fp32=fp32, bwd_chunk_tokens=128)
+    try:
+        adv = ctx.grpo_group_advantage(b.rewards, G=b.G)
+        if fused:
+            ctx.grpo_fused_logprob_loss_fwd_bwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                                b.mask, dW_accum=dW, dhidden_out=dH)
+        else:
+            f = ctx.grpo_fused_logprob_loss_fwd(b.hidden, b.W, b.targets, b.cu_seqlens, adv, b.old_logp, b.ref_logp,
+                                                b.mask)
+            ctx.grpo_fused_logprob_loss_bwd(b.hidden, b.W, b.targets, f["lse"], f["coeff"], dW_accum=dW, dhidden_out=dH)
+        torch.cuda.synchronize()
+        ref = run_cuda(ctx, b, fused=fused)
+    finally:
+        ctx.close()
+    for pool in (pool_h, pool_w):
+        assert torch.all(pool[:guard] == 7.0) and torch.all(pool[-guard:] == 7.0)
+    assert torch.equal(dH, ref["dH"]) and torch.equal(dW, ref["dW"])
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_workspace_is_not_overrun(fused):
+    """The library writes nothing beyond the grpo_workspace_bytes(max_T) it asked for: a step at exactly max_T tokens
+    in a workspace of exactly that size, sentinel bytes behind it."""
+    import ctypes as C
+    from paper_2606_26997_b200 import GrpoContext
+    b = make_config(3, device="cuda", d=136, V=2500, len_div=30, w_std=0.08, mask_frac=0.2)
+    ctx = GrpoContext(b.d, b.V, eps_std=b.eps_std, clip_lo=b.clip_lo, clip_hi=b.clip_hi, kl_beta=b.kl_beta,
+                      group_size=b.G, bwd_chunk_tokens=256)
+    need = ctx.workspace_bytes(b.T)
+    guard = 1 << 16
+    pool = torch.full((need + 256 + guard,), 0x5A, dtype=torch.uint8, device="cuda")
+    base = (pool.data_ptr() + 255) // 256 * 256
+    off = base - pool.data_ptr()
+    assert ctx.lib.grpo_set_workspace(ctx.h, C.c_void_p(base), need, b.T, 1) == 0
+    ctx.workspace, ctx.max_tokens, ctx.n_slots = pool, b.T, 1          # the binding must not re-allocate
+    try:
+        out = run_cuda(ctx, b, fused=fused)
+        assert ctx.grpo_check_errors_sync() == 0
+    finally:
+        ctx.close()
+    assert torch.all(pool[off + need:] == 0x5A)
+    assert_gates(gates(b, out, run_oracle(b)))
