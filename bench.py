@@ -308,6 +308,8 @@ def run_ours(args):
         extra["bwd_skip_zero_tiles"] = -1
     if args.no_drift_gate:
         extra["gemm_drift_epoch_kb"] = -1
+    elif args.drift_epoch:
+        extra["gemm_drift_epoch_kb"] = args.drift_epoch
     if args.fp8:
         extra["fp8_logits"] = 1
     if args.max_ctas:
@@ -806,6 +808,7 @@ def main():
     ap.add_argument("--no-variants", action="store_true", help="do not time the other variant beside the headline")
     ap.add_argument("--no-tile-skip", action="store_true", help="bwd_skip_zero_tiles = off (A/B runs)")
     ap.add_argument("--no-drift-gate", action="store_true", help="gemm_drift_epoch_kb = off (A/B runs)")
+    ap.add_argument("--drift-epoch", type=int, default=0, help="gemm_drift_epoch_kb (A/B runs; 0 = library default 32)")
     ap.add_argument("--max-ctas", type=int, default=0, help="grpo_config.gemm_max_ctas (A/B runs; 0 = every SM)")
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
