@@ -213,6 +213,7 @@ class GrpoContext:
     # ------------------------------------------------------------------ A1
     def grpo_group_advantage(self, rewards, G: int = 0, cu_groups=None, n_groups: Optional[int] = None,
                              want_zero_var: bool = False, stream=None):
+        """A1 - Eq. 1: A_i = (r_i - mean_g) / (std_g + eps_std), one warp per group (include/grpo.h)."""
         S = rewards.numel()
         if n_groups is None:
             n_groups = (cu_groups.numel() - 1) if cu_groups is not None else S // G
@@ -227,6 +228,8 @@ class GrpoContext:
     # ------------------------------------------------------------------ A2 + A3
     def grpo_fused_logprob_loss_fwd(self, hidden, W, targets, cu_seqlens, adv, old_logp, ref_logp=None, mask=None,
                                     loss_denom: float = 0.0, loss_accum=None, metrics_accum=None, stream=None):
+        """A2 + A3 - LM-head contraction with online log-sum-exp, clipped surrogate, optional KL,
+        masked mean (loss mask): returns logp / lse / coeff [T] and the accumulated loss (include/grpo.h)."""
         T, d = hidden.shape
         S = cu_seqlens.numel() - 1
         self.ensure_workspace(T, 1)
@@ -279,6 +282,8 @@ class GrpoContext:
     # ------------------------------------------------------------------ A4 - A6
     def grpo_fused_logprob_loss_bwd(self, hidden, W, targets, lse, coeff, dW_accum=None, grad_scale: float = 1.0,
                                     want_dhidden: bool = True, dhidden_out=None, stream=None):
+        """A4 - A6 - recompute the logits chunk by chunk, dZ = coeff (1[v=y] - p), dH = dZ W, dW += dZ^T H
+        (north_star; accumulation until the update boundary: PAPER.md:111)."""
         T, d = hidden.shape
         self.ensure_workspace(T, 1)
         if want_dhidden and dhidden_out is None:
@@ -400,6 +405,9 @@ class GrpoContext:
 
     def grpo_enqueue_groups(self, groups: Sequence[GroupDesc], W, dW_accum, loss_accum, metrics_accum=None,
                             loss_denom: float = 0.0, streams=None):
+        """A0 + A7 - append complete groups in arrival order and run one logical update of U groups when
+        it is complete, cut into whole-group launches under the token budget; returns
+        (groups consumed so far, update boundary reached)."""
         arr = (GroupDesc * max(len(groups), 1))(*groups)
         sarr, ns = self._streams(streams)
         consumed, boundary = C.c_int32(self._consumed_seen), C.c_int32(0)
@@ -417,6 +425,7 @@ class GrpoContext:
         return consumed.value, bool(boundary.value)
 
     def grpo_flush(self, W, dW_accum, loss_accum, metrics_accum=None, loss_denom: float = 0.0, streams=None):
+        """End of round: run what is pending (< U groups) as a final short update (Alg. 1 l.16-22)."""
         sarr, ns = self._streams(streams)
         consumed, boundary = C.c_int32(self._consumed_seen), C.c_int32(0)
         st = self.lib.grpo_flush(self.h, _dev(W, torch.bfloat16, "W"), _dev(dW_accum, torch.float32, "dW_accum"),
@@ -447,6 +456,8 @@ class GrpoContext:
     def grpo_step_host(self, hidden_h, targets_h, cu_seqlens_h, rewards_h, old_logp_h, n_groups: int, G: int, W,
                        dW_accum, ref_logp_h=None, mask_h=None, loss_denom: float = 0.0, loss_h=None, logp_h=None,
                        dhidden_h=None, stream=None):
+        """A1 - A6 over HOST buffers in one C-ABI call (H2D, compute, D2H pipelined inside the library): what
+        bench.py's e2e leg times."""
         T = hidden_h.shape[0]
         self.ensure_workspace(T, 1)
         if loss_h is None:
