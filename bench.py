@@ -299,6 +299,11 @@ def run_ours(args):
         return run_sweep_T(args, dev)
     # ---- workload: BASELINE.json configs[1]; rank r draws its own complete group (seed r)
     gen_kw = dict(old_sigma=0.3, mask_frac=0.1) if args.off_policy else {}
+    if args.d:
+        gen_kw["d"] = args.d
+    if args.V:
+        gen_kw["V"] = args.V
+    args.informational = bool(args.off_policy or args.d or args.V or args.prenorm or args.fp8 or args.config != 2)
     b = make_config(args.config, seed=rank_seed(rank), device=dev, prenorm=args.prenorm, **gen_kw)
     if args.cgp_mode != "full":
         return run_cgp_stream(args, b, dev, world)
@@ -375,7 +380,7 @@ def run_ours(args):
     # ---- end to end through the C ABI with HOST buffers (grpo_step_host): H2D + compute + D2H per step.  Timed
     # right after the headline region so that both see the same thermal / power state of the board.
     e2e_s, h2d, d2h = 0.0, 0, 0
-    if args.config == 2 and not args.prenorm and not args.fp8 and not args.off_policy:
+    if not args.informational:
         pin = lambda t: None if t is None else t.cpu().pin_memory()
         h_hidden, h_targets, h_cu, h_rewards, h_old = (pin(b.hidden), pin(b.targets), pin(b.cu_seqlens), pin(b.rewards),
                                                        pin(b.old_logp))
@@ -459,7 +464,7 @@ def run_ours(args):
                               "ms_per_step": v_ms / args.steps}
 
     # ---- informational runs (--config 3/4/5, --prenorm) are device-resident: no e2e / cpu_baseline legs
-    if args.config != 2 or args.prenorm or args.fp8 or args.off_policy:
+    if args.informational:
         ms_total, _, tokens_all = reduce_over_ranks(ms_total, 0.0, T, world, dev)
         if rank == 0:
             line = build_line(args, b, world, tokens_all * args.steps / (ms_total * 1e-3), ms_total, None, 0, 0,
@@ -756,7 +761,9 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "e4m3 (A2, A4 operands) + bf16" if getattr(args, "fp8", False) else "bf16", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config] + (" (informational: --off-policy, old log-prob noise 0.3, "
-                                                         "10 % of the tokens masked)" if args.off_policy else ""),
+                                                         "10 % of the tokens masked)" if args.off_policy else "")
+                               + (f" (informational: d = {d}, V = {V} instead of the Qwen3-1.7B head)"
+                                  if (args.d or args.V) else ""),
                    "variant": "fp8_logits (informational PRECISION STUDY, NEXT-4: e4m3 operands for A2 / A4; does not meet "
                    "north_star's log-prob tolerance)" if args.fp8 else "prenorm (informational, NEXT-4): RMSNorm fwd + north_star path + RMSNorm bwd fused behind A5"
                    if args.prenorm else "stash_logits (3 contractions, DESIGN.md section 11)" if args.stash
@@ -801,6 +808,8 @@ def main():
     ap.add_argument("--fp8", action="store_true",
                     help="informational precision study (NEXT-4): grpo_config.fp8_logits = 1 (e4m3 operands for the two "
                          "logit contractions); no e2e / cpu_baseline legs")
+    ap.add_argument("--d", type=int, default=0, help="informational: another hidden width (the workload's recipe otherwise)")
+    ap.add_argument("--V", type=int, default=0, help="informational: another vocabulary size")
     ap.add_argument("--off-policy", action="store_true",
                     help="informational: the workload in the off-policy regime of config 1b (old log-prob noise 0.3: "
                          "20-40 %% of the tokens clipped; 10 %% masked; no KL), whose zero-coefficient rows the backward "

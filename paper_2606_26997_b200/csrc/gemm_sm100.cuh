@@ -65,6 +65,12 @@ struct GemmParams {
   int m_total, n_total;              // valid rows / cols of C
   int m_tiles, n_tiles, k_blocks;
   int n_fastest;                     // unit order: 1 = n tile fastest (A5/A6), 0 = m tile fastest (A2/A4)
+  // L2 working-set bounds of the unit ORDER (never of a reduction: results do not depend on them).  n_fastest = 1:
+  // the n tiles are walked in groups of n_group (all m tiles of a group before the next group), so that the B
+  // panels a wave re-reads from L2 - A6: the chunk's hidden-state columns - stay what they are at d = 2048 when d
+  // is larger.  n_fastest = 0: the m tiles are walked in blocks of m_block (all n tiles of a block before the next
+  // block; A4: the block's hidden-state rows stay L2-resident while W streams).  0 = one group / block.
+  int n_group, m_block;
   // EPI_LSE: a unit is (m tile, contiguous range of n tiles).  The vocab split is a function of V ALONE (never of
   // the launch's row count), so a token's log-sum-exp is summed in the same order whatever launch it is part of
   // (batch invariance).  Units are walked in blocks of `lse_block` m tiles (= CTA pairs of the
@@ -172,12 +178,20 @@ __device__ __forceinline__ Unit unit_to_tiles(const GemmParams& p, const Extent&
     t.kb1 = min(e.k_blocks, t.kb0 + p.kb_per_split);
   }
   int m_idx;
-  if (p.n_fastest) {
-    t.n0 = u % p.n_tiles;
-    m_idx = u / p.n_tiles;
-  } else {
-    m_idx = u % e.m_tiles;
-    t.n0 = u / e.m_tiles;
+  if (p.n_fastest) {                                      // groups of n tiles; inside a group: m tile, then n tile fastest
+    const int ng = p.n_group > 0 ? min(p.n_group, p.n_tiles) : p.n_tiles;
+    const int per_group = ng * e.m_tiles;                 // only the last group can be short
+    const int g = u / per_group, r = u - g * per_group;
+    const int gsz = min(ng, p.n_tiles - g * ng);
+    m_idx = r / gsz;
+    t.n0 = g * ng + (r - m_idx * gsz);
+  } else {                                                // blocks of m tiles; inside a block: n tile, then m tile fastest
+    const int mb = p.m_block > 0 ? min(p.m_block, e.m_tiles) : e.m_tiles;
+    const int per_block = mb * p.n_tiles;                 // only the last block can be short
+    const int b = u / per_block, r = u - b * per_block;
+    const int bsz = min(mb, e.m_tiles - b * mb);
+    t.n0 = r / bsz;
+    m_idx = b * mb + (r - t.n0 * bsz);
   }
   t.n1 = t.n0 + 1;
   t.m_tile = m_idx;

@@ -155,6 +155,14 @@ static int64_t chunk_tokens(const grpo_config& c) { return c.bwd_chunk_tokens > 
 // of (batch invariance: CGP changes "only group dispatch timing and order - not samples, advantages, or gradient
 // computation").  Load balance comes from the ORDER the units are walked in, never from re-cutting
 // a reduction.
+// L2 working-set bounds of the unit orders (gemm_sm100.cuh: n_group / m_block / lse_block; results never depend on
+// them).  Chosen so that d = 2048 walks its units exactly as it always has and wider models keep a comparable L2
+// footprint.  DRAM reads per launch at d = 4096, T = 16-19k: A2 68 GB without a bound, 28 GB with 80 MB blocks, 10 with
+// 56 MB, 8 with 40 MB (algorithmic 1.4; step time best at 56 MB); A4 10 GB -> 4; A6 18 GB -> 12.
+static const int64_t kA2AllBytes = 80ll << 20;     // A2: every pair its own token tile while their rows fit in this ...
+static const int64_t kA2BlockBytes = 56ll << 20;   // ... else blocks of token tiles of this many bytes of hidden state
+static const int64_t kA4BlockBytes = 40ll << 20;   // A4 blocks (A4 also streams the dZ chunk out through L2)
+static const int kNGroupTiles = 8;                 // A5 / A6: d tiles (256 columns) walked together (2048 columns)
 static const int kLseTilesPerSplit = 8;      // 256-column vocab tiles per A2 unit (2048 logits)
 static const int kDhKSplit = 4;              // K ranges of A5 (K = V)
 static void lse_split(int V, int* n_split, int* tiles_per_split) {
@@ -308,7 +316,12 @@ static int32_t launch_gemm_cg(grpo_ctx* ctx, int kind, const CUtensorMap& tmA, c
   const int ctas = ctx->cfg.gemm_max_ctas > 0 ? std::min(ctx->cfg.gemm_max_ctas, ctx->num_sms) : ctx->num_sms;
   const int grid = CG * std::min(n_units, std::max(ctas / CG, 1));
   GemmParams pl = p;
+  // A2 walks its units in blocks of lse_block token tiles whose hidden-state rows stay L2-resident while W streams:
+  // every pair of the grid gets its own token tile as long as those rows fit (80 MB: 74 tiles at d = 2048)
+  const int64_t m_tile_bytes = static_cast<int64_t>(BM) * CG * ctx->cfg.d * 2;
   pl.lse_block = grid / CG;
+  if (pl.lse_block * m_tile_bytes > kA2AllBytes)
+    pl.lse_block = static_cast<int>(std::max<int64_t>(1, kA2BlockBytes / m_tile_bytes));
   // drift gate (gemm_sm100.cuh): epoch counters live in the launch's workspace slot, zeroed on the stream
   const int xsync = ctx->cfg.gemm_drift_epoch_kb == 0 ? 32 : ctx->cfg.gemm_drift_epoch_kb;
   pl.sync_lag = 1;   // epochs a pair may lead the slowest pair by (2-8 measured: no different from 1)
@@ -982,6 +995,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_total = static_cast<int>(rows); p.n_total = c.V;
       p.m_tiles = m_tiles; p.n_tiles = (c.V + BN - 1) / BN; p.k_blocks = (c.d + BK - 1) / BK;
       p.n_fastest = 0;
+      p.m_block = static_cast<int>(std::max<int64_t>(1, kA4BlockBytes / (static_cast<int64_t>(TM) * c.d * 2)));
       p.row_offset = row_off; p.targets = y_c;
       p.scale_log2e = c.logit_scale * kLog2e; p.logit_scale = c.logit_scale;
       p.lse = lse_c; p.coeff = coeff_c; p.coeff_mul = c.logit_scale * grad_scale;
@@ -1009,7 +1023,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       std::memset(&p, 0, sizeof(p));
       p.m_total = static_cast<int>(rows); p.n_total = c.d;
       p.m_tiles = m_tiles; p.n_tiles = (c.d + BN - 1) / BN; p.k_blocks = (c.V + BK - 1) / BK;
-      p.n_fastest = 1;
+      p.n_fastest = 1; p.n_group = kNGroupTiles;
       p.k_split = k_split; p.kb_per_split = kb_per_split; p.c_split_stride = L.chunk_rows * c.d;
       p.c_out = dh_part; p.c_pitch = c.d;
       p.dyn_rows = dyn_rows;
@@ -1046,7 +1060,7 @@ static int32_t bwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
       p.m_total = c.V; p.n_total = c.d;
       p.m_tiles = (c.V + TM - 1) / TM; p.n_tiles = (c.d + BN - 1) / BN;
       p.k_blocks = static_cast<int>((rows + BK - 1) / BK);
-      p.n_fastest = 1;
+      p.n_fastest = 1; p.n_group = kNGroupTiles;
       p.c_out = dW_accum; p.c_pitch = c.d; p.dyn_rows = dyn_rows;
       p.sync = slot_ptr<unsigned int>(ctx, slot, L.off_sync);
       CUtensorMap tmDW;

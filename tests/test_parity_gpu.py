@@ -293,3 +293,13 @@ def test_step_is_cuda_graph_capturable():
         assert torch.equal(f["logp"], ref[3])
     assert ctx.grpo_check_errors_sync() == 0
     ctx.close()
+
+
+# ------------------------------------------------------------------ wide hidden sizes: L2-bounded unit orders
+def test_wide_hidden_size_walks_its_units_in_l2_sized_groups():
+    """d = 4352 (17 d tiles: the A5 / A6 units are walked in groups of 8, 8 and 1 tiles; 2.2 MB of hidden state per
+    token tile: A2 blocks of 25 and A4 blocks of 17 token tiles, the last ones short) with T ~ 11k tokens (43 token
+    tiles): only the ORDER of the units changes with these bounds, so the gates are the usual ones."""
+    b = make_config(4, device="cuda", seed=2, d=4352, V=1500, len_div=38.0, w_std=0.05, old_sigma=0.3, mask_frac=0.1)
+    assert b.T > 9500
+    _check(b)
