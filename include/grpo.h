@@ -166,6 +166,42 @@ int32_t grpo_loss_from_partials(grpo_ctx* ctx, int32_t n_shards, const float* m2
                                 double loss_denom, float* logp_out, float* lse_out, float* coeff_out, float* loss_accum,
                                 float* metrics_accum, void* stream);
 
+/* ---- A3 for callers that must not allocate -----------------------------------------------------------------
+ * Everything above needs a context (grpo_create calls cudaMalloc / cudaMallocHost) and a workspace the caller has to
+ * allocate.  Some callers cannot do either at the point where they need the loss: a trainer whose framework has
+ * already handed the whole of HBM to its own caching allocator (a raw cudaMalloc then fails, or takes memory the
+ * framework counts on), a step running while the decode side of the same process overlaps rollouts on other streams
+ * (cudaMalloc / cudaFree synchronise the device and stall them; PAPER.md:92-111 is about keeping exactly that
+ * overlap), a loss-only rank of a vocab-parallel job that holds no vocab shard and would otherwise size a workspace
+ * for contractions it never runs, or a plug-in that is only ever given input and output pointers.
+ *
+ * grpo_loss_from_partials_static is grpo_loss_from_partials (same kernels, same arithmetic, same argument meaning)
+ * with NO context and NO workspace: the switches come from *cfg (HOST; read during the call: clip_lo, clip_hi,
+ * kl_beta, kl_type, dual_clip, loss_agg), S_norm replaces grpo_set_seq_denom (loss_agg 1: sequences of the whole
+ * logical update, 0 = this call's S), and the kernel's scratch - block sums and arrival counter of the fixed-order
+ * loss reduction, the token counts that define the mean, 336 KiB in all - is an array compiled into the library.
+ * Every GPU that loads the library holds that array until the process exits.  The call runs no cudaMalloc, cudaFree,
+ * cudaMallocHost or any other allocating routine; inputs and outputs are the caller's, as everywhere else.
+ *
+ * Limits: T <= GRPO_STATIC_MAX_TOKENS and S <= GRPO_STATIC_MAX_SEQUENCES, otherwise GRPO_ERR_WORKSPACE and nothing
+ * is launched (cut the update into several calls with an explicit loss_denom / S_norm, or use the workspace path).
+ * First call on a device: looks the array's device address up once (with that device current) and checks the arch;
+ * make that first call outside any stream capture.  Later calls on that device only enqueue work on `stream`.
+ * Sharing: there is ONE array per GPU, shared by every caller and every stream in the process, and it keeps the last
+ * call's contents (the call clears the words that must start at zero).  Two calls whose work overlaps on the same
+ * GPU race on it and give wrong loss / metrics sums: order them on one stream or with events.
+ * err_flags: device int32 [1] or NULL; bit 0 is OR-ed in when a target id >= V_global is seen (such tokens are
+ * ignored, as in the forward); with NULL the condition is not reported.  The caller clears the word. */
+#define GRPO_STATIC_MAX_TOKENS 1048576
+#define GRPO_STATIC_MAX_SEQUENCES 65536
+int32_t grpo_loss_from_partials_static(const grpo_config* cfg /*HOST*/, int32_t n_shards, const float* m2,
+                                       const float* s2, const float* zy, const int32_t* targets, int32_t V_global,
+                                       const int32_t* cu_seqlens, int32_t S, int32_t S_norm, int64_t T,
+                                       const float* adv, const float* old_logp, const float* ref_logp,
+                                       const uint8_t* mask, double loss_denom, float* logp_out, float* lse_out,
+                                       float* coeff_out, float* loss_accum, float* metrics_accum, int32_t* err_flags,
+                                       void* stream);
+
 /* A4-A6.  lse, coeff from the forward.  grad_scale multiplies both gradients (upstream dLoss).
  * dhidden_out [T, d] (bf16, or fp32 if cfg.dhidden_fp32) is OVERWRITTEN; dW_accum fp32 [V, d] is
  * ADDED to with atomics (caller zeroes it at the optimizer boundary).  Either may be NULL to skip. */

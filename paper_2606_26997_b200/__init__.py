@@ -5,5 +5,5 @@ ctypes binding.  Importing the package does not load the library; using it witho
 library raises (no CPU / PyTorch fallback exists).
 """
 from .binding import (GrpoConfig, GrpoContext, GrpoError, GroupDesc, EXPORTS, grpo_cgp_plan,  # noqa: F401
-                      load_library)
+                      grpo_loss_from_partials_static, load_library)
 from .build import build, LIB_PATH  # noqa: F401

@@ -22,7 +22,7 @@ EXPORTS = [
     "grpo_set_workspace", "grpo_group_advantage", "grpo_fused_logprob_loss_fwd", "grpo_fused_logprob_loss_bwd",
     "grpo_fused_logprob_loss_fwd_bwd", "grpo_set_entropy_out", "grpo_set_seq_denom", "grpo_bwd_row_stats_sync",
     "grpo_rmsnorm_fwd", "grpo_rmsnorm_bwd", "grpo_fused_logprob_loss_bwd_prenorm", "grpo_debug_max_active_clusters",
-    "grpo_vocab_shard_partials", "grpo_loss_from_partials",
+    "grpo_vocab_shard_partials", "grpo_loss_from_partials", "grpo_loss_from_partials_static",
     "grpo_shard_granularity", "grpo_shard_create", "grpo_shard_import", "grpo_shard_release", "grpo_stitch_map",
     "grpo_stitch_unmap",
     "grpo_enqueue_groups", "grpo_flush", "grpo_queue_state", "grpo_reset_round", "grpo_cgp_plan",
@@ -108,6 +108,8 @@ def load_library() -> C.CDLL:
     lib.grpo_vocab_shard_partials.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     lib.grpo_loss_from_partials.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, i32, i64, vp, vp, vp, vp, f64, vp, vp, vp,
                                             vp, vp, vp]
+    lib.grpo_loss_from_partials_static.argtypes = [C.POINTER(GrpoConfig), i32, vp, vp, vp, vp, i32, vp, i32, i32, i64,
+                                                   vp, vp, vp, vp, f64, vp, vp, vp, vp, vp, vp, vp]
     lib.grpo_debug_max_active_clusters.argtypes = [vp, i32, C.POINTER(i32)]
     lib.grpo_rmsnorm_fwd.argtypes = [vp, vp, vp, f32, i64, vp, vp, vp]
     lib.grpo_rmsnorm_bwd.argtypes = [vp, vp, vp, vp, vp, i32, i64, vp, vp, vp]
@@ -155,6 +157,44 @@ def grpo_cgp_plan(group_tokens: Sequence[int], U: int, token_budget: int = 0, fl
     nl = C.c_int32(0)
     _check(lib.grpo_cgp_plan(arr, n, U, token_budget, int(flush), out, max(n, 1), C.byref(nl)))
     return [out[i] for i in range(nl.value)]
+
+
+STATIC_MAX_TOKENS = 1048576        # GRPO_STATIC_MAX_TOKENS / GRPO_STATIC_MAX_SEQUENCES of include/grpo.h
+STATIC_MAX_SEQUENCES = 65536
+
+
+def grpo_loss_from_partials_static(m2, s2, zy, targets, V_global: int, cu_seqlens, adv, old_logp, out, ref_logp=None,
+                                   mask=None, loss_denom: float = 0.0, S_norm: int = 0, err_flags=None, stream=None,
+                                   **switches):
+    """A3 on gathered vocab-shard partials for callers that cannot allocate GPU memory where they need the loss
+    (include/grpo.h, "A3 for callers that must not allocate"): no GrpoContext, no workspace - the kernel's scratch is
+    an array built into libgrpo_b200.so - and this function creates no tensor either.  A framework that has given all
+    of HBM to its own allocator, a step whose neighbouring streams must not be stalled by cudaMalloc's device
+    synchronisation, or a loss-only rank without a vocab shard can call it with buffers it already owns.
+
+    `out` holds the caller's buffers: logp / lse / coeff fp32 [T], loss fp32 [1] (ADDED to), optionally metrics
+    fp32 [4] (ADDED to).  `switches` are grpo_config fields (clip_lo, clip_hi, kl_beta, kl_type, dual_clip, loss_agg).
+    T <= STATIC_MAX_TOKENS and S <= STATIC_MAX_SEQUENCES, else GrpoError(GRPO_ERR_WORKSPACE).  All calls on one GPU
+    share the built-in array: keep them ordered on one stream (or by events); calls that overlap on the GPU race."""
+    lib = load_library()
+    cfg = GrpoConfig()
+    _check(lib.grpo_default_config(C.byref(cfg)))
+    for k, v in switches.items():
+        if not hasattr(cfg, k):
+            raise AttributeError(f"grpo_config has no field {k}")
+        setattr(cfg, k, v)
+    n_shards, T = m2.shape
+    S = cu_seqlens.numel() - 1
+    _check(lib.grpo_loss_from_partials_static(
+        C.byref(cfg), n_shards, _dev(m2, torch.float32, "m2", n_shards * T), _dev(s2, torch.float32, "s2", n_shards * T),
+        _dev(zy, torch.float32, "zy", n_shards * T), _dev(targets, torch.int32, "targets", T), int(V_global),
+        _dev(cu_seqlens, torch.int32, "cu_seqlens"), S, int(S_norm), T, _dev(adv, torch.float32, "adv", S),
+        _dev(old_logp, torch.float32, "old_logp", T), _dev(ref_logp, torch.float32, "ref_logp", T),
+        _dev(mask, torch.uint8, "mask", T), float(loss_denom), _dev(out["logp"], torch.float32, "logp", T),
+        _dev(out["lse"], torch.float32, "lse", T), _dev(out["coeff"], torch.float32, "coeff", T),
+        _dev(out["loss"], torch.float32, "loss", 1), _dev(out.get("metrics"), torch.float32, "metrics", 4),
+        _dev(err_flags, torch.int32, "err_flags", 1), _stream(stream)))
+    return out
 
 
 class GrpoContext:

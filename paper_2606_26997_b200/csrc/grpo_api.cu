@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstring>
 #include <deque>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1606,4 +1607,109 @@ extern "C" int32_t grpo_debug_gemm(grpo_ctx* ctx, int32_t layout, const void* A,
     return launch_gemm<true, true, EPI_STORE>(ctx, GRPO_KERNEL_DEBUG, tmA, tmB, p, units, st);
   }
   return fail(GRPO_ERR_INVALID_ARG, "layout must be 0, 1 or 2");
+}
+
+// ------------------------------------------------------------------------------------- A3 without any allocation
+// grpo_loss_from_partials_static (include/grpo.h): the A3 launch of grpo_loss_from_partials with its scratch - the
+// per-block partial sums and arrival counter of the fixed-order loss reduction, the loss-bearing token counts that
+// define the mean - in an array that is part of the library image instead of a context's workspace slot.
+// Layout of the array (bytes): [0, 256) header {u32 arrival counter, f32 total token count, i32 unread error word};
+// then 5 floats per 256-token block; then one float per sequence.
+namespace {
+constexpr int64_t kStaticMaxBlocks = (GRPO_STATIC_MAX_TOKENS + 255) / 256;
+constexpr int64_t kStaticOffPart = 256;
+constexpr int64_t kStaticOffSeq = kStaticOffPart + kStaticMaxBlocks * 5 * 4;
+constexpr int64_t kStaticBytes = kStaticOffSeq + static_cast<int64_t>(GRPO_STATIC_MAX_SEQUENCES) * 4;
+constexpr int kStaticMaxDevices = 64;
+}  // namespace
+
+// Every GPU that loads the library carries one copy of this array until the process exits.
+static __device__ __align__(256) unsigned char g_static_loss_scratch[kStaticBytes];
+
+// In host code `g_static_loss_scratch` is only a handle for the runtime's symbol table, never a device address: the
+// address on the CURRENT device comes from cudaGetSymbolAddress, asked once per device and remembered here.
+static void* g_static_scratch_addr[kStaticMaxDevices] = {nullptr};
+static std::mutex g_static_scratch_mutex;
+
+static int32_t static_scratch_for_current_device(uint8_t** out) {
+  int dev = 0;
+  CU_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(GRPO_ERR_INVALID_ARG, "device ordinal %d not supported", dev);
+  std::lock_guard<std::mutex> guard(g_static_scratch_mutex);
+  void* p = g_static_scratch_addr[dev];
+  int32_t status = GRPO_OK;
+  if (p == nullptr) {   // first call on this device: set-up (do it before any stream capture)
+    int major = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) status = fail(GRPO_ERR_CUDA, "cudaDeviceGetAttribute failed: %s", cudaGetErrorString(e));
+    else if (major != 10) status = fail(GRPO_ERR_ARCH, "device %d is sm_%dx; this library is built for sm_100a only", dev, major);
+    else {
+      e = cudaGetSymbolAddress(&p, g_static_loss_scratch);
+      if (e != cudaSuccess || p == nullptr)
+        status = fail(GRPO_ERR_CUDA, "cudaGetSymbolAddress(g_static_loss_scratch) failed on device %d: %s", dev,
+                      cudaGetErrorString(e));
+      else g_static_scratch_addr[dev] = p;
+    }
+  }
+  if (status != GRPO_OK) return status;
+  *out = static_cast<uint8_t*>(p);
+  return GRPO_OK;
+}
+
+extern "C" int32_t grpo_loss_from_partials_static(const grpo_config* cfg, int32_t n_shards, const float* m2,
+                                                  const float* s2, const float* zy, const int32_t* targets,
+                                                  int32_t V_global, const int32_t* cu_seqlens, int32_t S,
+                                                  int32_t S_norm, int64_t T, const float* adv, const float* old_logp,
+                                                  const float* ref_logp, const uint8_t* mask, double loss_denom,
+                                                  float* logp_out, float* lse_out, float* coeff_out, float* loss_accum,
+                                                  float* metrics_accum, int32_t* err_flags, void* stream) {
+  if (!cfg || !m2 || !s2 || !zy || !targets || !cu_seqlens || !adv || !old_logp || !logp_out || !lse_out || !coeff_out ||
+      !loss_accum)
+    return fail(GRPO_ERR_INVALID_ARG, "a required pointer is NULL");
+  if (n_shards < 1 || V_global < 1 || T <= 0 || S <= 0) return fail(GRPO_ERR_SHAPE, "need n_shards, V_global, T, S > 0");
+  if (T > GRPO_STATIC_MAX_TOKENS)
+    return fail(GRPO_ERR_WORKSPACE, "T=%lld exceeds GRPO_STATIC_MAX_TOKENS=%d: the built-in scratch array holds no more; "
+                "cut the call or use grpo_loss_from_partials with a workspace", (long long)T, GRPO_STATIC_MAX_TOKENS);
+  if (S > GRPO_STATIC_MAX_SEQUENCES)
+    return fail(GRPO_ERR_WORKSPACE, "S=%d exceeds GRPO_STATIC_MAX_SEQUENCES=%d: the built-in scratch array holds no more; "
+                "cut the call or use grpo_loss_from_partials with a workspace", S, GRPO_STATIC_MAX_SEQUENCES);
+  if (S_norm != 0 && S_norm < S) return fail(GRPO_ERR_INVALID_ARG, "S_norm=%d is smaller than this call's S=%d", S_norm, S);
+  if (cfg->loss_agg != 0 && cfg->loss_agg != 1) return fail(GRPO_ERR_INVALID_ARG, "loss_agg must be 0 or 1");
+  if (cfg->kl_type < 0 || cfg->kl_type > 2 || (cfg->dual_clip != 0.f && !(cfg->dual_clip > 1.f)))
+    return fail(GRPO_ERR_INVALID_ARG, "kl_type must be 0, 1 or 2 and dual_clip 0 or > 1");
+  uint8_t* scratch = nullptr;
+  GRPO_TRY(static_scratch_for_current_device(&scratch));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  unsigned int* block_count = reinterpret_cast<unsigned int*>(scratch);
+  float* total = reinterpret_cast<float*>(scratch + 4);
+  int32_t* err_word = err_flags ? err_flags : reinterpret_cast<int32_t*>(scratch + 8);
+  float* block_part = reinterpret_cast<float*>(scratch + kStaticOffPart);
+  float* seq_count = reinterpret_cast<float*>(scratch + kStaticOffSeq);
+  // the array keeps what the previous call left: the arrival counter and the token total must start at zero (the
+  // block sums and per-sequence counts are written before they are read)
+  CU_OK(cudaMemsetAsync(scratch, 0, 16, st));
+  const bool implicit_denom = cfg->loss_agg == 0 && !(loss_denom > 0.0);
+  if (cfg->loss_agg == 1 || implicit_denom) {
+    const int threads = 128;
+    const int blocks = static_cast<int>((static_cast<int64_t>(S) * 32 + threads - 1) / threads);
+    token_count_kernel<<<blocks, threads, 0, st>>>(mask, targets, V_global, cu_seqlens, S, seq_count, total);
+    CU_OK(cudaGetLastError());
+  }
+  LossParams lp;
+  std::memset(&lp, 0, sizeof(lp));
+  lp.T = T; lp.t_begin = 0; lp.S = S; lp.S_norm = S_norm > 0 ? S_norm : S; lp.V = V_global;
+  lp.n_split = n_shards; lp.part_stride = T;
+  lp.part_m = m2; lp.part_s = s2; lp.zy = zy; lp.n_zy = n_shards; lp.zy_stride = T;
+  lp.targets = targets; lp.cu_seqlens = cu_seqlens; lp.adv = adv; lp.old_logp = old_logp; lp.ref_logp = ref_logp;
+  lp.mask = mask; lp.seq_count = seq_count; lp.total_count = total;
+  lp.denom_host = loss_denom > 0.0 ? static_cast<float>(loss_denom) : 0.f;
+  lp.loss_agg = cfg->loss_agg; lp.clip_lo = cfg->clip_lo; lp.clip_hi = cfg->clip_hi; lp.kl_beta = cfg->kl_beta;
+  lp.kl_type = cfg->kl_type; lp.dual_clip = cfg->dual_clip;
+  lp.logp = logp_out; lp.lse = lse_out; lp.coeff = coeff_out; lp.loss_accum = loss_accum;
+  lp.metrics_accum = metrics_accum; lp.err_flag = err_word;
+  lp.block_part = block_part; lp.block_count = block_count;
+  const int blocks = static_cast<int>((T + 255) / 256);
+  loss_epilogue_kernel<<<blocks, 256, 0, st>>>(lp);
+  CU_OK(cudaGetLastError());
+  return GRPO_OK;
 }
