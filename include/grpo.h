@@ -140,8 +140,10 @@ int32_t grpo_fused_logprob_loss_fwd(grpo_ctx* ctx, const void* hidden, const voi
 
 /* loss_agg = 1 only (per-sequence mean, then mean over sequences): the number of sequences of the WHOLE logical
  * update that later grpo_fused_logprob_loss_fwd / _fwd_bwd calls of this context divide by, for callers that cut
- * one update into several calls (micro-batches); 0 (default) = each call's own S.  grpo_enqueue_groups does not
- * use it: it counts the sequences of the update's groups itself (R10). */
+ * one update into several calls (micro-batches); 0 (default) = each call's own S.  grpo_enqueue_groups / grpo_flush
+ * count the sequences of the update's groups themselves (R10) while this is 0; a data-parallel rank, which
+ * holds only its share of the update's groups, sets the update's GLOBAL sequence count here before it enqueues
+ * them (an update with more local sequences than the stated count is GRPO_ERR_INVALID_ARG and nothing runs). */
 int32_t grpo_set_seq_denom(grpo_ctx* ctx, int32_t n_sequences);
 
 /* ---- NEXT-3(b): vocab-parallel (tensor-parallel) forward -------------------------

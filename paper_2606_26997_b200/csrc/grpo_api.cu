@@ -1371,6 +1371,14 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
       pos += k;
     }
     for (const auto& g : upd) S_update += g.desc.G;
+    // data parallelism (loss_agg 1): this rank holds only its share of the update's groups; the per-sequence mean
+    // still averages over the sequences of the WHOLE update, which the caller states with grpo_set_seq_denom
+    if (ctx->cfg.loss_agg == 1 && ctx->seq_denom > 0) {
+      if (ctx->seq_denom < S_update)
+        return fail(GRPO_ERR_INVALID_ARG, "grpo_set_seq_denom(%d) is smaller than the %d sequences of this update",
+                    ctx->seq_denom, S_update);
+      S_update = ctx->seq_denom;
+    }
   }
 
   // implicit denominator of the whole update: count loss-bearing tokens of all its groups first

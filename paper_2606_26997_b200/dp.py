@@ -3,7 +3,8 @@
 Complete groups are independent units of work, and the paper's trainer ran DP = 2.
 A logical update of U groups is dealt to the ranks by arrival position (group k of the update ->
 rank k mod world); every rank runs A1-A6 on its groups through ``grpo_enqueue_groups`` with the denominator of the
-WHOLE update (R10), accumulating into its local fp32 ``dW`` / loss; at the update boundary ONE sum
+WHOLE update (R10: ``loss_denom=global_denominator(...)`` for the token mean; for ``loss_agg = 1``
+``ctx.grpo_set_seq_denom(global_sequences(...))`` before enqueueing), accumulating into its local fp32 ``dW`` / loss; at the update boundary ONE sum
 all-reduce of ``dW`` (1.245 GB at the Qwen3-1.7B head) plus the scalars gives every rank the full-update gradient:
 by the additivity of the step over groups (P12) the result equals the single-rank full-batch step up to fp32
 summation order.
@@ -11,8 +12,9 @@ summation order.
 The all-reduce is issued on a side stream behind an event of the compute stream and returns immediately, so it
 overlaps with the next update's contractions, which accumulate into the OTHER of two gradient buffers
 (``buffers()`` hands them out alternately).  ``torch.distributed`` is plumbing only (NCCL over NVLink 5 on the GPU
-box; gloo in the CPU tests): no arithmetic of the method lives here.  Nothing in this module was timed on more than
-one GPU (none is reachable from this build); DESIGN.md section 7 says so.
+box; gloo in the CPU tests): no arithmetic of the method lives here.  Every branch has run on ONE GPU (a one-rank
+NCCL group, tests/test_dp_gpu.py); nothing in this module has run or been timed on more than one GPU (none is
+reachable from this build); DESIGN.md section 7 says so.
 """
 from __future__ import annotations
 
@@ -48,8 +50,14 @@ class BoundaryHandle:
 
 
 class GrpoDataParallel:
-    def __init__(self, process_group=None, comm_stream: Optional["torch.cuda.Stream"] = None):
+    """always_reduce: issue the collectives even when the group has ONE rank (they are then identities).  A single
+    GPU can host a one-rank NCCL group, so this is how the CUDA / NCCL branches below are executed where no second
+    GPU is reachable (tests/test_dp_gpu.py); leave it off in production."""
+
+    def __init__(self, process_group=None, comm_stream: Optional["torch.cuda.Stream"] = None,
+                 always_reduce: bool = False):
         self.pg = process_group
+        self.always_reduce = always_reduce
         self.world = dist.get_world_size(process_group) if dist.is_initialized() else 1
         self.rank = dist.get_rank(process_group) if dist.is_initialized() else 0
         self._comm_stream = comm_stream
@@ -63,7 +71,7 @@ class GrpoDataParallel:
     def global_denominator(self, local_loss_tokens: int) -> float:
         """Loss-bearing tokens of the WHOLE update (token-mean denominator, R10): sum over ranks of the
         local counts (host integers: the sequence lengths are host data in the CGP handoff)."""
-        if self.world == 1:
+        if self.world == 1 and not self.always_reduce:
             return float(local_loss_tokens)
         t = torch.tensor([float(local_loss_tokens)], dtype=torch.float64)
         if dist.get_backend(self.pg) == "nccl":
@@ -99,7 +107,7 @@ class GrpoDataParallel:
         the next update's kernels run concurrently.  CPU tensors (gloo tests): asynchronous works."""
         tensors = [t for t in (dW_accum, loss_accum, metrics_accum) if t is not None]
         h = BoundaryHandle()
-        if self.world == 1:
+        if self.world == 1 and not self.always_reduce:
             return h
         if dW_accum.is_cuda:
             if self._comm_stream is None:
@@ -126,12 +134,46 @@ class _RawCudaBuffer:
         self.__cuda_array_interface__ = {"shape": (n_float32,), "typestr": "<f4", "data": (ptr, False), "version": 2}
 
 
+def _node_identity() -> str:
+    """Something every process on one machine agrees on, containers included (the kernel's boot id), else the
+    hostname."""
+    try:
+        with open("/proc/sys/kernel/random/boot_id") as f:
+            return f.read().strip()
+    except OSError:
+        return socket.gethostname()
+
+
+def _require_one_node(dp: "GrpoDataParallel", identity: Optional[str] = None, device: Optional[int] = None):
+    """The stitched accumulator needs (1) every rank on ONE machine - shard handles travel as file descriptors over
+    Unix sockets - and (2) peer access between the ranks' GPUs, since the A6 reduce-adds are NVLink stores into the
+    peers' memory.  Raises on EVERY rank (the facts are all-gathered) instead of hanging in connect() or faulting in
+    the kernel.  GPUs hidden behind per-rank CUDA_VISIBLE_DEVICES all read as device 0 here and cannot be checked:
+    cuMemSetAccess in grpo_stitch_map then reports the missing access."""
+    if device is None:
+        device = torch.cuda.current_device() if torch.cuda.is_available() else -1
+    me = (identity if identity is not None else _node_identity(), int(device))
+    everyone = [None] * dp.world
+    dist.all_gather_object(everyone, me, group=dp.pg)
+    nodes = sorted({n for n, _ in everyone})
+    if len(nodes) > 1:
+        raise RuntimeError(f"StitchedGradient needs all {dp.world} ranks on one node (shard handles are POSIX file "
+                           f"descriptors passed over Unix sockets); the group spans {len(nodes)} nodes. Use "
+                           "GrpoDataParallel.reduce_boundary (all-reduce) across nodes.")
+    if me[1] >= 0:
+        for r, (_, dev_r) in enumerate(everyone):
+            if r != dp.rank and dev_r >= 0 and dev_r != me[1] and not torch.cuda.can_device_access_peer(me[1], dev_r):
+                raise RuntimeError(f"StitchedGradient: GPU {me[1]} (rank {dp.rank}) has no peer access to GPU {dev_r} "
+                                   f"(rank {r}); the stitched accumulator needs NVLink / P2P between all ranks.")
+
+
 def _exchange_fds(own_fd: int, dp: "GrpoDataParallel") -> List[int]:
     """Every rank's exported shard descriptor, by rank (own at dp.rank).  POSIX file descriptors only cross process
     boundaries as SCM_RIGHTS ancillary data: every rank serves its descriptor on a Unix socket, then fetches the
-    others'."""
+    others'.  One node only: checked first (_require_one_node)."""
     if dp.world == 1:
         return [own_fd]
+    _require_one_node(dp)
     tag = [uuid.uuid4().hex if dp.rank == 0 else None]
     dist.broadcast_object_list(tag, src=0, group=dp.pg)
     path = lambda r: f"/tmp/grpo_stitch_{tag[0]}_{r}.sock"

@@ -92,3 +92,36 @@ def test_single_process_is_identity():
     dp.reduce_boundary(t, torch.ones(1)).wait()
     assert torch.equal(t, torch.ones(4, 2))
     assert [assign_groups(7, 3, r) for r in range(3)] == [[0, 3, 6], [1, 4], [2, 5]]
+
+
+def _node_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2606_26997_b200.dp import GrpoDataParallel, _require_one_node
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dp = GrpoDataParallel()
+    _require_one_node(dp, device=-1)                              # both ranks really are on this machine
+    try:
+        _require_one_node(dp, identity=f"node-{rank}", device=-1)  # pretend they are not
+        q.put((rank, "no error"))
+    except RuntimeError as e:
+        q.put((rank, str(e)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_stitched_gradient_refuses_ranks_on_different_nodes():
+    """The stitched accumulator passes shard handles as file descriptors over Unix sockets: one machine only.  Ranks
+    on different machines get a clear error on EVERY rank instead of a hang in connect()."""
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_node_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for r in range(world):
+        assert "one node" in res[r] and "spans 2 nodes" in res[r]
