@@ -126,6 +126,108 @@ class GrpoDataParallel:
         return h
 
 
+# ---------------------------------------------------------------------- vocab (tensor) parallel
+def vocab_shard_bounds(V: int, world: int, multiple: int = 8) -> List[int]:
+    """Row bounds [v_0 = 0, v_1, ..., v_world = V] of the vocab shards: as even as possible, every inner bound a
+    multiple of `multiple` rows (keeps every shard 16-byte aligned for TMA whatever d is)."""
+    if world < 1 or V < world:
+        raise ValueError(f"cannot cut V={V} rows into {world} shards")
+    bounds = [0]
+    for r in range(1, world):
+        b = (V * r // world) // multiple * multiple
+        bounds.append(max(b, bounds[-1] + 1))
+    bounds.append(V)
+    return bounds
+
+
+class GrpoVocabParallel:
+    """Vocab-parallel (tensor-parallel) GRPO step (the paper's trainer ran TP = 4,
+    PAPER.md:197, which cuts the LM head by vocabulary rows).  Rank r owns rows [v0, v1) of W and of dW and a context
+    created with V = v1 - v0.  EVERY rank holds the same packed batch (hidden, targets, rewards, ...) - with TP the
+    transformer body's output is replicated - and after ``step`` every rank holds the same loss, metrics, logp and
+    the full dHidden; dW stays sharded by rows.
+
+    The exchange is two collectives per step: ONE all-gather of the per-token partials ([3, T] fp32 per rank:
+    running max, sum of 2^(z - max), target logit) and ONE sum all-reduce of the partial dHidden ([T, d] fp32).
+    Everything else runs in the library's kernels; this class only moves buffers (torch.distributed: NCCL on a GPU
+    box, gloo in the tests).  The loss / metrics accumulators are REPLICATED, never summed over the TP group.  Not
+    run or timed on more than one GPU."""
+
+    def __init__(self, d: int, V_global: int, process_group=None, make_context: bool = True,
+                 always_reduce: bool = False, **ctx_kw):
+        self.pg = process_group
+        self.always_reduce = always_reduce            # issue the collectives even in a one-rank group (tests)
+        self.world = dist.get_world_size(process_group) if dist.is_initialized() else 1
+        self.rank = dist.get_rank(process_group) if dist.is_initialized() else 0
+        self.d, self.V_global = d, V_global
+        self.bounds = vocab_shard_bounds(V_global, self.world)
+        self.v0, self.v1 = self.bounds[self.rank], self.bounds[self.rank + 1]
+        self.ctx = None
+        if make_context:
+            from .binding import GrpoContext
+            ctx_kw.setdefault("dhidden_fp32", 1)          # the partial dHidden is summed over ranks: keep it fp32
+            if not ctx_kw["dhidden_fp32"]:
+                raise ValueError("GrpoVocabParallel sums partial dHidden over ranks and needs dhidden_fp32=1")
+            self.ctx = GrpoContext(d, self.v1 - self.v0, **ctx_kw)
+
+    def close(self):
+        if self.ctx is not None:
+            self.ctx.close()
+            self.ctx = None
+
+    # ------------------------------------------------------------------ buffer plumbing
+    def shard_rows(self, W_full: torch.Tensor) -> torch.Tensor:
+        """This rank's rows of a full [V, d] matrix (a copy, contiguous)."""
+        return W_full[self.v0:self.v1].contiguous()
+
+    def local_targets(self, targets: torch.Tensor) -> torch.Tensor:
+        """Shard-local target ids: y - v0; ignored tokens (y < 0) stay ignored in every shard.  Ids that land outside
+        [0, v1 - v0) simply have no one-hot entry in this shard (include/grpo.h)."""
+        shifted = targets - self.v0
+        return torch.where(targets < 0, torch.full_like(targets, -1), shifted).contiguous()
+
+    def gather_partials(self, m2: torch.Tensor, s2: torch.Tensor, zy: torch.Tensor):
+        """ONE all-gather of this rank's [3, T] partials -> three contiguous [world, T] arrays in shard order, the
+        layout grpo_loss_from_partials reads."""
+        T = m2.numel()
+        mine = torch.stack((m2, s2, zy)).contiguous()                                # [3, T]
+        if self.world == 1 and not self.always_reduce:
+            everyone = mine.unsqueeze(0)
+        else:
+            flat = torch.empty(self.world * 3, T, dtype=mine.dtype, device=mine.device)    # ranks concatenated on dim 0
+            dist.all_gather_into_tensor(flat, mine, group=self.pg)
+            everyone = flat.view(self.world, 3, T)
+        by_kind = everyone.permute(1, 0, 2).contiguous()                             # [3, world, T]
+        return by_kind[0], by_kind[1], by_kind[2]
+
+    def reduce_dhidden(self, dH_partial: torch.Tensor) -> torch.Tensor:
+        """Sum of the ranks' partial dHidden, in place."""
+        if self.world > 1 or self.always_reduce:
+            dist.all_reduce(dH_partial, op=dist.ReduceOp.SUM, group=self.pg)
+        return dH_partial
+
+    # ------------------------------------------------------------------ the step
+    def step(self, hidden, W_shard, targets, cu_seqlens, rewards, G: int, old_logp, ref_logp=None, mask=None,
+             dW_shard_accum=None, loss_accum=None, metrics_accum=None, loss_denom: float = 0.0,
+             grad_scale: float = 1.0):
+        """A1 -> A2 on the shard -> all-gather -> A3 -> A4-A6 on the shard -> all-reduce of dHidden.
+        targets are GLOBAL ids.  Returns logp / lse / coeff / loss (replicated), dH (full, fp32) and adds the
+        shard's rows of dW into dW_shard_accum ([v1 - v0, d] fp32)."""
+        ctx = self.ctx
+        y_loc = self.local_targets(targets)
+        m2, s2, zy = ctx.grpo_vocab_shard_partials(hidden, W_shard, y_loc)
+        m2g, s2g, zyg = self.gather_partials(m2, s2, zy)
+        adv = ctx.grpo_group_advantage(rewards, G=G)
+        f = ctx.grpo_loss_from_partials(m2g, s2g, zyg, targets, self.V_global, cu_seqlens, adv, old_logp, ref_logp,
+                                        mask, loss_denom=loss_denom, loss_accum=loss_accum,
+                                        metrics_accum=metrics_accum)
+        dH = ctx.grpo_fused_logprob_loss_bwd(hidden, W_shard, y_loc, f["lse"], f["coeff"], dW_accum=dW_shard_accum,
+                                             grad_scale=grad_scale)
+        f["dH"] = self.reduce_dhidden(dH)
+        f["adv"] = adv
+        return f
+
+
 # ---------------------------------------------------------------------- fused GEMM -> reduce-scatter (stitched dW)
 class _RawCudaBuffer:
     """A raw device range exposed through __cuda_array_interface__ so that torch can alias it."""

@@ -159,6 +159,19 @@ def _nccl_worker(port, q):
     ok_sg = torch.equal(sg.full, ref["dW"]) and sg.local_rows == (0, b.V)
     sg.close()
     ctx.close()
+    # the vocab-parallel exchange on NCCL: all_gather_into_tensor of the [3, T] partials, all-reduce of dHidden
+    from paper_2606_26997_b200.dp import GrpoVocabParallel
+    vp = GrpoVocabParallel(b.d, b.V, always_reduce=True, max_tokens=b.T, eps_std=b.eps_std, clip_lo=b.clip_lo,
+                           clip_hi=b.clip_hi, kl_beta=b.kl_beta, loss_agg=b.loss_agg, group_size=b.G,
+                           bwd_chunk_tokens=1024)
+    dW_vp = torch.zeros(b.V, b.d, dtype=torch.float32, device="cuda")
+    g = vp.step(b.hidden, vp.shard_rows(b.W), b.targets, b.cu_seqlens, b.rewards, b.G, b.old_logp, b.ref_logp, b.mask,
+                dW_shard_accum=dW_vp)
+    torch.cuda.synchronize()
+    ok_vp = (vp.v0, vp.v1) == (0, b.V) and (g["logp"] - ref["logp"]).abs().max().item() <= 2e-5 and \
+        ((dW_vp - ref["dW"]).norm() / ref["dW"].norm()).item() <= 2e-3
+    vp.close()
+    ok_sg = ok_sg and ok_vp
     q.put((ok, ok_sg))
     dist.destroy_process_group()
 

@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 import torch
 
-from oracle.grpo_oracle import (OracleConfig, dH_rows, dW_rows, group_advantage, loss_terms, token_advantage,
+from oracle.grpo_oracle import (OracleConfig, backward, dH_rows, dW_rows, group_advantage, loss_terms, token_advantage,
                                 token_logprobs, token_rows)
 from tests.parity_util import (TOL_GRAD_REL, TOL_LOGP_ABS, TOL_LOSS_REL, _dense_part_rel, make_ctx, rel_l2, run_cuda,
                                to64, worst_block_rel)
@@ -125,6 +125,24 @@ def test_config2_full_size_bench_workload():
     dense_ref = dH_ref - entry[:, None] * Wy
     assert np.linalg.norm(dense_ref) < 0.1 * np.linalg.norm(dH_ref)
     assert _dense_part_rel(to64(dH32[torch.from_numpy(rows).cuda()]), dense_ref, entry, Wy) <= TOL_GRAD_REL
+    del dH32
+    # WHOLE-MATRIX gradient parity for the workload bench.py times (SURVEY.md section 8(d) cfg 2: the full oracle):
+    # every element of dH [18701, 2048] and dW [151936, 2048] against the float64 backward - a wrong 32 x 32
+    # reduce box, one wrong vocab tile or one wrong token row anywhere fails, not only on the sampled rows above.
+    dH_full, dW_full = backward(x["H"], x["W"], x["y"], lse, lt["coeff"], chunk_tokens=2048)
+    dH_all = to64(out["dH"])
+    assert rel_l2(dH_all, dH_full) <= TOL_GRAD_REL
+    rn = np.linalg.norm(dH_full, axis=1)
+    row_err = np.linalg.norm(dH_all - dH_full, axis=1) / np.maximum(rn, 1e-2 * np.median(rn[rn > 0]))
+    assert row_err.max() <= 2 * TOL_GRAD_REL, (int(row_err.argmax()), float(row_err.max()))
+    assert (dH_all[rn == 0] == 0).all()
+    del dH_all, dH_full
+    dW_all = out["dW"].cpu().numpy()
+    assert rel_l2(dW_all, dW_full) <= TOL_GRAD_REL
+    never = np.ones(b.V, dtype=bool)
+    never[tgt] = False
+    assert rel_l2(dW_all[never], dW_full[never]) <= TOL_GRAD_REL      # dense softmax term alone, all such rows
+    assert worst_block_rel(dW_all, dW_full, (32, 32)) <= 2 * TOL_GRAD_REL      # every 32 x 32 reduce box of A6
 
 
 # ------------------------------------------------------------------ configs[1] shape, LM-like logits, off-policy
@@ -191,6 +209,36 @@ def test_config3_full_size_sampled():
     _check_sampled(b, out, rows, _oracle_sampled(b, rows, float(b.T)))
     assert _colsum_rel(out["dW"]) <= 2e-3
     assert to64(out["metrics"])[0] == b.T
+    # full float64 forward (every token's lse / logp / coefficient), then oracle gradients that reach every tile of
+    # the backward: one dW row in EVERY 32-row reduce box of A6 (4 748 rows, at a position that moves through the
+    # box) and one dH row in every 256-row pair tile (285 rows) - `backward` restricted to those vocab rows / token
+    # rows, which is the full-batch term of each (lse and coeff come from the full forward).
+    x = b.numpy_f64()
+    lse, logp = token_logprobs(x["H"], x["W"], x["y"])
+    adv, _ = group_advantage(x["rewards"], G=b.G, eps_std=b.eps_std)
+    lt = loss_terms(logp, x["old_logp"], x["ref_logp"], None, token_advantage(adv, x["cu_seqlens"]), x["cu_seqlens"],
+                    _ocfg(b))
+    assert np.abs(to64(out["logp"]) - logp).max() <= TOL_LOGP_ABS
+    assert np.abs(to64(out["lse"]) - lse).max() <= TOL_LOGP_ABS
+    assert abs(out["loss"].item() - lt["loss"]) <= TOL_LOSS_REL * max(abs(lt["loss"]), lt["abs_loss"])
+    assert rel_l2(to64(out["coeff"]), lt["coeff"]) <= 1e-3
+    k = np.arange((b.V + 31) // 32)
+    vids = np.minimum(32 * k + (7 * k) % 32, b.V - 1)
+    pos = np.full(b.V, -1, dtype=np.int64)
+    pos[vids] = np.arange(len(vids))
+    y_sub = np.where(x["y"] >= 0, pos[np.clip(x["y"], 0, b.V - 1)], -1)      # one-hot only where the target is sampled
+    _, dW_ref = backward(x["H"], x["W"][vids], y_sub, lse, lt["coeff"], chunk_tokens=4096)
+    dW = to64(out["dW"][torch.from_numpy(vids).cuda()])
+    assert rel_l2(dW, dW_ref) <= TOL_GRAD_REL
+    assert worst_block_rel(dW, dW_ref, (1, 32)) <= 2 * TOL_GRAD_REL    # the sampled row's segment of every reduce box
+    trow = np.minimum(256 * np.arange((b.T + 255) // 256) + (37 * np.arange((b.T + 255) // 256)) % 256, b.T - 1)
+    dH_ref, _ = backward(x["H"][trow], x["W"], x["y"][trow], lse[trow], lt["coeff"][trow], chunk_tokens=512)
+    dH = to64(out["dH"][torch.from_numpy(trow).cuda()])
+    assert rel_l2(dH, dH_ref) <= TOL_GRAD_REL
+    rn = np.linalg.norm(dH_ref, axis=1)
+    row_err = np.linalg.norm(dH - dH_ref, axis=1) / np.maximum(rn, 1e-2 * np.median(rn[rn > 0]))
+    assert row_err.max() <= 2 * TOL_GRAD_REL
+    assert (dH[rn == 0] == 0).all()                                    # zero coefficient (beta > 0: only if masked)
 
 
 # ------------------------------------------------------------------ configs[3]: 8 x G=16 long tail, ~0.5M tokens

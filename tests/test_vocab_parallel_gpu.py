@@ -3,8 +3,17 @@ PAPER.md:197), emulated on ONE GPU: the vocab matrix is cut into row shards, eac
 shard) produces per-token (max, sum-exp, target-logit) partials, the gathered partials go through
 grpo_loss_from_partials, and every rank runs the backward on its shard with shard-local targets and the global
 lse / coeff.  Concatenated dW shards and the SUM of the partial dHidden must match the float64 oracle of the
-unsharded step within north_star's tolerances, and the unsharded CUDA path to fp32 noise.  The exchange itself (an
-all-gather of [T] x 3 floats and an all-reduce of [T, d]) is plain torch.distributed and is not exercised here."""
+unsharded step within north_star's tolerances, and the unsharded CUDA path to fp32 noise.  The exchange itself (ONE
+all-gather of [3, T] floats and ONE all-reduce of [T, d]) is `dp.py::GrpoVocabParallel`:
+`test_two_tp_ranks_run_the_exchange` runs its `step` in two processes on cuda:0 (gloo, as NCCL refuses two ranks on
+one device) against the oracle of the unsharded step; a one-rank NCCL group runs the NCCL calls
+(tests/test_dp_gpu.py)."""
+import os
+import socket
+import sys
+
+import torch.distributed as dist
+import torch.multiprocessing as mp
 import numpy as np
 import pytest
 import torch
@@ -75,3 +84,71 @@ def test_sharded_vocab_equals_the_unsharded_step(bounds, kw):
     assert (out["logp"] - full["logp"]).abs().max().item() <= 2e-5
     assert rel_l2(to64(out["dH"]), to64(full["dH"])) <= 2e-3 and rel_l2(to64(out["dW"]), to64(full["dW"])) <= 2e-3
     assert to64(out["metrics"])[3] == to64(full["metrics"])[3]
+
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _tp_batch():
+    return make_config(1, device="cuda", seed=11, variant="1b", n_groups=4, G=4, d=128, V=3000, len_div=0.2, w_std=0.1,
+                       mask_frac=0.2, bad_target_frac=0.1, kl_beta=0.02)
+
+
+def _tp_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2606_26997_b200.dp import GrpoVocabParallel
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    b = _tp_batch()                                                     # replicated batch, as the TP body leaves it
+    vp = GrpoVocabParallel(b.d, b.V, max_tokens=b.T, eps_std=b.eps_std, clip_lo=b.clip_lo, clip_hi=b.clip_hi,
+                           kl_beta=b.kl_beta, loss_agg=b.loss_agg, group_size=b.G, bwd_chunk_tokens=1024)
+    W_shard = vp.shard_rows(b.W)
+    dW_shard = torch.zeros(vp.v1 - vp.v0, b.d, dtype=torch.float32, device="cuda")
+    loss = torch.zeros(1, dtype=torch.float32, device="cuda")
+    metrics = torch.zeros(4, dtype=torch.float32, device="cuda")
+    f = vp.step(b.hidden, W_shard, b.targets, b.cu_seqlens, b.rewards, b.G, b.old_logp, b.ref_logp, b.mask,
+                dW_shard_accum=dW_shard, loss_accum=loss, metrics_accum=metrics)
+    torch.cuda.synchronize()
+    assert vp.ctx.grpo_check_errors_sync() == 0
+    q.put((rank, vp.v0, vp.v1, dW_shard.cpu().numpy(), f["dH"].cpu().numpy(), f["logp"].cpu().numpy(),
+           f["coeff"].cpu().numpy(), float(loss.item()), metrics.cpu().numpy()))
+    vp.close()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def test_two_tp_ranks_run_the_exchange():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_tp_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((q.get(timeout=600) for _ in range(world)), key=lambda r: r[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    b = _tp_batch()
+    ref = run_oracle(b)
+    assert [(r[1], r[2]) for r in res] == [(0, 1496), (1496, 3000)]
+    dW = np.concatenate([r[3] for r in res])                            # dW stays sharded by rows
+    assert rel_l2(dW, ref["dW"]) <= TOL_GRAD_REL
+    for rank, v0, v1, dW_r, dH, logp, coeff, loss, metrics in res:
+        assert rel_l2(dW_r, ref["dW"][v0:v1]) <= TOL_GRAD_REL
+        assert rel_l2(dH, ref["dH"]) <= TOL_GRAD_REL                    # the all-reduced, full dHidden
+        assert np.abs(logp - ref["logp"]).max() <= TOL_LOGP_ABS
+        assert rel_l2(coeff, ref["coeff"]) <= 1e-3
+        assert abs(loss - ref["loss"]) <= TOL_LOSS_REL * max(abs(ref["loss"]), ref["abs_loss"])   # replicated, not summed
+        np.testing.assert_allclose(metrics, ref["metrics"], rtol=1e-4, atol=1e-3)
+    for k in (4, 5, 6, 8):                                              # every rank ends with the same bits
+        np.testing.assert_array_equal(res[0][k], res[1][k])
+    assert res[0][7] == res[1][7]
