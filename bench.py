@@ -161,6 +161,44 @@ class ClockSampler:
         return out
 
 
+def cublas_anchor(torch_index: int, seconds: float = 1.0):
+    """Same-run, same-box anchor for the roofline fraction: ~`seconds` of back-to-back torch.matmul (cuBLAS) bf16
+    8192 x 8192 x 2048 with N(0,1) operands on this device, outside every timed region, with its own clock sample.
+    MEASURED_PEAKS.json was taken on another lease (other clocks under the same power cap); this is the library's
+    rate on THIS board at THIS moment, so kernel TFLOP/s divided by it does not move with the box."""
+    import torch
+    dev = torch.device("cuda", torch_index)
+    M = N = 8192
+    K = 2048
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(7)
+    A = torch.randn(M, K, generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    B = torch.randn(N, K, generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    C = torch.empty(M, N, device=dev, dtype=torch.bfloat16)
+    fn = lambda: torch.matmul(A, B.t(), out=C)
+    for _ in range(20):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(20):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    n = max(20, int(seconds * 1e3 / (e0.elapsed_time(e1) / 20)))
+    sampler = ClockSampler(torch_index)
+    sampler.start()
+    e0.record()
+    for _ in range(n):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / n
+    return {"tflops": 2.0 * M * N * K / ms / 1e9, "shape": [M, N, K], "calls": n, "seconds": ms * n * 1e-3,
+            "api": "torch.matmul bf16 (cuBLAS), N(0,1) operands", "clocks": clocks}
+
+
 # ----------------------------------------------------------------------------------------- oracle legs
 def oracle_sample(device="cpu", len_div=SAMPLE_LEN_DIV):
     """Bounded sample of the timed workload for the CPU oracle: configs[1] with lengths / len_div."""
@@ -463,6 +501,12 @@ def run_ours(args):
                               "value": v_tok * args.steps / (v_ms * 1e-3), "unit": UNIT,
                               "ms_per_step": v_ms / args.steps}
 
+    # ---- same-run cuBLAS anchor (outside every timed region): the roofline fraction against the library's rate on
+    # this board, now
+    args.cublas_anchor = None
+    if world == 1 and not args.no_anchor:
+        args.cublas_anchor = cublas_anchor(local)
+
     # ---- informational runs (--config 3/4/5, --prenorm) are device-resident: no e2e / cpu_baseline legs
     if args.informational:
         ms_total, _, tokens_all = reduce_over_ranks(ms_total, 0.0, T, world, dev)
@@ -756,6 +800,14 @@ def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, p
                                                                        "contraction (3 recompute / 2 stash); 8*T*V*d for "
                                                                        "the north_star path when no tile is skipped"},
     }
+    anchor = getattr(args, "cublas_anchor", None)
+    if anchor:
+        roofline["same_run_cublas_tflops"] = anchor["tflops"]
+        roofline["frac_of_same_run_cublas"] = dom_tflops / anchor["tflops"]
+        roofline["all_gemms"]["frac_of_same_run_cublas"] = path_tflops / anchor["tflops"]
+        if roofline["whole_step"] is not None:
+            roofline["whole_step"]["frac_of_same_run_cublas"] = step_tflops / anchor["tflops"]
+        roofline["same_run_cublas"] = anchor
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -822,6 +874,8 @@ def main():
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-energy", action="store_true", help="skip the >= 2 s NVML energy leg (profiling runs)")
+    ap.add_argument("--no-anchor", action="store_true",
+                    help="skip the ~1 s same-run cuBLAS bf16 matmul leg (roofline.same_run_cublas_tflops)")
     ap.add_argument("--power-study", action="store_true",
                     help="informational: the step and cuBLAS on their operands vs all-zero operands (what the data costs "
                          "under the board power cap)")

@@ -128,7 +128,9 @@ int32_t grpo_group_advantage(grpo_ctx* ctx, const float* rewards, const int32_t*
 /* A2 + A3.  targets int32 [T] (<0: token ignored; >=V: ignored and an error bit is raised, see
  * grpo_check_errors_sync).  adv fp32 [S].  old_logp fp32 [T].  ref_logp fp32 [T] or NULL (no KL).
  * mask u8 [T] or NULL (all ones).  loss_denom > 0: explicit denominator of the whole logical update
- * (loss_agg 0); <= 0: max(sum of this call's mask, 1).
+ * (loss_agg 0); <= 0: max(sum of this call's mask, 1), counted on the device in fp32 - exact up to 2^24 tokens, so a
+ * call (or a grpo_enqueue_groups update) of more than 16 777 216 tokens without an explicit loss_denom is
+ * GRPO_ERR_SHAPE and nothing runs.
  * Outputs: logp_out, lse_out, coeff_out fp32 [T] (coeff_t = d loss / d logp_t, consumed by bwd);
  * loss_accum fp32 [1] is ADDED to; metrics_accum fp32 [4] or NULL is ADDED to:
  * {loss-bearing tokens, sum rho, sum k3, tokens whose policy gradient is clipped}. */

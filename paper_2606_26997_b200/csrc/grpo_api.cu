@@ -592,7 +592,12 @@ struct FwdArgs {
   float* logp_out; float* lse_out; float* coeff_out; float* loss_accum; float* metrics_accum;
   float* entropy_out = nullptr;   // nullable (grpo_set_entropy_out)
   int32_t S_norm = 0;             // loss_agg 1: sequences of the WHOLE logical update (0: this call's S)
+  int64_t T_call = 0;             // packed tokens of the call (bounds the fp32 token count of an implicit denominator)
 };
+
+// The loss-bearing token count behind an IMPLICIT token-mean denominator is accumulated in fp32 on the device, which
+// is exact up to 2^24 tokens; larger calls must state loss_denom (include/grpo.h).
+static const int64_t kMaxCountedTokens = int64_t(1) << 24;
 
 static int32_t fwd_check(grpo_ctx* ctx, int32_t S, int64_t T) {
   if (!ctx->ws) return fail(GRPO_ERR_WORKSPACE, "no workspace set (grpo_set_workspace)");
@@ -611,6 +616,9 @@ static int32_t fwd_counts(grpo_ctx* ctx, int slot, const int32_t* targets, const
   float* total = slot_ptr<float>(ctx, slot, L.off_total);
   float* seq_count = slot_ptr<float>(ctx, slot, L.off_seq_count);
   const bool implicit_denom = c.loss_agg == 0 && !(a.loss_denom > 0.0) && a.denom_dev == nullptr;
+  if (implicit_denom && a.T_call > kMaxCountedTokens)
+    return fail(GRPO_ERR_SHAPE, "T=%lld: the token-mean denominator is counted in fp32, exact only up to 2^24 tokens; "
+                "pass loss_denom > 0 for a call this large", (long long)a.T_call);
   if (c.loss_agg == 1 || implicit_denom) {
     CU_OK(cudaMemsetAsync(total, 0, 4, st));
     const int threads = 128;
@@ -740,6 +748,7 @@ static int32_t fwd_impl(grpo_ctx* ctx, int slot, const void* hidden, const void*
             logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
   a.entropy_out = entropy_out;
   a.S_norm = S_norm;
+  a.T_call = T;
   GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
   // A2 + A3 in launches of at most fwd_block_rows rows: bounds the LSE partial buffers; a row's result does not
   // depend on how the call is cut (fixed vocab split)
@@ -819,6 +828,7 @@ extern "C" int32_t grpo_loss_from_partials(grpo_ctx* ctx, int32_t n_shards, cons
   FwdArgs a{cu_seqlens, S, adv, old_logp, ref_logp, mask, loss_denom, nullptr,
             logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
   a.S_norm = ctx->seq_denom;
+  a.T_call = T;
   GRPO_TRY(fwd_counts(ctx, 0, targets, a, st, V_global));
   return loss_rows(ctx, 0, m2, s2, nullptr, n_shards, T, zy, n_shards, T, V_global, targets, a, 0, T, st);
 }
@@ -1146,6 +1156,7 @@ extern "C" int32_t grpo_fused_logprob_loss_fwd_bwd(grpo_ctx* ctx, const void* hi
             logp_out, lse_out, coeff_out, loss_accum, metrics_accum};
   a.entropy_out = ctx->entropy_out;
   a.S_norm = ctx->seq_denom;
+  a.T_call = T;
   GRPO_TRY(fwd_counts(ctx, 0, targets, a, st));
   return bwd_impl(ctx, 0, hidden, W, targets, lse_out, coeff_out, T, grad_scale, dhidden_out, dW_accum, st, &a);
 }
@@ -1324,6 +1335,7 @@ static int32_t run_launch(grpo_ctx* ctx, const PendingGroup* groups, int k, cons
     FwdArgs a{d_cu_seq, S, d_adv, old_logp, ref_logp, mask, loss_denom, denom_dev,
               logp, lse, coeff, loss_accum, metrics_accum};
     a.S_norm = S_update;
+    a.T_call = T;
     GRPO_TRY(fwd_counts(ctx, slot, targets, a, st));
     GRPO_TRY(bwd_impl(ctx, slot, hidden, W, targets, lse, coeff, T, 1.0f, dh, dW_accum, st, &a));
   } else {
@@ -1383,6 +1395,13 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
 
   // implicit denominator of the whole update: count loss-bearing tokens of all its groups first
   const float* denom_dev = nullptr;
+  if (ctx->cfg.loss_agg == 0 && !(loss_denom > 0.0)) {   // fp32 count on the device: exact up to 2^24 tokens
+    int64_t T_update = 0;
+    for (const auto& g : upd) T_update += g.tokens;
+    if (T_update > kMaxCountedTokens)
+      return fail(GRPO_ERR_SHAPE, "update of %lld tokens: the token-mean denominator is counted in fp32, exact only "
+                  "up to 2^24 tokens; pass loss_denom > 0 for an update this large", (long long)T_update);
+  }
   if (ctx->cfg.loss_agg == 0 && !(loss_denom > 0.0) && sizes.size() > 1) {
     float* dd = ctx->denom_ring + (ctx->denom_next++ % kDenomRing);
     cudaStream_t s0 = static_cast<cudaStream_t>(streams ? streams[ctx->launches % n_streams] : nullptr);
@@ -1535,8 +1554,9 @@ extern "C" int32_t grpo_step_host(grpo_ctx* ctx, const void* hidden_host, const 
   CU_OK(cudaMemsetAsync(loss_dev, 0, 4, st));
   GRPO_TRY(grpo_group_advantage(ctx, d_rw, nullptr, n_groups, G, d_adv, nullptr, st));
   GRPO_TRY(fwd_check(ctx, S, T));
-  const FwdArgs a{d_cu, S, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr, loss_denom, nullptr,
-                  logp, lse, coeff, loss_dev, nullptr};
+  FwdArgs a{d_cu, S, d_adv, so, ref_logp_host ? sr : nullptr, mask_host ? sm : nullptr, loss_denom, nullptr,
+            logp, lse, coeff, loss_dev, nullptr};
+  a.T_call = T;
   GRPO_TRY(fwd_counts(ctx, 0, stg, a, st));
   if (c.stash_logits) {
     GRPO_TRY(bwd_impl(ctx, 0, sh, W, stg, lse, coeff, T, 1.0f, dhidden_host ? dh : nullptr, dW_accum, st, &a, &pipe));

@@ -303,3 +303,29 @@ def test_wide_hidden_size_walks_its_units_in_l2_sized_groups():
     b = make_config(4, device="cuda", seed=2, d=4352, V=1500, len_div=38.0, w_std=0.05, old_sigma=0.3, mask_frac=0.1)
     assert b.T > 9500
     _check(b)
+
+
+def test_implicit_token_mean_beyond_2_24_tokens_is_refused():
+    """The loss-bearing token count behind an implicit denominator is an fp32 sum on the device: exact only up to
+    2^24 tokens.  A larger call without loss_denom is refused (GRPO_ERR_SHAPE) before anything is launched; with an
+    explicit denominator the same call runs (W = 0: uniform softmax, logp = -ln V for every token)."""
+    from paper_2606_26997_b200 import GrpoContext, GrpoError
+    T, d, V = (1 << 24) + 8, 8, 8
+    ctx = GrpoContext(d, V, max_tokens=T)
+    assert ctx.workspace_bytes(T) < 8 << 30
+    z = lambda *shape, dt=torch.float32: torch.zeros(*shape, dtype=dt, device="cuda")
+    hidden, W, y = z(T, d, dt=torch.bfloat16), z(V, d, dt=torch.bfloat16), z(T, dt=torch.int32)
+    cu = torch.tensor([0, T], dtype=torch.int32, device="cuda")
+    adv, old = torch.ones(1, device="cuda"), torch.full((T,), -float(np.log(V)), device="cuda")
+    loss = z(1)
+    with pytest.raises(GrpoError) as e:
+        ctx.grpo_fused_logprob_loss_fwd(hidden, W, y, cu, adv, old, loss_accum=loss)
+    assert e.value.status == 2 and "2^24" in str(e.value)
+    torch.cuda.synchronize()
+    assert loss.item() == 0.0                                          # nothing ran
+    f = ctx.grpo_fused_logprob_loss_fwd(hidden, W, y, cu, adv, old, loss_denom=float(T), loss_accum=loss)
+    torch.cuda.synchronize()
+    assert ctx.grpo_check_errors_sync() == 0
+    assert (f["logp"] + float(np.log(V))).abs().max().item() <= 1e-6
+    assert abs(loss.item() + 1.0) <= 1e-3                              # rho = 1, A = 1: loss = -mean(rho A) = -1
+    ctx.close()
