@@ -329,6 +329,8 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.dp:
+        return run_dp(args, dev, rank, world, local)
     if args.power_study:
         assert world == 1, "--power-study is a one-GPU informational run"
         return run_power_study(args, dev)
@@ -748,6 +750,122 @@ def run_cgp_stream(args, b, dev, world):
     return 0
 
 
+def dp_update_plan(world: int, groups_per_rank: int):
+    """The logical update of the --dp arm: world x groups_per_rank complete groups in FIFO order, dealt by position
+    (k mod world) as GrpoDataParallel does; returns per rank the update positions it trains (host logic, unit-tested
+    under gloo in tests/test_multirank_cpu.py)."""
+    from paper_2606_26997_b200.dp import assign_groups
+    U = world * groups_per_rank
+    return U, [assign_groups(U, world, r) for r in range(world)]
+
+
+def run_dp(args, dev, rank, world, local):
+    """--dp allreduce|stitched (informational): ONE logical update of
+    world x k complete groups (configs[1] groups: G = 8, lengths U[512, 4096]) dealt to the ranks by
+    GrpoDataParallel; every rank trains its k groups through grpo_enqueue_groups with the update's global
+    denominator, then the update boundary reduces dW / loss / metrics over the ranks.  tokens/s INCLUDES the
+    reduction: `allreduce` = asynchronous NCCL all-reduce on a side stream into alternating buffer sets (the next
+    update's contractions overlap it; --dp-max-ctas leaves SMs to it), `stitched` = the A6 reduce-adds go straight
+    into the rank-sharded accumulator (StitchedGradient) and the boundary is a barrier.  With one rank the
+    collectives are still issued (always_reduce), so the line measures their fixed cost, not NVLink."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_26997_b200 import GrpoContext
+    from paper_2606_26997_b200.dp import GrpoDataParallel, StitchedGradient
+    from workloads.synth import make_config
+    k = args.dp_groups
+    if world == 1 and not dist.is_initialized():          # a one-rank NCCL group: the real collective calls still run
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29517")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    U, plan = dp_update_plan(world, k)
+    b = make_config(2, seed=rank_seed(rank), device=dev, n_groups=k)      # this rank's k groups of the update
+    dp = GrpoDataParallel(always_reduce=True)
+    gtok = [b.group_token_range(g)[1] - b.group_token_range(g)[0] for g in range(k)]
+    denom = dp.global_denominator(b.T)                                      # token mean over the WHOLE update
+    extra = {"gemm_max_ctas": args.dp_max_ctas} if args.dp_max_ctas else {}
+    ctx = GrpoContext(b.d, b.V, max_tokens=max(gtok), group_size=b.G, kl_beta=b.kl_beta, clip_lo=b.clip_lo,
+                      clip_hi=b.clip_hi, groups_per_update=k, token_budget=max(gtok), **extra)
+    dH = torch.empty(b.T, b.d, dtype=torch.bfloat16, device=dev)
+
+    def descs():
+        out = []
+        for g in range(k):
+            t0, t1 = b.group_token_range(g)
+            out.append(ctx.make_group_desc(plan[rank][g], b.seqlens[g * b.G:(g + 1) * b.G], b.hidden[t0:t1],
+                                           b.targets[t0:t1], b.old_logp[t0:t1],
+                                           b.rewards[g * b.G:(g + 1) * b.G].contiguous(),
+                                           None if b.ref_logp is None else b.ref_logp[t0:t1], None, dH[t0:t1], None))
+        return out
+
+    compute = torch.cuda.current_stream()
+    sg = StitchedGradient(ctx, b.V, b.d, dp) if args.dp == "stitched" else None
+    loss_s = torch.zeros(1, dtype=torch.float32, device=dev)
+    pending = []
+
+    def step():
+        if sg is not None:
+            loss_s.zero_()
+            _, boundary = ctx.grpo_enqueue_groups(descs(), b.W, sg.full, loss_s, loss_denom=denom)
+            assert boundary
+            sg.barrier()                                   # every rank's reduce-adds have landed: rows are final
+            sg.local.zero_()                               # (the optimizer would consume them here)
+            return
+        dW, loss, metrics = dp.buffers(b.V, b.d, device=dev)
+        if len(pending) == 2:                              # the set's previous reduction must have finished
+            pending.pop(0).wait(compute)
+        dW.zero_(); loss.zero_(); metrics.zero_()
+        _, boundary = ctx.grpo_enqueue_groups(descs(), b.W, dW, loss, metrics, loss_denom=denom)
+        assert boundary
+        pending.append(dp.reduce_boundary(dW, loss, metrics, compute_stream=compute))
+
+    def drain():
+        while pending:
+            pending.pop(0).wait(compute)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    drain()
+    torch.cuda.synchronize()
+    dist.barrier()
+    assert ctx.grpo_check_errors_sync() == 0
+    sampler = ClockSampler(local)
+    n0 = ctx.grpo_kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    drain()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    dist.barrier()
+    n1 = ctx.grpo_kernel_launches()
+    ms, _, tokens_all = reduce_over_ranks(e0.elapsed_time(e1), 0.0, b.T, world, dev)
+    if rank == 0:
+        line = {"metric": METRIC, "value": tokens_all * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "informational": "dp",
+                "config": {"workload": f"one logical update of U = {U} configs[1]-style complete groups (G = 8, lengths "
+                                       f"U[512, 4096], d = {b.d}, V = {b.V}) dealt {k} per rank; boundary reduction "
+                                       "INSIDE the timed region",
+                           "parallelism": f"dp{world} {args.dp}" + (f", gemm_max_ctas={args.dp_max_ctas}" if args.dp_max_ctas else ""),
+                           "tokens_per_step": int(tokens_all), "tokens_rank0": b.T, "groups_per_rank": k,
+                           "boundary_bytes_per_rank": 4 * b.V * b.d,
+                           "l2": "inputs larger than L2 (W 622 MB, dW 1.2 GB); no flush needed"},
+                "e2e": None, "gpu_launches": sum(n1.values()) - sum(n0.values()), "clocks": clocks,
+                "note": "world 1: the collectives run in a one-rank NCCL group (fixed cost only); nothing here has "
+                        "been timed on more than one GPU" if world == 1 else "max over ranks, device-timed"}
+        print(json.dumps(line), flush=True)
+    if sg is not None:
+        sg.close()
+    ctx.close()
+    dist.destroy_process_group()
+    return 0
+
+
 def build_line(args, b, world, value, ms_total, e2e_value, h2d, d2h, launches, prof, clocks, peaks, tokens_all,
                loss_val):
     T, d, V = b.T, b.d, b.V
@@ -874,6 +992,12 @@ def main():
     ap.add_argument("--bwd-chunk", type=int, default=0, help="grpo_config.bwd_chunk_tokens (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-energy", action="store_true", help="skip the >= 2 s NVML energy leg (profiling runs)")
+    ap.add_argument("--dp", choices=["allreduce", "stitched"], default=None,
+                    help="informational multi-GPU arm: one logical update of N x k complete groups dealt by "
+                         "GrpoDataParallel, tokens/s including the boundary reduction (DESIGN.md section 7)")
+    ap.add_argument("--dp-groups", type=int, default=2, help="--dp: complete groups per rank and update (k)")
+    ap.add_argument("--dp-max-ctas", type=int, default=0,
+                    help="--dp: gemm_max_ctas of the contraction kernels (leave SMs to the collective); 0 = all SMs")
     ap.add_argument("--no-anchor", action="store_true",
                     help="skip the ~1 s same-run cuBLAS bf16 matmul leg (roofline.same_run_cublas_tflops)")
     ap.add_argument("--power-study", action="store_true",

@@ -290,11 +290,15 @@ typedef struct {
  * HOST outputs: groups_consumed_out (total consumed so far), update_boundary_out (1 if an update was
  * run by this call: the caller may step the optimizer and zero dW once the streams reach this work).
  * n = 0 is allowed (continue draining the FIFO). */
-/* Errors leave the accumulators consistent: everything that can be rejected without the device (workspace
- * capacity, ref_logp given for some groups of a launch only) is checked for EVERY launch of the update before the
- * first kernel is enqueued - nothing is accumulated and the FIFO is unchanged.  If a launch fails later
- * (GRPO_ERR_CUDA), the groups of the launches already enqueued are consumed (groups_consumed_out counts them) and
- * the rest of the update stays at the head of the FIFO, so a retry never adds a group twice. */
+/* Errors: everything that can be rejected without the device (workspace capacity, ref_logp given for some groups
+ * of a launch only, an implicit denominator over more than 2^24 tokens) is checked for EVERY launch of the update
+ * before the first kernel is enqueued - nothing is accumulated and the FIFO is unchanged.  If a launch fails later
+ * (a CUDA error while enqueueing), the update is BROKEN: the launches already enqueued have added their share -
+ * scaled by this update's denominator - to dW / loss / metrics, kernels of the failed launch may have too, and the
+ * accumulators no longer hold a whole number of groups.  The context then refuses every further grpo_enqueue_groups
+ * / grpo_flush (GRPO_ERR_CUDA) until the caller has discarded the update - zero dW_accum / loss_accum /
+ * metrics_accum - and called grpo_reset_round, which empties the FIFO (groups_consumed_out says how many groups of
+ * the round had been consumed); the caller resubmits what the round still needs. */
 int32_t grpo_enqueue_groups(grpo_ctx* ctx, const grpo_group_desc* groups, int32_t n, const void* W,
                             float* dW_accum, float* loss_accum, float* metrics_accum, double loss_denom,
                             void* const* streams, int32_t n_streams, int32_t* groups_consumed_out,

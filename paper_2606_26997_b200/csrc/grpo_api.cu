@@ -113,6 +113,7 @@ struct grpo_ctx {
   std::deque<PendingGroup> fifo;
   int64_t launches = 0;
   int32_t consumed = 0;
+  bool update_broken = false;    // a launch failed after part of its update was enqueued (see drain_one_update)
   // kernel accounting (always) and per-launch CUDA-event timing (only while profiling is on)
   int64_t kernel_count[GRPO_NUM_KERNEL_KINDS] = {0};
   bool profiling = false;
@@ -1192,6 +1193,7 @@ extern "C" int32_t grpo_reset_round(grpo_ctx* ctx) {
   if (!ctx) return fail(GRPO_ERR_INVALID_ARG, "ctx is NULL");
   ctx->fifo.clear();
   ctx->consumed = 0;
+  ctx->update_broken = false;
   return GRPO_OK;
 }
 
@@ -1362,6 +1364,10 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
                                 float* metrics_accum, double loss_denom, void* const* streams, int32_t n_streams,
                                 int32_t* boundary) {
   *boundary = 0;
+  if (ctx->update_broken)
+    return fail(GRPO_ERR_CUDA, "an earlier launch failed in the middle of a logical update: its partial sums are in the "
+                "accumulators and were scaled by that update's denominator; discard the update (zero dW / loss / "
+                "metrics), then call grpo_reset_round and resubmit the round's remaining groups");
   if (ctx->fifo.empty()) return GRPO_OK;
   std::vector<int64_t> tokens;
   tokens.reserve(ctx->fifo.size());
@@ -1430,6 +1436,10 @@ static int32_t drain_one_update(grpo_ctx* ctx, bool flush, const void* W, float*
       // cannot add them twice; the failed launch and the rest of the update stay at the head of the FIFO
       ctx->fifo.erase(ctx->fifo.begin(), ctx->fifo.begin() + pos);
       ctx->consumed += pos;
+      // the rest of the update cannot simply be re-planned: it would get a new boundary, denominator and sequence
+      // count, and kernels of the failed launch may already have added to the accumulators.  Refuse further
+      // dispatch until the caller has discarded the update (grpo_reset_round).
+      if (rc == GRPO_ERR_CUDA || pos > 0) ctx->update_broken = true;
       return rc;
     }
     ctx->launches++;

@@ -79,3 +79,15 @@ def test_ours_arm_fails_loudly_without_cuda():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "1"],
                        capture_output=True, text=True, timeout=300)
     assert r.returncode != 0 and "no CUDA device" in (r.stderr + r.stdout)
+
+
+def test_dp_arm_deals_the_update_by_fifo_position():
+    """bench.py --dp: one logical update of world x k groups, dealt k mod world like GrpoDataParallel; every position
+    is trained by exactly one rank."""
+    sys.path.insert(0, ROOT)
+    import bench
+    U, plan = bench.dp_update_plan(2, 3)
+    assert U == 6 and plan == [[0, 2, 4], [1, 3, 5]]
+    U, plan = bench.dp_update_plan(8, 2)
+    assert U == 16 and sorted(p for r in plan for p in r) == list(range(16)) and all(len(r) == 2 for r in plan)
+    assert bench.dp_update_plan(1, 2) == (2, [[0, 1]])
