@@ -40,7 +40,7 @@ UNIT = "tokens/s"
 SAMPLE_LEN_DIV = 8.0           # cpu_baseline leg: T ~ 2.3k tokens
 REF_SAMPLE_LEN_DIV = 32.0      # --impl reference arm: T ~ 580 tokens per step
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.txt")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r03_traffic.txt")
 KERNEL_SOURCES = ("gemm_sm100.cuh", "ptx_sm100.cuh", "token_kernels.cuh", "grpo_api.cu")
 
 
@@ -56,7 +56,7 @@ def kernel_source_hash():
 
 def load_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of each contraction kernel, from the committed
-    `ncu --set full` capture (profiles/r02_traffic.txt: `key value` lines, written from the capture's raw page).
+    `ncu --set full` capture (profiles/r03_traffic.txt: `key value` lines, written from the capture's raw page).
     The capture names the source hash of the build it profiled; a capture of ANOTHER build is not reported as this
     build's traffic: the figure is dropped (null) and the mismatch is said on stderr and in the JSON line."""
     if not os.path.exists(TRAFFIC_FILE):
@@ -69,11 +69,11 @@ def load_traffic():
                 vals[line[0]] = line[1]
     have = kernel_source_hash()
     if vals.get("kernel_source_hash") != have:
-        msg = (f"profiles/r02_traffic.txt is a capture of build {vals.get('kernel_source_hash')}, this build is {have}: "
+        msg = (f"profiles/r03_traffic.txt is a capture of build {vals.get('kernel_source_hash')}, this build is {have}: "
                "roofline.traffic dropped (re-run the ncu capture)")
         print("bench.py: " + msg, file=sys.stderr)
         return {}, msg
-    return {k: float(v) for k, v in vals.items() if k.startswith("gemm_")}, "profiles/r02_traffic.txt"
+    return {k: float(v) for k, v in vals.items() if k.startswith("gemm_")}, "profiles/r03_traffic.txt"
 
 
 def load_peaks():
