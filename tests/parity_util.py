@@ -3,7 +3,7 @@ same bits, and compute the gates of BASELINE.json north_star plus the sub-block 
 import numpy as np
 import torch
 
-from oracle.grpo_oracle import OracleConfig, grpo_step
+from oracle.grpo_oracle import OracleConfig, grpo_step, round_to_bf16
 
 TOL_LOGP_ABS = 2e-3      # per-token log-prob abs err (north_star)
 TOL_LOSS_REL = 1e-3      # loss rel err, relative to max(|loss|, sum |w l|) (R21)
@@ -63,11 +63,7 @@ def to64(t):
     return t.detach().double().cpu().numpy()
 
 
-def bf16_round(x):
-    """float64 -> nearest bf16 (ties to even), returned as float64."""
-    u = np.asarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)
-    u = ((u + 0x7FFF + ((u >> 16) & 1)) >> 16) << 16
-    return u.astype(np.uint32).view(np.float32).astype(np.float64)
+bf16_round = round_to_bf16      # float64 -> nearest bf16 (ties to even) as float64: the oracle's, pinned against torch
 
 
 def _bf16_neighbours(x):
